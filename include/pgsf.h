@@ -1,0 +1,162 @@
+/*
+ * pgsf.h -- C ABI of the B200-native hot path of the filter-based HI source finder of
+ * arXiv 1507.04941 (Westerlund & Harris, "Performance Analysis of GPU-Accelerated Filter-Based
+ * Source Finding for HI Spectral Line Image Data").
+ *
+ * Citations "P:<n>" are line numbers of the paper text; "C-<n>" are the readings
+ * listed in DESIGN.md where the paper is silent.
+ *
+ * What the path computes:
+ *   for every Gaussian scale s of a filter bank:
+ *     f_s  = 3-D convolution of the cube d with the outer-product Gaussian of sigma_s     (Eq. 2)
+ *     m, sd = mean and standard deviation of f_s over a box around every voxel
+ *     mask |= f_s > m + k * sd
+ *   count = number of set mask voxels.
+ *
+ * Data layout (C-0): a cube is nx*ny*nz fp32 values, linear index x + nx*(y + ny*z): x (right
+ * ascension) is unit stride, z (frequency) is the slowest axis; `batch` cubes follow each other
+ * with stride nx*ny*nz.  Masks use the same indexing with one byte per voxel.
+ *
+ * Ownership: every cube / mask / count / workspace pointer named d_* is a caller-owned DEVICE
+ * pointer (e.g. a torch tensor's data_ptr()); h_* are HOST pointers.  The library never frees
+ * caller memory, never writes d_in, and allocates only its own small constants (plus, for the
+ * *_host entry point, plan-owned staging buffers released by pgsf_plan_destroy).
+ *
+ * Execution: calls validate on the host, enqueue work on `cuda_stream` (a cudaStream_t passed as
+ * void*; NULL = the legacy default stream) and return WITHOUT synchronising; results (including
+ * *d_count) are valid once the caller has synchronised the stream.  pgsf_find_multiscale_host is
+ * the exception: it synchronises before returning.  One plan must not be used from two threads
+ * at once.
+ *
+ * Errors: every call returns a pgsf_status; nothing throws or aborts across the ABI.  The text of
+ * the last error of a plan is available from pgsf_last_error().  There is no CPU fallback: on a
+ * machine without a CUDA device pgsf_plan_create returns PGSF_ERR_CUDA.
+ */
+#ifndef PGSF_H
+#define PGSF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define PGSF_API __attribute__((visibility("default")))
+#else
+#define PGSF_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pgsf_plan pgsf_plan; /* opaque host object */
+
+typedef enum {
+    PGSF_OK = 0,
+    PGSF_ERR_INVALID_ARG = 1, /* null / misaligned pointer, bad extent, scale out of range, ... */
+    PGSF_ERR_UNSUPPORTED = 2, /* radius or box above the supported maximum, device not sm_100 */
+    PGSF_ERR_OOM = 3,         /* an internal allocation failed */
+    PGSF_ERR_CUDA = 4         /* a CUDA runtime call failed; see pgsf_last_error */
+} pgsf_status;
+
+/* plan flags */
+#define PGSF_FLAG_FORCE_GENERIC 0x1u /* use only the generic (any shape / any radius) kernels */
+
+#define PGSF_MAX_SCALES 8
+#define PGSF_MAX_RADIUS 96 /* largest supported ceil(truncate*sigma) on any axis */
+#define PGSF_MAX_BOX_HALF 128
+
+typedef struct {
+    int32_t nx, ny, nz;   /* extents of ONE cube INCLUDING any halo; x is unit stride (C-0)       */
+    int32_t batch;        /* >= 1 identically shaped cubes, stride nx*ny*nz elements              */
+    int32_t halo[3];      /* (x,y,z) voxels next to each face excluded from mask and count (C-11) */
+    int32_t n_scales;     /* 1..PGSF_MAX_SCALES                                                   */
+    const double *sigmas; /* HOST: n_scales x (sigma_x, sigma_y, sigma_z) in voxels, >= 0;
+                             0 = identity along that axis                                         */
+    double truncate;      /* radius = ceil(truncate*sigma) (C-2); the paper's configs use 3.0     */
+    int32_t box_half[3];  /* (hx,hy,hz) >= 0: statistics window [v-h, v+h] per axis (C-6)         */
+    double k;             /* threshold in local-standard-deviation units (C-10); configs use 4.0  */
+    uint32_t flags;       /* PGSF_FLAG_*                                                          */
+} pgsf_plan_desc;
+
+/*
+ * pgsf_plan_create -- host only.  For every scale and axis: r = ceil(truncate*sigma); taps
+ * g[o] = exp(-o^2 / (2 sigma^2)) for o = -r..r evaluated in fp64, divided by their fp64 sum
+ * (C-1..C-3; the paper only says "Gaussian filters"), rounded to fp32 and uploaded to
+ * `device`.  Each batch entry is a standalone cube: input outside it is zero (C-5).
+ * Returns INVALID_ARG for nx,ny,nz,batch < 1, n_scales outside 1..PGSF_MAX_SCALES, negative
+ * sigma / box_half / halo, 2*halo >= extent, truncate <= 0; UNSUPPORTED for a radius above
+ * PGSF_MAX_RADIUS or box_half above PGSF_MAX_BOX_HALF; CUDA if `device` cannot be used.
+ * On failure *out is NULL.
+ */
+PGSF_API pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int device);
+
+/* Releases the plan and everything it owns.  NULL is allowed. */
+PGSF_API pgsf_status pgsf_plan_destroy(pgsf_plan *plan);
+
+/* Bytes of DEVICE scratch the caller must pass as d_workspace to the calls below (256-byte
+ * aligned; may be 0, in which case d_workspace may be NULL).  0 for a NULL plan. */
+PGSF_API size_t pgsf_plan_workspace_bytes(const pgsf_plan *plan);
+
+/* Text of the last error recorded on this plan ("" if none).  With plan == NULL: the text of the
+ * last pgsf_plan_create failure of the calling thread. */
+PGSF_API const char *pgsf_last_error(const pgsf_plan *plan);
+
+/* Copies the fp32 taps the kernels use for (scale, axis) to HOST `taps` (capacity `cap` floats)
+ * and the radius to *radius; returns INVALID_ARG if cap < 2*radius+1.  For tests. */
+PGSF_API pgsf_status pgsf_plan_get_taps(const pgsf_plan *plan, int scale, int axis, float *taps, int cap,
+                               int *radius);
+
+/*
+ * pgsf_filter3d -- Eq. 2 with the index ranges of Eq. 3-5 for the Gaussian of
+ * scale `scale`, evaluated as three 1-D passes (x, y, z), which is exact for an outer-product
+ * filter up to fp32 rounding:
+ *     d_out[x,y,z] = sum_ox sum_oy sum_oz d_in[x+ox, y+oy, z+oz] gx[ox] gy[oy] gz[oz],
+ * input outside the cube = 0, taps not renormalised at the faces (C-5).  fp32 throughout.
+ * d_in, d_out: batch*nx*ny*nz floats, 16-byte aligned, must not overlap.  d_out has the input's
+ * full extents.
+ */
+PGSF_API pgsf_status pgsf_filter3d(pgsf_plan *plan, int scale, const float *d_in, float *d_out,
+                          void *d_workspace, void *cuda_stream);
+
+/*
+ * pgsf_local_threshold -- local statistics and voxel selection of one
+ * filtered cube, with the plan's box_half, k and halo:
+ *     S1 = sum of f, S2 = sum of f^2 over the box [v-h, v+h] clipped to the cube (C-7), n = its
+ *     voxel count; m = S1/n; var = max(S2/n - m^2, 0) (population, C-8); t = m + k*sqrt(var);
+ *     sel = f > t (strict, one-sided, C-10), forced to 0 within `halo` of a face (C-11).
+ * d_mask (uint8, same indexing): or_into == 0 -> mask = sel; or_into != 0 -> mask |= sel.
+ * d_mean / d_std (nullable): fp32 m and sqrt(var) for every voxel (parity aid).
+ * d_count (nullable): receives the number of non-zero bytes of the RESULTING mask (after the OR,
+ * outside the halo) (C-15).
+ */
+PGSF_API pgsf_status pgsf_local_threshold(pgsf_plan *plan, const float *d_filtered, uint8_t *d_mask,
+                                 int or_into, float *d_mean, float *d_std,
+                                 unsigned long long *d_count, void *d_workspace, void *cuda_stream);
+
+/*
+ * pgsf_find_multiscale -- the whole hot path: for every scale of the plan, filter
+ * d_in, threshold, OR into d_mask; *d_count = set voxels of the final mask.
+ * d_filtered: HOST array of n_scales DEVICE pointers receiving the filtered cubes, or NULL /
+ * NULL entries = do not keep (the workspace then holds one scratch cube).
+ */
+PGSF_API pgsf_status pgsf_find_multiscale(pgsf_plan *plan, const float *d_in, float *const *d_filtered,
+                                 uint8_t *d_mask, unsigned long long *d_count, void *d_workspace,
+                                 void *cuda_stream);
+
+/*
+ * pgsf_find_multiscale_host -- same result from HOST buffers: copies h_in to plan-owned device
+ * buffers (allocated on first use), runs pgsf_find_multiscale, copies the mask (and, when
+ * h_filtered != NULL, the filtered cubes: n_scales host pointers) back, writes *h_count, and
+ * synchronises.  Page-locked host memory makes the copies asynchronous but is not required.
+ */
+PGSF_API pgsf_status pgsf_find_multiscale_host(pgsf_plan *plan, const float *h_in, float *const *h_filtered,
+                                      uint8_t *h_mask, unsigned long long *h_count);
+
+/* Number of kernels this library has launched on behalf of `plan` since creation (bench.py's
+ * gpu_launches evidence). */
+PGSF_API unsigned long long pgsf_plan_launch_count(const pgsf_plan *plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PGSF_H */

@@ -1,0 +1,387 @@
+// C ABI of libpgsf.so: plan construction (host), argument validation, kernel dispatch.
+// See include/pgsf.h for the contract of every entry point.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "pgsf_internal.h"
+
+namespace {
+
+thread_local std::string g_create_err;
+
+pgsf_status fail(pgsf_plan *p, pgsf_status st, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (p) p->err = buf;
+    else g_create_err = buf;
+    return st;
+}
+
+pgsf_status cuda_fail(pgsf_plan *p, cudaError_t e, const char *what)
+{
+    return fail(p, PGSF_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+// radius = ceil(truncate * sigma) in fp64 (C-2); sigma = 0 -> 0
+int radius_of(double sigma, double truncate)
+{
+    if (!(sigma > 0.0)) return 0;
+    return (int)ceil(truncate * sigma);
+}
+
+// fp64 taps, renormalised over the truncated support (C-1, C-3), rounded to fp32 once.
+void make_taps(double sigma, int r, float *g /* 2r+1 */)
+{
+    if (r == 0) { g[0] = 1.f; return; }
+    double w[pgsf::kMaxTaps];
+    double sum = 0.0;
+    for (int o = -r; o <= r; ++o) {
+        w[o + r] = exp(-0.5 * ((double)o / sigma) * ((double)o / sigma));
+        sum += w[o + r];
+    }
+    for (int o = -r; o <= r; ++o) g[o + r] = (float)(w[o + r] / sum);
+}
+
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+size_t round256(size_t v) { return (v + 255u) & ~(size_t)255u; }
+
+}  // namespace
+
+extern "C" {
+
+pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int device)
+{
+    if (out == nullptr) return fail(nullptr, PGSF_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (desc == nullptr) return fail(nullptr, PGSF_ERR_INVALID_ARG, "desc is NULL");
+    if (desc->nx < 1 || desc->ny < 1 || desc->nz < 1 || desc->batch < 1)
+        return fail(nullptr, PGSF_ERR_INVALID_ARG, "extents and batch must be >= 1");
+    if ((long long)desc->nx * desc->ny >= (1LL << 31))
+        return fail(nullptr, PGSF_ERR_UNSUPPORTED, "nx*ny must be < 2^31");
+    if (desc->n_scales < 1 || desc->n_scales > PGSF_MAX_SCALES)
+        return fail(nullptr, PGSF_ERR_INVALID_ARG, "n_scales must be in 1..%d", PGSF_MAX_SCALES);
+    if (desc->sigmas == nullptr) return fail(nullptr, PGSF_ERR_INVALID_ARG, "sigmas is NULL");
+    if (!(desc->truncate > 0.0)) return fail(nullptr, PGSF_ERR_INVALID_ARG, "truncate must be > 0");
+    if (!(desc->k >= 0.0)) return fail(nullptr, PGSF_ERR_INVALID_ARG, "k must be >= 0");
+    const int ext[3] = {desc->nx, desc->ny, desc->nz};
+    for (int a = 0; a < 3; ++a) {
+        if (desc->box_half[a] < 0 || desc->halo[a] < 0)
+            return fail(nullptr, PGSF_ERR_INVALID_ARG, "box_half and halo must be >= 0");
+        if (desc->halo[a] > 0 && 2 * desc->halo[a] >= ext[a])
+            return fail(nullptr, PGSF_ERR_INVALID_ARG, "2*halo must be < extent");
+        if (desc->box_half[a] > PGSF_MAX_BOX_HALF)
+            return fail(nullptr, PGSF_ERR_UNSUPPORTED, "box_half above %d", PGSF_MAX_BOX_HALF);
+    }
+    for (int i = 0; i < desc->n_scales * 3; ++i) {
+        const double s = desc->sigmas[i];
+        if (!(s >= 0.0) || !isfinite(s))
+            return fail(nullptr, PGSF_ERR_INVALID_ARG, "sigma must be finite and >= 0");
+        if (radius_of(s, desc->truncate) > PGSF_MAX_RADIUS)
+            return fail(nullptr, PGSF_ERR_UNSUPPORTED, "radius ceil(truncate*sigma) above %d",
+                        PGSF_MAX_RADIUS);
+    }
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDeviceCount (no CPU fallback exists)");
+    if (device < 0 || device >= ndev)
+        return fail(nullptr, PGSF_ERR_CUDA, "device %d not present (%d devices)", device, ndev);
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDeviceProperties");
+    if (prop.major != 10)
+        return fail(nullptr, PGSF_ERR_UNSUPPORTED, "device is sm_%d%d; this library is built for sm_100a",
+                    prop.major, prop.minor);
+
+    pgsf_plan *p = new (std::nothrow) pgsf_plan();
+    if (!p) return fail(nullptr, PGSF_ERR_OOM, "plan allocation failed");
+    p->desc = *desc;
+    memcpy(p->sigmas, desc->sigmas, sizeof(double) * 3 * desc->n_scales);
+    p->desc.sigmas = p->sigmas;
+    p->device = device;
+    p->sm_count = prop.multiProcessorCount;
+    p->dims.nx = desc->nx;
+    p->dims.ny = desc->ny;
+    p->dims.nz = desc->nz;
+    p->dims.plane = (long long)desc->nx * desc->ny;
+    p->dims.cube = p->dims.plane * desc->nz;
+    p->launches = 0;
+    p->h_d_in = nullptr;
+    p->h_d_mask = nullptr;
+    p->h_d_count = nullptr;
+    p->h_d_ws = nullptr;
+    p->h_stream = nullptr;
+    for (int s = 0; s < PGSF_MAX_SCALES; ++s) p->h_d_f[s] = nullptr;
+
+    const bool force_generic = (desc->flags & PGSF_FLAG_FORCE_GENERIC) != 0;
+    bool fast = !force_generic && (desc->nx % 4 == 0);
+    for (int s = 0; s < desc->n_scales; ++s) {
+        pgsf::ScalePlan &sp = p->scales[s];
+        memset(&sp, 0, sizeof sp);
+        for (int a = 0; a < 3; ++a) {
+            const double sg = desc->sigmas[3 * s + a];
+            sp.r[a] = radius_of(sg, desc->truncate);
+            sp.taps[a].r = sp.r[a];
+            make_taps(sg, sp.r[a], sp.taps[a].g);
+        }
+        const int rxy = sp.r[0] > sp.r[1] ? sp.r[0] : sp.r[1];
+        if (!pgsf::fast_xy_radius(rxy, &sp.rxy_c) || !pgsf::fast_z_radius(sp.r[2], &sp.rz_c)) {
+            fast = false;
+            continue;
+        }
+        // centre the true taps in the compiled window; the padding taps are exact zeros, so the
+        // extra FMAs add +0 and do not change the result
+        for (int o = -sp.r[0]; o <= sp.r[0]; ++o) sp.txy.gx[o + sp.rxy_c] = sp.taps[0].g[o + sp.r[0]];
+        for (int o = -sp.r[1]; o <= sp.r[1]; ++o) sp.txy.gy[o + sp.rxy_c] = sp.taps[1].g[o + sp.r[1]];
+        sp.tz.r = sp.rz_c;
+        for (int o = -sp.r[2]; o <= sp.r[2]; ++o) sp.tz.g[o + sp.rz_c] = sp.taps[2].g[o + sp.r[2]];
+    }
+    p->fast_filter = fast;
+    p->fast_stats = !force_generic && (desc->nx % 4 == 0) && pgsf::fast_stats_supported(p);
+
+    // workspace: [scratch filtered cube][filter temporaries][statistics temporaries]
+    p->ws_cube_bytes = round256((size_t)p->dims.cube * sizeof(float));
+    const size_t cubes = 1 + (p->fast_filter ? 1 : 2) + (p->fast_stats ? 0 : 4);
+    p->ws_bytes = cubes * p->ws_cube_bytes;
+    *out = p;
+    return PGSF_OK;
+}
+
+pgsf_status pgsf_plan_destroy(pgsf_plan *p)
+{
+    if (!p) return PGSF_OK;
+    if (p->h_d_in || p->h_d_mask || p->h_d_ws || p->h_d_count) {
+        cudaSetDevice(p->device);
+        cudaFree(p->h_d_in);
+        cudaFree(p->h_d_mask);
+        cudaFree(p->h_d_count);
+        cudaFree(p->h_d_ws);
+        for (int s = 0; s < PGSF_MAX_SCALES; ++s) cudaFree(p->h_d_f[s]);
+        if (p->h_stream) cudaStreamDestroy(p->h_stream);
+    }
+    delete p;
+    return PGSF_OK;
+}
+
+size_t pgsf_plan_workspace_bytes(const pgsf_plan *p) { return p ? p->ws_bytes : 0; }
+
+const char *pgsf_last_error(const pgsf_plan *p) { return p ? p->err.c_str() : g_create_err.c_str(); }
+
+unsigned long long pgsf_plan_launch_count(const pgsf_plan *p) { return p ? p->launches : 0ULL; }
+
+pgsf_status pgsf_plan_get_taps(const pgsf_plan *p, int scale, int axis, float *taps, int cap,
+                               int *radius)
+{
+    if (!p || scale < 0 || scale >= p->desc.n_scales || axis < 0 || axis > 2 || !taps || !radius)
+        return PGSF_ERR_INVALID_ARG;
+    const int r = p->scales[scale].r[axis];
+    *radius = r;
+    if (cap < 2 * r + 1) return PGSF_ERR_INVALID_ARG;
+    memcpy(taps, p->scales[scale].taps[axis].g, sizeof(float) * (2 * r + 1));
+    return PGSF_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+struct Workspace {
+    float *scratch;  // 1 cube
+    float *ftmp;     // 1 or 2 cubes
+    float *stmp;     // 0 or 4 cubes
+};
+
+Workspace carve(const pgsf_plan *p, void *ws)
+{
+    Workspace w;
+    char *b = static_cast<char *>(ws);
+    w.scratch = reinterpret_cast<float *>(b);
+    w.ftmp = reinterpret_cast<float *>(b + p->ws_cube_bytes);
+    w.stmp = reinterpret_cast<float *>(b + p->ws_cube_bytes * (1 + (p->fast_filter ? 1 : 2)));
+    return w;
+}
+
+pgsf_status check_ws(pgsf_plan *p, void *ws)
+{
+    if (p->ws_bytes > 0 && ws == nullptr) return fail(p, PGSF_ERR_INVALID_ARG, "d_workspace is NULL");
+    if ((reinterpret_cast<uintptr_t>(ws) & 255u) != 0)
+        return fail(p, PGSF_ERR_INVALID_ARG, "d_workspace must be 256-byte aligned");
+    return PGSF_OK;
+}
+
+pgsf_status filter_one(pgsf_plan *p, int scale, const float *in, float *out, const Workspace &w,
+                       cudaStream_t st)
+{
+    cudaError_t e;
+    if (p->fast_filter) e = pgsf::fast_filter3d(p, scale, in, out, w.ftmp, st);
+    else e = pgsf::generic_filter3d(p, scale, in, out, w.ftmp, w.ftmp + p->ws_cube_bytes / sizeof(float), st);
+    if (e != cudaSuccess) return cuda_fail(p, e, "filter launch");
+    return PGSF_OK;
+}
+
+pgsf_status threshold_one(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean,
+                          float *sd, unsigned long long *count, const Workspace &w, cudaStream_t st)
+{
+    cudaError_t e;
+    if (p->fast_stats) e = pgsf::fast_threshold(p, f, mask, or_into, mean, sd, count, st);
+    else e = pgsf::generic_threshold(p, f, mask, or_into, mean, sd, count, w.stmp, st);
+    if (e != cudaSuccess) return cuda_fail(p, e, "threshold launch");
+    return PGSF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+pgsf_status pgsf_filter3d(pgsf_plan *p, int scale, const float *d_in, float *d_out, void *d_ws,
+                          void *stream)
+{
+    if (!p) return PGSF_ERR_INVALID_ARG;
+    if (scale < 0 || scale >= p->desc.n_scales) return fail(p, PGSF_ERR_INVALID_ARG, "scale out of range");
+    if (!d_in || !d_out) return fail(p, PGSF_ERR_INVALID_ARG, "NULL cube pointer");
+    if (!aligned16(d_in) || !aligned16(d_out))
+        return fail(p, PGSF_ERR_INVALID_ARG, "cube pointers must be 16-byte aligned");
+    const size_t bytes = (size_t)p->dims.cube * p->desc.batch * sizeof(float);
+    const char *a = reinterpret_cast<const char *>(d_in), *b = reinterpret_cast<const char *>(d_out);
+    if (a < b + bytes && b < a + bytes) return fail(p, PGSF_ERR_INVALID_ARG, "d_out overlaps d_in");
+    pgsf_status s = check_ws(p, d_ws);
+    if (s != PGSF_OK) return s;
+    cudaError_t e = cudaSetDevice(p->device);
+    if (e != cudaSuccess) return cuda_fail(p, e, "cudaSetDevice");
+    const Workspace w = carve(p, d_ws);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    for (int bi = 0; bi < p->desc.batch; ++bi) {
+        s = filter_one(p, scale, d_in + (size_t)bi * p->dims.cube, d_out + (size_t)bi * p->dims.cube, w, st);
+        if (s != PGSF_OK) return s;
+    }
+    return PGSF_OK;
+}
+
+pgsf_status pgsf_local_threshold(pgsf_plan *p, const float *d_f, uint8_t *d_mask, int or_into,
+                                 float *d_mean, float *d_std, unsigned long long *d_count, void *d_ws,
+                                 void *stream)
+{
+    if (!p) return PGSF_ERR_INVALID_ARG;
+    if (!d_f || !d_mask) return fail(p, PGSF_ERR_INVALID_ARG, "NULL cube or mask pointer");
+    if (!aligned16(d_f) || !aligned16(d_mask) || !aligned16(d_mean) || !aligned16(d_std))
+        return fail(p, PGSF_ERR_INVALID_ARG, "pointers must be 16-byte aligned");
+    if (d_count && (reinterpret_cast<uintptr_t>(d_count) & 7u))
+        return fail(p, PGSF_ERR_INVALID_ARG, "d_count must be 8-byte aligned");
+    pgsf_status s = check_ws(p, d_ws);
+    if (s != PGSF_OK) return s;
+    cudaError_t e = cudaSetDevice(p->device);
+    if (e != cudaSuccess) return cuda_fail(p, e, "cudaSetDevice");
+    const Workspace w = carve(p, d_ws);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (d_count) {
+        e = cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), st);
+        if (e != cudaSuccess) return cuda_fail(p, e, "cudaMemsetAsync(count)");
+    }
+    for (int bi = 0; bi < p->desc.batch; ++bi) {
+        const size_t off = (size_t)bi * p->dims.cube;
+        s = threshold_one(p, d_f + off, d_mask + off, or_into, d_mean ? d_mean + off : nullptr,
+                          d_std ? d_std + off : nullptr, d_count, w, st);
+        if (s != PGSF_OK) return s;
+    }
+    return PGSF_OK;
+}
+
+pgsf_status pgsf_find_multiscale(pgsf_plan *p, const float *d_in, float *const *d_filtered,
+                                 uint8_t *d_mask, unsigned long long *d_count, void *d_ws, void *stream)
+{
+    if (!p) return PGSF_ERR_INVALID_ARG;
+    if (!d_in || !d_mask) return fail(p, PGSF_ERR_INVALID_ARG, "NULL cube or mask pointer");
+    if (!aligned16(d_in) || !aligned16(d_mask))
+        return fail(p, PGSF_ERR_INVALID_ARG, "pointers must be 16-byte aligned");
+    if (d_count && (reinterpret_cast<uintptr_t>(d_count) & 7u))
+        return fail(p, PGSF_ERR_INVALID_ARG, "d_count must be 8-byte aligned");
+    const int S = p->desc.n_scales;
+    if (d_filtered)
+        for (int s = 0; s < S; ++s)
+            if (d_filtered[s] && !aligned16(d_filtered[s]))
+                return fail(p, PGSF_ERR_INVALID_ARG, "d_filtered[%d] must be 16-byte aligned", s);
+    pgsf_status rc = check_ws(p, d_ws);
+    if (rc != PGSF_OK) return rc;
+    cudaError_t e = cudaSetDevice(p->device);
+    if (e != cudaSuccess) return cuda_fail(p, e, "cudaSetDevice");
+    const Workspace w = carve(p, d_ws);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (d_count) {
+        e = cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), st);
+        if (e != cudaSuccess) return cuda_fail(p, e, "cudaMemsetAsync(count)");
+    }
+    for (int bi = 0; bi < p->desc.batch; ++bi) {
+        const size_t off = (size_t)bi * p->dims.cube;
+        for (int s = 0; s < S; ++s) {
+            float *f = (d_filtered && d_filtered[s]) ? d_filtered[s] + off : w.scratch;
+            rc = filter_one(p, s, d_in + off, f, w, st);
+            if (rc != PGSF_OK) return rc;
+            rc = threshold_one(p, f, d_mask + off, s > 0, nullptr, nullptr,
+                               (s == S - 1) ? d_count : nullptr, w, st);
+            if (rc != PGSF_OK) return rc;
+        }
+    }
+    return PGSF_OK;
+}
+
+pgsf_status pgsf_find_multiscale_host(pgsf_plan *p, const float *h_in, float *const *h_filtered,
+                                      uint8_t *h_mask, unsigned long long *h_count)
+{
+    if (!p) return PGSF_ERR_INVALID_ARG;
+    if (!h_in || !h_mask) return fail(p, PGSF_ERR_INVALID_ARG, "NULL host pointer");
+    cudaError_t e = cudaSetDevice(p->device);
+    if (e != cudaSuccess) return cuda_fail(p, e, "cudaSetDevice");
+    const size_t nvox = (size_t)p->dims.cube * p->desc.batch;
+    const int S = p->desc.n_scales;
+    if (!p->h_d_in) {
+        if ((e = cudaStreamCreateWithFlags(&p->h_stream, cudaStreamNonBlocking)) != cudaSuccess)
+            return cuda_fail(p, e, "cudaStreamCreate");
+        if ((e = cudaMalloc(&p->h_d_in, nvox * sizeof(float))) != cudaSuccess ||
+            (e = cudaMalloc(&p->h_d_mask, nvox)) != cudaSuccess ||
+            (e = cudaMalloc(&p->h_d_count, sizeof(unsigned long long))) != cudaSuccess ||
+            (e = cudaMalloc(&p->h_d_ws, p->ws_bytes ? p->ws_bytes : 256)) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(p, PGSF_ERR_OOM, "device staging allocation failed: %s", cudaGetErrorString(e));
+        }
+    }
+    float *dptr[PGSF_MAX_SCALES] = {nullptr};
+    if (h_filtered) {
+        for (int s = 0; s < S; ++s) {
+            if (!h_filtered[s]) continue;
+            if (!p->h_d_f[s] && (e = cudaMalloc(&p->h_d_f[s], nvox * sizeof(float))) != cudaSuccess) {
+                cudaGetLastError();
+                return fail(p, PGSF_ERR_OOM, "device staging allocation failed: %s", cudaGetErrorString(e));
+            }
+            dptr[s] = p->h_d_f[s];
+        }
+    }
+    cudaStream_t st = p->h_stream;
+    if ((e = cudaMemcpyAsync(p->h_d_in, h_in, nvox * sizeof(float), cudaMemcpyHostToDevice, st)) != cudaSuccess)
+        return cuda_fail(p, e, "H2D copy");
+    pgsf_status rc = pgsf_find_multiscale(p, p->h_d_in, h_filtered ? dptr : nullptr, p->h_d_mask,
+                                          p->h_d_count, p->h_d_ws, st);
+    if (rc != PGSF_OK) return rc;
+    if ((e = cudaMemcpyAsync(h_mask, p->h_d_mask, nvox, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+        return cuda_fail(p, e, "D2H mask copy");
+    if (h_filtered)
+        for (int s = 0; s < S; ++s)
+            if (h_filtered[s] &&
+                (e = cudaMemcpyAsync(h_filtered[s], dptr[s], nvox * sizeof(float), cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+                return cuda_fail(p, e, "D2H filtered copy");
+    unsigned long long cnt = 0;
+    if ((e = cudaMemcpyAsync(&cnt, p->h_d_count, sizeof cnt, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+        return cuda_fail(p, e, "D2H count copy");
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(p, e, "stream synchronize");
+    if (h_count) *h_count = cnt;
+    return PGSF_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,154 @@
+// Generic kernels: any cube shape, any radius <= PGSF_MAX_RADIUS, any box.  One thread per output
+// voxel, every pass through global memory.  They are the path for shapes / radii the tiled sm_100a
+// kernels (pgsf_filter.cu, pgsf_stats.cu) do not cover, and a second implementation the parity
+// tests run against the same oracle.  Eq. 2 as three 1-D passes; P:152 as three
+// directional sums.
+#include "pgsf_internal.h"
+
+namespace pgsf {
+namespace {
+
+constexpr int kThreads = 256;
+
+__device__ __forceinline__ void decode(long long i, const Dims &d, int &x, int &y, int &z)
+{
+    x = (int)(i % d.nx);
+    long long q = i / d.nx;
+    y = (int)(q % d.ny);
+    z = (int)(q / d.ny);
+}
+
+// out[v] = sum_o in[v + o*e_AXIS] g[o], zero outside the cube (C-5)
+template <int AXIS>
+__global__ void __launch_bounds__(kThreads) k_conv1d(const float *__restrict__ in,
+                                                      float *__restrict__ out, Dims d, Taps t)
+{
+    long long i = (long long)blockIdx.x * kThreads + threadIdx.x;
+    if (i >= d.cube) return;
+    int x, y, z;
+    decode(i, d, x, y, z);
+    const int c = AXIS == 0 ? x : (AXIS == 1 ? y : z);
+    const int n = AXIS == 0 ? d.nx : (AXIS == 1 ? d.ny : d.nz);
+    const long long stride = AXIS == 0 ? 1 : (AXIS == 1 ? (long long)d.nx : d.plane);
+    const int lo = max(-t.r, -c), hi = min(t.r, n - 1 - c);
+    float acc = 0.f;
+    for (int o = lo; o <= hi; ++o) acc = fmaf(in[i + o * stride], t.g[o + t.r], acc);
+    out[i] = acc;
+}
+
+// One directional sum of P:152 over the window clipped to the cube (C-7).
+// FIRST: q1 = a, q2 = a*a; otherwise q1 = a, q2 = b.
+template <int AXIS, bool FIRST>
+__global__ void __launch_bounds__(kThreads) k_boxsum(const float *__restrict__ a,
+                                                      const float *__restrict__ b,
+                                                      float *__restrict__ oa, float *__restrict__ ob,
+                                                      Dims d, int h)
+{
+    long long i = (long long)blockIdx.x * kThreads + threadIdx.x;
+    if (i >= d.cube) return;
+    int x, y, z;
+    decode(i, d, x, y, z);
+    const int c = AXIS == 0 ? x : (AXIS == 1 ? y : z);
+    const int n = AXIS == 0 ? d.nx : (AXIS == 1 ? d.ny : d.nz);
+    const long long stride = AXIS == 0 ? 1 : (AXIS == 1 ? (long long)d.nx : d.plane);
+    const int lo = max(-h, -c), hi = min(h, n - 1 - c);
+    float s1 = 0.f, s2 = 0.f;
+    for (int o = lo; o <= hi; ++o) {
+        float v = a[i + o * stride];
+        s1 += v;
+        if (FIRST) s2 = fmaf(v, v, s2);
+        else s2 += b[i + o * stride];
+    }
+    oa[i] = s1;
+    ob[i] = s2;
+}
+
+__device__ __forceinline__ int clipped_len(int c, int h, int n)
+{
+    return min(c + h, n - 1) - max(c - h, 0) + 1;
+}
+
+// z-score / voxel selection: division-free form of f > m + k*sd,
+//   n f - S1 > k sqrt(max(n S2 - S1^2, 0))   <=>   f > S1/n + k sqrt(max(S2/n - (S1/n)^2, 0)).
+__global__ void __launch_bounds__(kThreads) k_threshold(
+    const float *__restrict__ f, const float *__restrict__ S1, const float *__restrict__ S2,
+    uint8_t *__restrict__ mask, int or_into, float *__restrict__ mean, float *__restrict__ sd,
+    unsigned long long *__restrict__ count, Dims d, int hx, int hy, int hz, int gx, int gy, int gz,
+    float k, float k2)
+{
+    long long i = (long long)blockIdx.x * kThreads + threadIdx.x;
+    int set = 0;
+    if (i < d.cube) {
+        int x, y, z;
+        decode(i, d, x, y, z);
+        const float n = (float)clipped_len(x, hx, d.nx) * (float)clipped_len(y, hy, d.ny) *
+                        (float)clipped_len(z, hz, d.nz);
+        const float v = f[i], s1 = S1[i], s2 = S2[i];
+        const float a = fmaf(n, v, -s1);
+        const float q = fmaxf(fmaf(n, s2, -s1 * s1), 0.f);
+        int sel = (a > kFlatGuard * n * fabsf(v)) && (a * a > k2 * q);
+        const bool core = x >= gx && x < d.nx - gx && y >= gy && y < d.ny - gy && z >= gz &&
+                          z < d.nz - gz;
+        if (!core) sel = 0;
+        else if (or_into) sel |= (mask[i] != 0);
+        mask[i] = (uint8_t)sel;
+        set = sel;
+        if (mean != nullptr) {
+            const float m = s1 / n;
+            mean[i] = m;
+            if (sd != nullptr) sd[i] = sqrtf(fmaxf(s2 / n - m * m, 0.f));
+        } else if (sd != nullptr) {
+            const float m = s1 / n;
+            sd[i] = sqrtf(fmaxf(s2 / n - m * m, 0.f));
+        }
+    }
+    if (count != nullptr) {
+        unsigned b = __ballot_sync(0xffffffffu, set);
+        __shared__ unsigned wsum[kThreads / 32];
+        if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = __popc(b);
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned t = 0;
+            for (int w = 0; w < kThreads / 32; ++w) t += wsum[w];
+            if (t) atomicAdd(count, (unsigned long long)t);
+        }
+    }
+    (void)k;
+}
+
+inline unsigned grid_for(long long n) { return (unsigned)((n + kThreads - 1) / kThreads); }
+
+}  // namespace
+
+cudaError_t generic_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp_a,
+                             float *tmp_b, cudaStream_t st)
+{
+    const Dims &d = p->dims;
+    const ScalePlan &sp = p->scales[scale];
+    const unsigned g = grid_for(d.cube);
+    k_conv1d<0><<<g, kThreads, 0, st>>>(in, tmp_a, d, sp.taps[0]);
+    k_conv1d<1><<<g, kThreads, 0, st>>>(tmp_a, tmp_b, d, sp.taps[1]);
+    k_conv1d<2><<<g, kThreads, 0, st>>>(tmp_b, out, d, sp.taps[2]);
+    p->launches += 3;
+    return cudaGetLastError();
+}
+
+cudaError_t generic_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean,
+                              float *sd, unsigned long long *count, float *tmp4, cudaStream_t st)
+{
+    const Dims &d = p->dims;
+    const unsigned g = grid_for(d.cube);
+    float *x1 = tmp4, *x2 = tmp4 + d.cube, *y1 = tmp4 + 2 * d.cube, *y2 = tmp4 + 3 * d.cube;
+    const int *h = p->desc.box_half;
+    k_boxsum<0, true><<<g, kThreads, 0, st>>>(f, nullptr, x1, x2, d, h[0]);
+    k_boxsum<1, false><<<g, kThreads, 0, st>>>(x1, x2, y1, y2, d, h[1]);
+    k_boxsum<2, false><<<g, kThreads, 0, st>>>(y1, y2, x1, x2, d, h[2]);
+    const float k = (float)p->desc.k;
+    k_threshold<<<g, kThreads, 0, st>>>(f, x1, x2, mask, or_into, mean, sd, count, d, h[0], h[1], h[2],
+                                        p->desc.halo[0], p->desc.halo[1], p->desc.halo[2], k,
+                                        (float)(p->desc.k * p->desc.k));
+    p->launches += 4;
+    return cudaGetLastError();
+}
+
+}  // namespace pgsf

@@ -1,0 +1,90 @@
+// Internal declarations shared by the translation units of libpgsf.so (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+
+#include "pgsf.h"
+
+namespace pgsf {
+
+constexpr int kMaxTaps = 2 * PGSF_MAX_RADIUS + 1;  // 193
+
+// Voxel selection is evaluated as  n f - S1 > k sqrt(max(n S2 - S1^2, 0)).  Where the window is flat
+// to fp32 precision (sd below ~3e-4 |mean|, the rounding floor of S2/n - m^2 in fp32) the sign of
+// n f - S1 is rounding noise; requiring n f - S1 > kFlatGuard * n |f| keeps such regions unselected
+// ("with std = 0 nothing is selected", reading C-10) and cannot change a well-conditioned decision.
+constexpr float kFlatGuard = 1e-5f;
+
+// Taps of one axis, passed BY VALUE as a kernel parameter: kernel parameters live in constant
+// bank 0, so a compile-time tap index becomes a uniform-register operand of FFMA/FFMA2 (the role
+// constant memory plays in the paper's kernel) without any per-module __constant__
+// state shared between plans.
+struct Taps {
+    float g[kMaxTaps + 3];  // g[o + r], o = -r..r; zero beyond
+    int r;
+};
+
+struct TapsXY {  // small radii only (x and y passes)
+    float gx[32];
+    float gy[32];
+};
+
+struct ScalePlan {
+    int r[3];            // true radii ceil(truncate*sigma)
+    int rxy_c;           // compiled radius used by the fast xy kernel (>= max(r[0], r[1])), 0 = none
+    int rz_c;            // compiled radius used by the fast z kernel (>= r[2]), 0 = none
+    Taps taps[3];        // true taps (generic path; also what pgsf_plan_get_taps reports)
+    TapsXY txy;          // taps centred in a 2*rxy_c+1 window, zero padded
+    Taps tz;             // taps centred in a 2*rz_c+1 window, zero padded
+};
+
+struct Dims {
+    int nx, ny, nz;
+    long long plane;     // nx*ny
+    long long cube;      // nx*ny*nz
+};
+
+}  // namespace pgsf
+
+struct pgsf_plan {
+    pgsf_plan_desc desc;
+    double sigmas[PGSF_MAX_SCALES * 3];
+    pgsf::ScalePlan scales[PGSF_MAX_SCALES];
+    pgsf::Dims dims;
+    int device;
+    int sm_count;
+    bool fast_filter;    // all scales have compiled radii, nx % 4 == 0
+    bool fast_stats;
+    size_t ws_bytes;     // total workspace
+    size_t ws_cube_bytes;
+    unsigned long long launches;
+    std::string err;
+    // plan-owned device staging for pgsf_find_multiscale_host
+    float *h_d_in;
+    float *h_d_f[PGSF_MAX_SCALES];
+    uint8_t *h_d_mask;
+    unsigned long long *h_d_count;
+    void *h_d_ws;
+    cudaStream_t h_stream;
+};
+
+namespace pgsf {
+
+// ---- generic kernels (pgsf_generic.cu): any shape, any radius <= PGSF_MAX_RADIUS ----------------
+cudaError_t generic_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp_a,
+                             float *tmp_b, cudaStream_t st);
+// tmp: 4 cubes
+cudaError_t generic_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean,
+                              float *sd, unsigned long long *count, float *tmp4, cudaStream_t st);
+
+// ---- fast kernels (pgsf_filter.cu, pgsf_stats.cu): nx % 4 == 0, 16-byte aligned, compiled radii --
+bool fast_xy_radius(int r, int *compiled);
+bool fast_z_radius(int r, int *compiled);
+cudaError_t fast_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp,
+                          cudaStream_t st);
+bool fast_stats_supported(const pgsf_plan *p);
+cudaError_t fast_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean,
+                           float *sd, unsigned long long *count, cudaStream_t st);
+
+}  // namespace pgsf

@@ -1,0 +1,300 @@
+"""Parity of the CUDA path (through the C ABI of include/pgsf.h) against the fp64 oracle, element by
+element on the same seeded inputs.  Tolerances: tests/parity.py (reading C-13 of DESIGN.md).
+All tests need a B200: run with `pytest -m gpu`."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pg():
+    from paper_1507_04941_b200 import binding, build
+    build.build()
+    binding.load_library()
+    assert torch.cuda.is_available(), "no GPU: the product path has no CPU fallback"
+    return binding
+
+
+@pytest.fixture(scope="module")
+def synth():
+    from paper_1507_04941_b200 import synth as s
+    return s
+
+
+IMPLS = [pytest.param(0, id="fast"), pytest.param(1, id="generic")]
+
+
+def _plan(pg, w, flags=0, k=None):
+    return pg.Plan(w.dims, w.sigmas, w.box_half, w.k if k is None else k, batch=w.batch, halo=w.halo,
+                   truncate=w.truncate, flags=flags)
+
+
+def _full_compare(pg, oracle, w, d, flags=0, k=None, check_stats=True):
+    """Whole-workload comparison (small cubes): find_multiscale + per-scale calls."""
+    kk = w.k if k is None else k
+    rep_total = parity.MaskReport(0, 0, 0)
+    with _plan(pg, w, flags, k) as plan:
+        mask, cnt, filt = plan.pgsf_find_multiscale(d, keep_filtered=True)
+        torch.cuda.synchronize()
+        gpu_count = int(cnt.item())
+        assert gpu_count == int(mask.sum().item())
+        nx, ny, nz = w.dims
+        oracle_total = 0
+        for b in range(w.batch):
+            res = oracle.find_full(d[b].cpu().numpy(), w.sigmas, w.box_half, kk, halo=w.halo,
+                                   truncate=w.truncate)
+            oracle_total += res.count
+            for s in range(len(w.sigmas)):
+                parity.assert_filter_close(filt[s][b].cpu().numpy(), res.scales[s].f, f"b{b} scale {s}")
+            inside = parity.halo_inside((0, 0, 0), w.dims, w.dims, w.halo)
+            rep = parity.assert_mask_ok(mask[b].cpu().numpy(), res, inside, f"b{b} OR mask")
+            rep_total.mismatches += rep.mismatches
+            rep_total.excused += rep.excused
+            rep_total.band_voxels += rep.band_voxels
+            if check_stats and b == 0:
+                # per-scale calls: filter3d == the cube find_multiscale kept; local_threshold stats
+                for s in range(len(w.sigmas)):
+                    f1 = plan.pgsf_filter3d(s, d)
+                    assert torch.equal(f1, filt[s]), "pgsf_filter3d differs from find_multiscale's cube"
+                    m1, c1, mean, std = plan.pgsf_local_threshold(f1, want_stats=True)
+                    torch.cuda.synchronize()
+                    st = res.scales[s].stats
+                    parity.assert_stats_close(mean[0].cpu().numpy(), std[0].cpu().numpy(), st, f"scale {s}")
+                    single = type(res)([res.scales[s]], st.mask * inside, int((st.mask * inside).sum()))
+                    parity.assert_mask_ok(m1[0].cpu().numpy(), single, inside, f"scale {s} mask")
+                    assert int(c1.item()) == int(m1.sum().item())
+        assert abs(gpu_count - oracle_total) <= rep_total.mismatches
+    return rep_total, gpu_count
+
+
+# ------------------------------------------------------------------------------------ config 1
+
+@pytest.mark.parametrize("flags", IMPLS)
+@pytest.mark.parametrize("k", [4.0, 3.0, 2.5])
+def test_config1_full(pg, synth, oracle, flags, k):
+    """BASELINE.json configs[0] in full; k = 3 and 2.5 are the supplementary runs of C-14 (the k = 4
+    mask of this cube is nearly empty)."""
+    w = synth.WORKLOADS[1]
+    d = synth.make_workload(w, "cuda")
+    rep, count = _full_compare(pg, oracle, w, d, flags, k)
+    print(f"config1 k={k}: count={count} mismatches={rep.mismatches} band={rep.band_voxels}")
+    if k <= 3.0:
+        assert count > 50          # the mask comparison is not vacuous
+
+
+# ------------------------------------------------------------------------------------ ragged shapes
+
+@pytest.mark.parametrize("flags", IMPLS)
+@pytest.mark.parametrize("dims,sigmas,box", [
+    ((104, 75, 150), ((1, 1, 2), (2, 2, 4)), (4, 5, 9)),          # several tiles + ragged tails
+    ((200, 150, 90), ((3, 3, 8),), (8, 8, 16)),
+    ((101, 67, 83), ((1, 1.5, 2), (2.5, 2, 4)), (3, 4, 5)),       # nx % 4 != 0 -> generic kernels
+    ((36, 300, 40), ((2, 1, 3),), (16, 2, 7)),
+])
+def test_ragged_cubes_full(pg, synth, oracle, flags, dims, sigmas, box):
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[2], dims, n_sources=12), sigmas=sigmas, box_half=box, k=3.0)
+    d = synth.make_workload(w, "cuda")
+    rep, count = _full_compare(pg, oracle, w, d, flags)
+    assert count > 0
+
+
+@pytest.mark.parametrize("flags", IMPLS)
+def test_batch_with_halo(pg, synth, oracle, flags):
+    """Config-4-like: pre-haloed sub-cubes, each a standalone zero-padded cube (C-11)."""
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[4], (96, 80, 112), batch=3, n_sources=6), halo=(16, 12, 20), k=3.0)
+    d = synth.make_workload(w, "cuda")
+    rep, count = _full_compare(pg, oracle, w, d, flags)
+    assert count > 0
+
+
+# ------------------------------------------------------------------------------------ degenerate cases
+
+@pytest.mark.parametrize("flags", IMPLS)
+@pytest.mark.parametrize("dims,sigmas,box", [
+    ((8, 8, 8), ((1, 1, 2),), (4, 4, 8)),             # radius and box larger than the cube
+    ((16, 12, 1), ((1, 1, 2),), (2, 2, 2)),           # a single channel
+    ((4, 1, 64), ((2, 2, 4),), (1, 1, 8)),            # a single spectrum-wide row
+    ((32, 32, 32), ((0, 0, 0),), (0, 0, 0)),          # identity filter, single-voxel window
+    ((32, 24, 40), ((0, 2, 0), (1, 0, 3)), (3, 0, 5)),
+    ((1, 1, 1), ((1, 1, 1),), (1, 1, 1)),
+])
+def test_degenerate_shapes(pg, synth, oracle, flags, dims, sigmas, box):
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[1], dims, n_sources=2), sigmas=sigmas, box_half=box, k=1.5)
+    d = synth.make_workload(w, "cuda")
+    _full_compare(pg, oracle, w, d, flags)
+
+
+@pytest.mark.parametrize("flags", IMPLS)
+def test_special_inputs(pg, synth, flags):
+    """Zero cube and power-of-two constant cube select nothing (S12); impulse reproduces the
+    outer-product taps (S2); mask(2d) == mask(d) and f(2d) == 2 f(d) bit for bit (S14)."""
+    dims, sig, box = (64, 48, 80), [(1, 1, 2), (2, 2, 4)], (4, 4, 8)
+    with pg.Plan(dims, sig, box, 4.0, flags=flags) as plan:
+        z = torch.zeros((1, dims[2], dims[1], dims[0]), device="cuda")
+        mask, cnt, filt = plan.pgsf_find_multiscale(z, keep_filtered=True)
+        assert int(cnt.item()) == 0 and int(mask.sum()) == 0 and float(filt[0].abs().max()) == 0.0
+        c = torch.full_like(z, 0.5)
+        mask, cnt, filt = plan.pgsf_find_multiscale(c, keep_filtered=True)
+        # constant where every tap is inside the cube; nothing selected where the whole window is
+        # constant (>= r + h from every face): sd = 0 there (C-10)
+        assert float((filt[1][0, 12:-12, 6:-6, 6:-6] - 0.5).abs().max()) < 2e-7
+        assert int(mask[0, 20:-20, 10:-10, 10:-10].sum()) == 0
+        imp = torch.zeros_like(z)
+        imp[0, 40, 24, 32] = 1.0
+        f = plan.pgsf_filter3d(0, imp)
+        gx, gy, gz = (np.array(plan.pgsf_plan_get_taps(0, a), dtype=np.float64) for a in range(3))
+        expect = gz[:, None, None] * gy[None, :, None] * gx[None, None, :]
+        got = f[0, 34:47, 21:28, 29:36].cpu().numpy().astype(np.float64)
+        assert np.max(np.abs(got - expect)) < 1e-8
+        assert float(f.sum()) == pytest.approx(1.0, abs=1e-5)
+        d = synth.make_cube((dims[2], dims[1], dims[0]), 5, 6, device="cuda")[None]
+        plan3 = pg.Plan(dims, sig, box, 3.0, flags=flags)
+        m1, c1, f1 = plan3.pgsf_find_multiscale(d, keep_filtered=True)
+        m2, c2, f2 = plan3.pgsf_find_multiscale(2.0 * d, keep_filtered=True)
+        torch.cuda.synchronize()
+        assert torch.equal(m1, m2) and int(c1.item()) == int(c2.item()) and int(c1.item()) > 0
+        assert torch.equal(2.0 * f1[1], f2[1])
+        plan3.close()
+
+
+def test_taps_match_oracle(pg, oracle):
+    sig = [(1.0, 1.5, 2.0), (2.5, 3.0, 32.0)]
+    with pg.Plan((64, 64, 64), sig, (2, 2, 2), 4.0) as plan:
+        for s, sg in enumerate(sig):
+            for a in range(3):
+                g = np.array(plan.pgsf_plan_get_taps(s, a))
+                ref = oracle.taps(sg[a])
+                assert len(g) == len(ref)
+                assert np.max(np.abs(g - ref)) <= 6e-8 * ref.max()
+
+
+def test_or_into_and_count_semantics(pg, synth):
+    dims = (64, 48, 80)
+    d = synth.make_cube((dims[2], dims[1], dims[0]), 8, 6, device="cuda")[None]
+    with pg.Plan(dims, [(1, 1, 2), (2, 2, 4)], (4, 4, 8), 3.0) as plan:
+        f0, f1 = plan.pgsf_filter3d(0, d), plan.pgsf_filter3d(1, d)
+        m0, c0, _, _ = plan.pgsf_local_threshold(f0)
+        m1, c1, _, _ = plan.pgsf_local_threshold(f1)
+        m01 = m0.clone()
+        _, c01, _, _ = plan.pgsf_local_threshold(f1, d_mask=m01, or_into=True)
+        mm, cm, _ = plan.pgsf_find_multiscale(d)
+        torch.cuda.synchronize()
+        assert torch.equal(m01, m0 | m1) and torch.equal(mm, m01)
+        assert int(c01.item()) == int(m01.sum()) == int(cm.item())
+        assert int(c0.item()) == int(m0.sum()) and int(c1.item()) == int(m1.sum())
+        assert set(torch.unique(mm).tolist()) <= {0, 1}
+
+
+def test_host_entry_point_and_stream(pg, synth):
+    dims = (64, 48, 80)
+    d = synth.make_cube((dims[2], dims[1], dims[0]), 8, 6, device="cuda")[None]
+    with pg.Plan(dims, [(1, 1, 2)], (4, 4, 8), 3.0) as plan:
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            mm, cm, _ = plan.pgsf_find_multiscale(d, stream=st)
+        st.synchronize()
+        h_in = d.cpu().pin_memory()
+        h_mask, count = plan.pgsf_find_multiscale_host(h_in)
+        assert count == int(cm.item()) and torch.equal(h_mask, mm.cpu())
+        assert plan.pgsf_plan_launch_count() > 0
+
+
+def test_api_errors_on_device(pg):
+    with pg.Plan((32, 32, 32), [(1, 1, 2)], (2, 2, 2), 4.0) as plan:
+        d = torch.zeros((1, 32, 32, 32), device="cuda")
+        with pytest.raises(pg.PgsfError) as ei:
+            plan.pgsf_filter3d(3, d)
+        assert ei.value.status == pg.PGSF_ERR_INVALID_ARG
+        with pytest.raises(pg.PgsfError):
+            plan.pgsf_filter3d(0, d, d)                      # aliasing
+        big = torch.zeros(32 ** 3 + 4, device="cuda")
+        with pytest.raises(pg.PgsfError):
+            plan._check(plan._lib.pgsf_filter3d(plan._h, 0, big.data_ptr() + 4, d.data_ptr(),
+                                                plan.workspace().data_ptr(), None))   # misaligned
+        with pytest.raises(ValueError):
+            plan.pgsf_filter3d(0, torch.zeros((1, 32, 32, 31), device="cuda"))
+
+
+# ------------------------------------------------------------------------------------ full-size configs
+
+def _brick_list(w, rng, n_interior, size):
+    """Seeded bricks: the 8 corners, 4 face/edge bricks, the rest interior."""
+    nx, ny, nz = w.dims
+    sx, sy, sz = (min(size, n) for n in w.dims)
+    lo = []
+    for cz in (0, nz - sz):
+        for cy in (0, ny - sy):
+            for cx in (0, nx - sx):
+                lo.append((cx, cy, cz))
+    mid = ((nx - sx) // 2, (ny - sy) // 2, (nz - sz) // 2)
+    lo += [(0, mid[1], mid[2]), (mid[0], ny - sy, mid[2]), (mid[0], mid[1], 0), (nx - sx, 0, mid[2])]
+    for _ in range(n_interior):
+        lo.append(tuple(int(rng.integers(0, n - s + 1)) for n, s in zip(w.dims, (sx, sy, sz))))
+    seen, out = set(), []
+    for l in lo:
+        if l not in seen:
+            seen.add(l)
+            out.append((l, (l[0] + sx, l[1] + sy, l[2] + sz)))
+    return out
+
+
+def _brick_compare(pg, oracle, synth, w, size, n_interior, batches=(0,)):
+    d = synth.make_workload(w, "cuda")
+    rng = np.random.default_rng(w.seed + 77)
+    total = parity.MaskReport(0, 0, 0)
+    worst = 0.0
+    with _plan(pg, w) as plan:
+        mask, cnt, filt = plan.pgsf_find_multiscale(d, keep_filtered=True)
+        torch.cuda.synchronize()
+        assert int(cnt.item()) == int(mask.sum(dtype=torch.int64).item())
+        for b in batches:
+            for lo, hi in _brick_list(w, rng, n_interior, size):
+                a, e = oracle.required_input_box(w.dims, w.sigmas, w.box_half, lo, hi, w.truncate)
+                sub = d[b, a[2]:e[2], a[1]:e[1], a[0]:e[0]].cpu().numpy()
+                res = oracle.find_region(sub, a, w.dims, w.sigmas, w.box_half, w.k, lo, hi, w.halo, w.truncate)
+                sl = (b, slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
+                for s in range(len(w.sigmas)):
+                    worst = max(worst, parity.assert_filter_close(filt[s][sl].cpu().numpy(), res.scales[s].f,
+                                                                  f"{w.name} b{b} brick {lo} scale {s}"))
+                inside = parity.halo_inside(lo, hi, w.dims, w.halo)
+                rep = parity.assert_mask_ok(mask[sl].cpu().numpy(), res, inside, f"{w.name} brick {lo}")
+                total.mismatches += rep.mismatches
+                total.excused += rep.excused
+                total.band_voxels += rep.band_voxels
+        count = int(cnt.item())
+    print(f"{w.name}: count={count} worst filter diff={worst:.2e} mask mismatches={total.mismatches} "
+          f"(band voxels {total.band_voxels})")
+    return count
+
+
+@pytest.mark.slow
+def test_config2_full_size_bricks(pg, oracle, synth):
+    count = _brick_compare(pg, oracle, synth, synth.WORKLOADS[2], 96, 6)
+    assert count > 1000
+
+
+@pytest.mark.slow
+def test_config3_full_size_bricks(pg, oracle, synth):
+    count = _brick_compare(pg, oracle, synth, synth.WORKLOADS[3], 96, 4)
+    assert count > 1000
+
+
+@pytest.mark.slow
+def test_config4_full_size_bricks(pg, oracle, synth):
+    count = _brick_compare(pg, oracle, synth, synth.WORKLOADS[4], 112, 2, batches=(0, 17, 42, 63))
+    assert count > 1000
+
+
+@pytest.mark.slow
+def test_config5_full_size_bricks(pg, oracle, synth):
+    count = _brick_compare(pg, oracle, synth, synth.WORKLOADS[5], 96, 4)
+    assert count > 100
