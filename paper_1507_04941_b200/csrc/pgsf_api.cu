@@ -142,7 +142,7 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
         for (int o = -sp.r[0]; o <= sp.r[0]; ++o) sp.txy.gx[o + sp.rxy_c] = sp.taps[0].g[o + sp.r[0]];
         for (int o = -sp.r[1]; o <= sp.r[1]; ++o) sp.txy.gy[o + sp.rxy_c] = sp.taps[1].g[o + sp.r[1]];
         sp.tz.r = sp.rz_c;
-        for (int o = -sp.r[2]; o <= sp.r[2]; ++o) sp.tz.g[o + sp.rz_c] = sp.taps[2].g[o + sp.r[2]];
+        for (int o = -sp.r[2]; o <= sp.r[2]; ++o) sp.tz.g[o + sp.rz_c + pgsf::kTapPad] = sp.taps[2].g[o + sp.r[2]];
     }
     p->fast_filter = fast;
     p->fast_stats = !force_generic && (desc->nx % 4 == 0) && pgsf::fast_stats_supported(p);

@@ -1,7 +1,307 @@
-// Tiled sm_100a filter kernels (placeholder until the fast path lands).
+// Tiled sm_100a kernels for the separable form of Eq. 2 (index ranges Eq. 3-5).
+//
+//   k_xy<R>  : per z-plane, x and y passes staged through shared memory (input tile + halo, zero
+//              filled outside the cube = the zero padding of reading C-5), result t2 to HBM.
+//   k_z<RZ>  : the frequency axis (filters are largest along z).  A CTA stages a slab of
+//              ZB + 2 RZ planes of a 128-column strip in shared memory; every thread owns four
+//              x columns and PZ consecutive channels and walks along z with its accumulators in
+//              registers.
+//
+// Both passes are plain FP32 FMAs: the inner loops are packed `fma.rn.f32x2` (SASS FFMA2) whose
+// tap operand is a kernel-parameter constant, i.e. a uniform register broadcast -- the sm_100a form
+// of the paper's "filter value is read from constant memory".  One FFMA2 retires two
+// voxel-taps per issue slot, which leaves issue slots for the shared-memory loads.
+//
+// Preconditions (checked by the plan): nx % 4 == 0, 16-byte aligned cubes, radius in the compiled
+// set (smaller radii run in the next larger window with exact-zero padding taps).
 #include "pgsf_internal.h"
+
 namespace pgsf {
-bool fast_xy_radius(int, int *c) { *c = 0; return false; }
-bool fast_z_radius(int, int *c) { *c = 0; return false; }
-cudaError_t fast_filter3d(pgsf_plan *, int, const float *, float *, float *, cudaStream_t) { return cudaErrorNotSupported; }
+namespace {
+
+// ------------------------------------------------------------------------------------ helpers
+
+__device__ __forceinline__ float2 ffma2(float2 a, float g, float2 c)
+{
+    // d = a * {g, g} + c, both halves in one instruction
+    const float2 gg = make_float2(g, g);
+    unsigned long long ra = *reinterpret_cast<const unsigned long long *>(&a);
+    unsigned long long rb = *reinterpret_cast<const unsigned long long *>(&gg);
+    unsigned long long rc = *reinterpret_cast<const unsigned long long *>(&c);
+    unsigned long long rd;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(rd) : "l"(ra), "l"(rb), "l"(rc));
+    return *reinterpret_cast<float2 *>(&rd);
+}
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem, bool valid)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    const int bytes = valid ? 16 : 0;  // src-size 0 -> 16 bytes of zeros
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gmem), "r"(bytes));
+}
+__device__ __forceinline__ void cp_async_wait_all()
+{
+    asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
+}
+
+constexpr int round4(int v) { return (v + 3) & ~3; }
+
+// ------------------------------------------------------------------------------------ x/y passes
+
+constexpr int XY_TX = 64;       // output tile
+constexpr int XY_TY = 32;
+constexpr int XY_THREADS = 256;
+constexpr int XY_PY = 4;        // y outputs per thread in the y pass
+constexpr int XY_QX = 8;        // x outputs per thread in the x pass
+
+template <int R>
+struct XYShape {
+    static constexpr int R4 = round4(R);
+    static constexpr int W = XY_TX + 2 * R4;   // staged columns
+    static constexpr int HI = XY_TY + 2 * R;   // staged rows
+    static constexpr int SMEM = (HI * W + XY_TY * W) * 4;
+};
+
+template <int R>
+__global__ void __launch_bounds__(XY_THREADS) k_xy(const float *__restrict__ in, float *__restrict__ out,
+                                                   Dims d, TapsXY t)
+{
+    using S = XYShape<R>;
+    extern __shared__ __align__(16) float smem[];
+    float *s_in = smem;                 // [HI][W]
+    float *s_t1 = smem + S::HI * S::W;  // [TY][W]
+    const int tid = threadIdx.x;
+    const int x0 = blockIdx.x * XY_TX, y0 = blockIdx.y * XY_TY, z = blockIdx.z;
+    const float *plane_in = in + (long long)z * d.plane;
+
+    // stage the input tile + halo; anything outside the cube becomes 0 (C-5)
+    constexpr int W4 = S::W / 4;
+    for (int i = tid; i < W4 * S::HI; i += XY_THREADS) {
+        const int r = i / W4, c4 = i - r * W4;
+        const int gy = y0 - R + r, gx = x0 - S::R4 + 4 * c4;
+        const bool ok = gy >= 0 && gy < d.ny && gx >= 0 && gx < d.nx;
+        const float *src = ok ? plane_in + (long long)gy * d.nx + gx : plane_in;
+        cp_async16(s_in + r * S::W + 4 * c4, src, ok);
+    }
+    cp_async_wait_all();
+    __syncthreads();
+
+    // y pass (Eq. 4): t1[y][x] = sum_o in[y+o][x] gy[o] for every staged column; pairs along x
+    constexpr int YB = XY_TY / XY_PY;
+    for (int task = tid; task < W4 * YB; task += XY_THREADS) {
+        const int yb = task / W4, c4 = task - yb * W4;
+        float2 acc[XY_PY][2];
+#pragma unroll
+        for (int p = 0; p < XY_PY; ++p) acc[p][0] = acc[p][1] = make_float2(0.f, 0.f);
+        const float *col = s_in + (yb * XY_PY) * S::W + 4 * c4;
+#pragma unroll
+        for (int j = 0; j < XY_PY + 2 * R; ++j) {
+            const float4 v = *reinterpret_cast<const float4 *>(col + j * S::W);
+#pragma unroll
+            for (int p = 0; p < XY_PY; ++p) {
+                const int o = j - p;
+                if (o >= 0 && o <= 2 * R) {
+                    acc[p][0] = ffma2(make_float2(v.x, v.y), t.gy[o], acc[p][0]);
+                    acc[p][1] = ffma2(make_float2(v.z, v.w), t.gy[o], acc[p][1]);
+                }
+            }
+        }
+#pragma unroll
+        for (int p = 0; p < XY_PY; ++p)
+            *reinterpret_cast<float4 *>(s_t1 + (yb * XY_PY + p) * S::W + 4 * c4) =
+                make_float4(acc[p][0].x, acc[p][0].y, acc[p][1].x, acc[p][1].y);
+    }
+    __syncthreads();
+
+    // x pass (Eq. 3): t2[y][x] = sum_o t1[y][x+o] gx[o]; each thread QX consecutive outputs
+    constexpr int XB = XY_TX / XY_QX;
+    for (int task = tid; task < XY_TY * XB; task += XY_THREADS) {
+        const int row = task / XB, xb = task - row * XB;
+        const int gy = y0 + row, gx = x0 + xb * XY_QX;
+        if (gy >= d.ny || gx >= d.nx) continue;
+        constexpr int NV = XY_QX + 2 * S::R4;
+        float v[NV];
+        const float *src = s_t1 + row * S::W + xb * XY_QX;  // staged column 0 <-> x0 - R4
+#pragma unroll
+        for (int j = 0; j < NV / 4; ++j) {
+            const float4 q = *reinterpret_cast<const float4 *>(src + 4 * j);
+            v[4 * j] = q.x; v[4 * j + 1] = q.y; v[4 * j + 2] = q.z; v[4 * j + 3] = q.w;
+        }
+        float acc[XY_QX];
+#pragma unroll
+        for (int i = 0; i < XY_QX; ++i) acc[i] = 0.f;
+#pragma unroll
+        for (int o = 0; o <= 2 * R; ++o)
+#pragma unroll
+            for (int i = 0; i < XY_QX; ++i) acc[i] = fmaf(v[i + o + (S::R4 - R)], t.gx[o], acc[i]);
+        float *dst = out + (long long)z * d.plane + (long long)gy * d.nx + gx;
+#pragma unroll
+        for (int i = 0; i < XY_QX; i += 4)
+            if (gx + i < d.nx)
+                *reinterpret_cast<float4 *>(dst + i) = make_float4(acc[i], acc[i + 1], acc[i + 2], acc[i + 3]);
+    }
+}
+
+// ------------------------------------------------------------------------------------ z pass
+
+constexpr int Z_XT = 128;       // columns per CTA (32 float4 lanes = one warp per plane row)
+constexpr int Z_PZ = 8;         // channels per thread
+constexpr int Z_WARPS = 8;      // z groups per CTA
+constexpr int Z_THREADS = 32 * Z_WARPS;
+constexpr int Z_ZB = Z_PZ * Z_WARPS;   // 64 output channels per CTA
+
+template <int RZ>
+struct ZShape {
+    static constexpr int PLANES = Z_ZB + 2 * RZ;
+    static constexpr int SMEM = PLANES * Z_XT * 4;
+};
+
+template <int RZ>
+__global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, float *__restrict__ out,
+                                                 Dims d, Taps t)
+{
+    using S = ZShape<RZ>;
+    extern __shared__ __align__(16) float smem[];  // [PLANES][Z_XT]
+    const int tid = threadIdx.x, lane = tid & 31, wz = tid >> 5;
+    const int z0 = blockIdx.x * Z_ZB, x0 = blockIdx.y * Z_XT, y = blockIdx.z;
+    const int gx = x0 + 4 * lane;
+    const bool col_ok = gx < d.nx;
+    const float *col_in = in + (long long)y * d.nx + (col_ok ? gx : 0);
+
+    // stage channels z0-RZ .. z0+ZB+RZ-1 of this 128-column strip; outside the cube -> 0 (C-5)
+    for (int pz = wz; pz < S::PLANES; pz += Z_WARPS) {
+        const int gz = z0 - RZ + pz;
+        const bool ok = col_ok && gz >= 0 && gz < d.nz;
+        cp_async16(smem + pz * Z_XT + 4 * lane, ok ? col_in + (long long)gz * d.plane : in, ok);
+    }
+    cp_async_wait_all();
+    __syncthreads();
+
+    // Eq. 5: f[z] = sum_o t2[z+o] gz[o]; the thread walks along z, PZ accumulators x 4 columns.
+    // Taps are stored at g[o + kTapPad] with kTapPad zeros on both sides.
+    float2 acc[Z_PZ][2];
+#pragma unroll
+    for (int p = 0; p < Z_PZ; ++p) acc[p][0] = acc[p][1] = make_float2(0.f, 0.f);
+    const float *base = smem + (wz * Z_PZ) * Z_XT + 4 * lane;
+    if constexpr (RZ <= 48) {
+        // fully unrolled: every tap index is a compile-time constant-bank offset
+#pragma unroll
+        for (int j = 0; j < Z_PZ + 2 * RZ; ++j) {
+            const float4 v = *reinterpret_cast<const float4 *>(base + j * Z_XT);
+#pragma unroll
+            for (int p = 0; p < Z_PZ; ++p) {
+                const int o = j - p;
+                if (o >= 0 && o <= 2 * RZ) {
+                    acc[p][0] = ffma2(make_float2(v.x, v.y), t.g[o + kTapPad], acc[p][0]);
+                    acc[p][1] = ffma2(make_float2(v.z, v.w), t.g[o + kTapPad], acc[p][1]);
+                }
+            }
+        }
+    } else {
+        // too long to unroll: walk the PZ + 2 RZ staged channels in chunks of 8; the zero padding of
+        // the tap array makes the ramp-up / ramp-down iterations the same code as the steady state
+        static_assert((Z_PZ + 2 * RZ) % 8 == 0 && kTapPad >= Z_PZ - 1, "chunking");
+#pragma unroll 1
+        for (int jc = 0; jc < Z_PZ + 2 * RZ; jc += 8) {
+#pragma unroll
+            for (int jj = 0; jj < 8; ++jj) {
+                const float4 v = *reinterpret_cast<const float4 *>(base + (jc + jj) * Z_XT);
+#pragma unroll
+                for (int p = 0; p < Z_PZ; ++p) {
+                    const float g = t.g[jc + jj - p + kTapPad];
+                    acc[p][0] = ffma2(make_float2(v.x, v.y), g, acc[p][0]);
+                    acc[p][1] = ffma2(make_float2(v.z, v.w), g, acc[p][1]);
+                }
+            }
+        }
+    }
+    if (!col_ok) return;
+    float *col_out = out + (long long)y * d.nx + gx;
+#pragma unroll
+    for (int p = 0; p < Z_PZ; ++p) {
+        const int gz = z0 + wz * Z_PZ + p;
+        if (gz < d.nz)
+            *reinterpret_cast<float4 *>(col_out + (long long)gz * d.plane) =
+                make_float4(acc[p][0].x, acc[p][0].y, acc[p][1].x, acc[p][1].y);
+    }
+}
+
+template <int R>
+cudaError_t launch_xy(const float *in, float *out, const Dims &d, const TapsXY &t, cudaStream_t st)
+{
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_xy<R>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             XYShape<R>::SMEM);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dim3 grid((d.nx + XY_TX - 1) / XY_TX, (d.ny + XY_TY - 1) / XY_TY, d.nz);
+    k_xy<R><<<grid, XY_THREADS, XYShape<R>::SMEM, st>>>(in, out, d, t);
+    return cudaGetLastError();
+}
+
+template <int RZ>
+cudaError_t launch_z(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st)
+{
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_z<RZ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             ZShape<RZ>::SMEM);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dim3 grid((d.nz + Z_ZB - 1) / Z_ZB, (d.nx + Z_XT - 1) / Z_XT, d.ny);
+    k_z<RZ><<<grid, Z_THREADS, ZShape<RZ>::SMEM, st>>>(in, out, d, t);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+bool fast_xy_radius(int r, int *c)
+{
+    static const int set[] = {3, 6, 9, 12};
+    for (int v : set)
+        if (r <= v) { *c = v; return true; }
+    *c = 0;
+    return false;
+}
+
+bool fast_z_radius(int r, int *c)
+{
+    static const int set[] = {6, 12, 24, 48, 72, 96};
+    for (int v : set)
+        if (r <= v) { *c = v; return true; }
+    *c = 0;
+    return false;
+}
+
+cudaError_t fast_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp,
+                          cudaStream_t st)
+{
+    const Dims &d = p->dims;
+    const ScalePlan &sp = p->scales[scale];
+    if (d.ny > 65535 || d.nz > 65535) return cudaErrorInvalidConfiguration;
+    cudaError_t e;
+    switch (sp.rxy_c) {
+    case 3: e = launch_xy<3>(in, tmp, d, sp.txy, st); break;
+    case 6: e = launch_xy<6>(in, tmp, d, sp.txy, st); break;
+    case 9: e = launch_xy<9>(in, tmp, d, sp.txy, st); break;
+    case 12: e = launch_xy<12>(in, tmp, d, sp.txy, st); break;
+    default: return cudaErrorNotSupported;
+    }
+    if (e != cudaSuccess) return e;
+    switch (sp.rz_c) {
+    case 6: e = launch_z<6>(tmp, out, d, sp.tz, st); break;
+    case 12: e = launch_z<12>(tmp, out, d, sp.tz, st); break;
+    case 24: e = launch_z<24>(tmp, out, d, sp.tz, st); break;
+    case 48: e = launch_z<48>(tmp, out, d, sp.tz, st); break;
+    case 72: e = launch_z<72>(tmp, out, d, sp.tz, st); break;
+    case 96: e = launch_z<96>(tmp, out, d, sp.tz, st); break;
+    default: return cudaErrorNotSupported;
+    }
+    p->launches += 2;
+    return e;
+}
+
 }  // namespace pgsf

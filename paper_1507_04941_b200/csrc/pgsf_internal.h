@@ -20,9 +20,10 @@ constexpr float kFlatGuard = 1e-5f;
 // bank 0, so a compile-time tap index becomes a uniform-register operand of FFMA/FFMA2 (the role
 // constant memory plays in the paper's kernel) without any per-module __constant__
 // state shared between plans.
+constexpr int kTapPad = 8;  // zero taps in front of (and behind) the z taps of the tiled kernel
 struct Taps {
-    float g[kMaxTaps + 3];  // g[o + r], o = -r..r; zero beyond
-    int r;
+    float g[kMaxTaps + 2 * kTapPad + 2];  // generic path: g[o + r], o = -r..r; zero beyond
+    int r;                                // tiled z pass:  g[o + r + kTapPad]
 };
 
 struct TapsXY {  // small radii only (x and y passes)
