@@ -1,0 +1,415 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the whole hot path (multi-scale filter + local threshold, every row of
+SURVEY.md 8(a)) on synthetic cubes shaped like BASELINE.json's configs.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config {1..5}] [--impl b200|reference]
+
+One "step" = one pgsf_find_multiscale call over one batch of synthetic input (all scales, filtered
+cubes kept as outputs, mask, count).  Prints ONE JSON line (rank 0).
+for the definition of every field.  N > 1 = N independent replicas (the path does not shard:
+DESIGN.md "Multi-GPU"), no data-path collective; the timing is the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Gvoxel/s per Gaussian scale (filter+threshold)"
+UNIT = "Gvoxel-scales/s"
+STATS_FLOPS = 21            # statistics + threshold per voxel per scale
+FP32_LANES_PER_SM = 128     # B200_PROFILING.md unit counts: 148 SMs, 1965 MHz max SM clock
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            j = json.load(fh)
+        return {"hbm_gbs": float(j["hbm_gbs"]), "sm_max_mhz": float(j.get("sm_max_mhz", 1965.0)),
+                "source": "measured (MEASURED_PEAKS.json)"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+def _alu_peak_tflops(sm_count: int, sm_mhz: float) -> float:
+    """FP32 CUDA-core peak: SMs x 128 lanes x 2 flop x clock."""
+    return sm_count * FP32_LANES_PER_SM * 2 * sm_mhz * 1e6 / 1e12
+
+
+def _radius(sigma: float, truncate: float) -> int:
+    import math
+    return int(math.ceil(truncate * sigma)) if sigma > 0 else 0
+
+
+def _taps(w):
+    """[(Tx, Ty, Tz)] per scale: the true tap counts 2 ceil(3 sigma) + 1."""
+    return [tuple(2 * _radius(s[a], w.truncate) + 1 for a in range(3)) for s in w.sigmas]
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------ CPU oracle leg
+
+CPU_SAMPLE = (256, 256, 512)   # cpu_baseline leg: ~10-30 s of host work
+REF_SAMPLE = (128, 128, 256)   # --impl reference: a few seconds per step, K steps within minutes
+
+
+def _oracle_sample_region(w, size=CPU_SAMPLE):
+    """The bounded sample the oracle is timed on: a centred brick of at most `size` voxels of the
+    workload's cube, all scales."""
+    lo = tuple(max(0, (n - s) // 2) for n, s in zip(w.dims, size))
+    hi = tuple(min(n, l + s) for n, l, s in zip(w.dims, lo, size))
+    return lo, hi
+
+
+def time_oracle(w, sub, a, lo, hi, repeats: int = 1):
+    """Seconds per pass of the fp64 oracle (as it stands, all host cores via its OpenMP loops) over
+    the sample region; returns (seconds, voxel_scales, threads)."""
+    from oracle import pgsf_oracle
+    pgsf_oracle.build()
+    threads = pgsf_oracle.set_threads(0)
+    best = None
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        pgsf_oracle.find_region(sub, a, w.dims, w.sigmas, w.box_half, w.k, lo, hi, w.halo, w.truncate)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    vs = (hi[0] - lo[0]) * (hi[1] - lo[1]) * (hi[2] - lo[2]) * len(w.sigmas)
+    return best, vs, threads
+
+
+def _sample_text(w, lo, hi):
+    return (f"centred brick {hi[0]-lo[0]}x{hi[1]-lo[1]}x{hi[2]-lo[2]} of {w.name}, all {len(w.sigmas)} scales, "
+            f"oracle region mode (input brick +-(r+h)); rate = brick voxel-scales / wall time")
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle (oracle/, fp64, gcc -O2 + OpenMP) on the host cores; every step is
+    one pass over the bounded sample of the same workload.  Rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import torch
+    from paper_1507_04941_b200 import synth
+    lo, hi = _oracle_sample_region(w, REF_SAMPLE)
+    # the sample brick is cut from the same seeded cube when a GPU is there to generate it quickly;
+    # otherwise (no GPU) an equally shaped seeded brick is generated on the host
+    from oracle import pgsf_oracle
+    a, e = pgsf_oracle.required_input_box(w.dims, w.sigmas, w.box_half, lo, hi, w.truncate)
+    shape = (e[2] - a[2], e[1] - a[1], e[0] - a[0])
+    if torch.cuda.is_available():
+        torch.cuda.set_device(0)
+        d = synth.make_workload(w, "cuda:0")
+        sub = d[0, a[2]:e[2], a[1]:e[1], a[0]:e[0]].cpu().numpy()
+        del d
+        torch.cuda.empty_cache()
+    else:
+        sub = synth.make_cube(shape, w.seed, max(1, w.n_sources // 64), device="cpu", sxy_range=w.sxy_range,
+                              sz_range=w.sz_range, amp_range=w.amp_range).numpy()
+    for _ in range(min(args.warmup, 1)):
+        time_oracle(w, sub, a, lo, hi)
+    t = []
+    threads = 1
+    for _ in range(args.steps):
+        dt, vs, threads = time_oracle(w, sub, a, lo, hi)
+        t.append(dt)
+    sec = sum(t) / len(t)
+    value = vs / sec / 1e9
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": sec * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "sample": _sample_text(w, lo, hi)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
+                         "sample": _sample_text(w, lo, hi)},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------ B200 arm
+
+def _kernel_work(name: str, w, taps, n_vox: int):
+    """Algorithmic (flops, bytes) of ONE launch of the kernel `name`: the work
+    the separable method must do, not what the implementation happens to move."""
+    S = len(taps)
+    kind, _, tail = name.partition("_")
+    if kind == "xy" and tail == "all":       # x and y passes of every scale from one read of the input
+        return 2 * sum(t[0] + t[1] for t in taps) * n_vox, (4 + 4 * S) * n_vox
+    if kind == "xy" and tail.startswith("s"):
+        t = taps[int(tail[1:])]
+        return 2 * (t[0] + t[1]) * n_vox, 8 * n_vox
+    if kind == "z" and tail.startswith("s"):
+        t = taps[int(tail[1:])]
+        return 2 * t[2] * n_vox, 8 * n_vox
+    if kind == "stats" and tail == "all":    # statistics of every scale, one mask write
+        return STATS_FLOPS * S * n_vox, (4 * S + 1) * n_vox
+    if kind == "stats":
+        return STATS_FLOPS * n_vox, 5 * n_vox
+    return 0, 0
+
+
+def run_b200(args, w):
+    import torch
+    import torch.distributed as dist
+    from paper_1507_04941_b200 import binding, build, synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a B200: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    binding.load_library()
+    props = torch.cuda.get_device_properties(local_rank)
+    peaks = _peaks()
+
+    # every rank runs its own replica of the workload (seed offset by rank)
+    from dataclasses import replace
+    wr = replace(w, seed=w.seed + 100 * rank) if rank else w
+    d = synth.make_workload(wr, dev)
+    n_vox = w.voxels
+    S = len(w.sigmas)
+    taps = _taps(w)
+    plan = binding.Plan(w.dims, w.sigmas, w.box_half, w.k, batch=w.batch, halo=w.halo, truncate=w.truncate,
+                        device=local_rank)
+    filt = [torch.empty_like(d) for _ in range(S)]
+    mask = torch.empty(d.shape, dtype=torch.uint8, device=dev)
+    cnt = torch.zeros(1, dtype=torch.int64, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        plan.pgsf_find_multiscale(d, d_filtered=filt, d_mask=mask, d_count=cnt, stream=stream)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    plan.pgsf_plan_set_profiling(True)
+    l0 = plan.pgsf_plan_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    launches = plan.pgsf_plan_launch_count() - l0
+    prof = plan.pgsf_plan_profile()
+    plan.pgsf_plan_set_profiling(False)
+    clocks = sampler.stop()
+    count = int(cnt.item())
+    if world > 1:
+        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = n_vox * S * world / (ms_step * 1e-3) / 1e9
+
+    # ---- roofline of the dominant kernel + of the whole path
+    alu_peak = _alu_peak_tflops(props.multi_processor_count, peaks["sm_max_mhz"])
+    hbm_peak = peaks["hbm_gbs"]
+    kern = []
+    for name, (n, ms) in prof.items():
+        fl, by = _kernel_work(name, w, taps, w.dims[0] * w.dims[1] * w.dims[2])
+        kern.append({"name": name, "launches": n, "ms_per_launch": ms / max(n, 1), "share": ms / max(ms_total, 1e-9),
+                     "flops": fl, "bytes": by})
+    kern.sort(key=lambda k: -k["share"])
+    roofline = None
+    if kern:
+        k0 = kern[0]
+        t_alu = k0["flops"] / (alu_peak * 1e12)
+        t_hbm = k0["bytes"] / (hbm_peak * 1e9)
+        sec = k0["ms_per_launch"] * 1e-3
+        if t_alu >= t_hbm:
+            ach = k0["flops"] / sec / 1e12
+            roofline = {"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak}
+        else:
+            ach = k0["bytes"] / sec / 1e9
+            roofline = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak}
+        roofline.update({"kernel": k0["name"], "ms_per_launch": k0["ms_per_launch"], "share_of_step": k0["share"],
+                         "traffic": None, "peak_source": ("148 SM x 128 lanes x 2 x sm_max_mhz" if t_alu >= t_hbm
+                                                          else peaks["source"])})
+    path_flops = sum(2 * sum(t) + STATS_FLOPS for t in taps) * n_vox
+    path_bytes = (4 + 4 * S + 1) * n_vox
+    t_path = max(path_flops / (alu_peak * 1e12), path_bytes / (hbm_peak * 1e9))
+    path = {"flops_per_voxel": path_flops / n_vox, "bytes_per_voxel": path_bytes / n_vox,
+            "roofline_ms": t_path * 1e3, "frac": t_path * 1e3 / ms_step,
+            "bound": "alu" if path_flops / (alu_peak * 1e12) >= path_bytes / (hbm_peak * 1e9) else "hbm"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": w.name, "dims_xyz": list(w.dims), "batch": w.batch, "halo": list(w.halo),
+                   "sigmas": [list(s) for s in w.sigmas], "box_half": list(w.box_half), "k": w.k,
+                   "voxels": n_vox, "scales": S, "filtered_cubes_kept": True, "count": count,
+                   "l2": "inputs larger than L2 (input %.1f GiB, outputs %.1f GiB per step)" % (
+                       n_vox * 4 / 2**30, n_vox * (4 * S + 1) / 2**30),
+                   "parallelism": "replicas only (no collective)"},
+        "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline, "path_roofline": path,
+        "kernels": [{"name": k["name"], "launches": k["launches"], "ms_per_launch": round(k["ms_per_launch"], 4),
+                     "share": round(k["share"], 4)} for k in kern],
+    }
+    return line, dict(plan=plan, d=d, filt=filt, mask=mask, cnt=cnt, rank=rank, world=world, dev=dev)
+
+
+def run_e2e(args, w, ctx):
+    """Same metric through pgsf_find_multiscale_host: HOST (pinned) buffers in and out, the
+    host->device copy of the cube and the device->host copy of mask + count inside the timed region."""
+    import torch
+    import torch.distributed as dist
+    plan, d, world, dev = ctx["plan"], ctx["d"], ctx["world"], ctx["dev"]
+    S = len(w.sigmas)
+    h_in = torch.empty(d.shape, dtype=torch.float32, pin_memory=True)
+    h_in.copy_(d)
+    expect = int(ctx["cnt"].item())
+    # free the device-resident buffers of the first leg: the host entry point owns its own staging
+    ctx["filt"].clear()
+    ctx["d"] = None
+    del d
+    plan._ws = None
+    torch.cuda.empty_cache()
+    h_mask = torch.empty(h_in.shape, dtype=torch.uint8, pin_memory=True)
+    steps = max(1, min(args.steps, 5))
+    count = 0
+    for _ in range(min(args.warmup, 2)):
+        _, count = plan.pgsf_find_multiscale_host(h_in, h_mask)
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        _, count = plan.pgsf_find_multiscale_host(h_in, h_mask)   # synchronises before returning
+    torch.cuda.synchronize()
+    sec = (time.perf_counter() - t0) / steps
+    if world > 1:
+        t = torch.tensor([sec], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        sec = float(t.item())
+    assert count == expect, f"host entry point count {count} != device path count {expect}"
+    return {"value": w.voxels * S * world / sec / 1e9, "unit": UNIT, "ms_per_step": sec * 1e3, "steps": steps,
+            "h2d_bytes_per_step": w.voxels * 4, "d2h_bytes_per_step": w.voxels + 8,
+            "api": "pgsf_find_multiscale_host (pinned host cube in; mask + count out)"}
+
+
+def run_cpu_baseline(w, sub, a, lo, hi):
+    sec, vs, threads = time_oracle(w, sub, a, lo, hi)
+    return {"value": vs / sec / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle", "seconds": sec,
+            "sample": _sample_text(w, lo, hi)}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5],
+                    help="BASELINE.json config (1-based); default 3 = the 8 GiB cube the north star is quoted on")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+    from paper_1507_04941_b200 import synth
+    w = synth.WORKLOADS[args.config]
+    if args.impl == "reference":
+        run_reference(args, w)
+        return
+    line, ctx = run_b200(args, w)
+    rank, world = ctx["rank"], ctx["world"]
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import pgsf_oracle
+        lo, hi = _oracle_sample_region(w)
+        a, e = pgsf_oracle.required_input_box(w.dims, w.sigmas, w.box_half, lo, hi, w.truncate)
+        sub = ctx["d"][0, a[2]:e[2], a[1]:e[1], a[0]:e[0]].cpu().numpy()
+    if not args.no_e2e:
+        line["e2e"] = run_e2e(args, w, ctx)
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        ctx["plan"].close()
+        cpu = run_cpu_baseline(w, sub, a, lo, hi)
+    line["cpu_baseline"] = cpu
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -156,6 +156,19 @@ PGSF_API pgsf_status pgsf_find_multiscale_host(pgsf_plan *plan, const float *h_i
  * gpu_launches evidence). */
 PGSF_API unsigned long long pgsf_plan_launch_count(const pgsf_plan *plan);
 
+/*
+ * Per-kernel device timing, for bench.py's roofline line.  pgsf_plan_set_profiling(plan, 1) clears
+ * the table and makes every later launch of this plan be bracketed by a cudaEvent pair recorded on
+ * the stream the kernel is launched on; 0 switches it off.  pgsf_plan_profile_collect waits for the
+ * pending events (it synchronises with those launches), adds their durations to the per-kernel-name
+ * totals and writes the number of names to *n_entries; pgsf_plan_profile_entry copies entry
+ * `index`: its name (NUL terminated, at most cap bytes), launch count and summed milliseconds.
+ */
+PGSF_API pgsf_status pgsf_plan_set_profiling(pgsf_plan *plan, int enable);
+PGSF_API pgsf_status pgsf_plan_profile_collect(pgsf_plan *plan, int *n_entries);
+PGSF_API pgsf_status pgsf_plan_profile_entry(const pgsf_plan *plan, int index, char *name, int cap,
+                                             unsigned long long *launches, double *ms_total);
+
 #ifdef __cplusplus
 }
 #endif

@@ -24,7 +24,8 @@ _STATUS = {0: "PGSF_OK", 1: "PGSF_ERR_INVALID_ARG", 2: "PGSF_ERR_UNSUPPORTED", 3
 
 EXPORTS = ["pgsf_plan_create", "pgsf_plan_destroy", "pgsf_plan_workspace_bytes", "pgsf_last_error",
            "pgsf_plan_get_taps", "pgsf_filter3d", "pgsf_local_threshold", "pgsf_find_multiscale",
-           "pgsf_find_multiscale_host", "pgsf_plan_launch_count"]
+           "pgsf_find_multiscale_host", "pgsf_plan_launch_count", "pgsf_plan_set_profiling",
+           "pgsf_plan_profile_collect", "pgsf_plan_profile_entry"]
 
 
 class PgsfError(RuntimeError):
@@ -73,6 +74,12 @@ def load_library() -> ctypes.CDLL:
         lib.pgsf_find_multiscale_host.restype = i
         lib.pgsf_plan_launch_count.argtypes = [vp]
         lib.pgsf_plan_launch_count.restype = ctypes.c_ulonglong
+        lib.pgsf_plan_set_profiling.argtypes = [vp, i]
+        lib.pgsf_plan_set_profiling.restype = i
+        lib.pgsf_plan_profile_collect.argtypes = [vp, ctypes.POINTER(i)]
+        lib.pgsf_plan_profile_collect.restype = i
+        lib.pgsf_plan_profile_entry.argtypes = [vp, i, ctypes.c_char_p, i, u64p, ctypes.POINTER(ctypes.c_double)]
+        lib.pgsf_plan_profile_entry.restype = i
         _lib = lib
     return _lib
 
@@ -145,6 +152,22 @@ class Plan:
 
     def pgsf_plan_launch_count(self) -> int:
         return int(self._lib.pgsf_plan_launch_count(self._h))
+
+    def pgsf_plan_set_profiling(self, enable: bool) -> None:
+        self._check(self._lib.pgsf_plan_set_profiling(self._h, int(bool(enable))))
+
+    def pgsf_plan_profile(self) -> dict:
+        """{kernel name: (launches, total ms)} of the launches since profiling was switched on
+        (synchronises with them)."""
+        n = ctypes.c_int(0)
+        self._check(self._lib.pgsf_plan_profile_collect(self._h, ctypes.byref(n)))
+        out = {}
+        for idx in range(n.value):
+            name = ctypes.create_string_buffer(64)
+            cnt, ms = ctypes.c_ulonglong(0), ctypes.c_double(0.0)
+            self._check(self._lib.pgsf_plan_profile_entry(self._h, idx, name, 64, ctypes.byref(cnt), ctypes.byref(ms)))
+            out[name.value.decode()] = (int(cnt.value), float(ms.value))
+        return out
 
     def workspace(self) -> Optional[torch.Tensor]:
         """A torch-owned device buffer of pgsf_plan_workspace_bytes() (allocated once)."""

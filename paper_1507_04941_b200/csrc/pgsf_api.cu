@@ -50,11 +50,51 @@ void make_taps(double sigma, int r, float *g /* 2r+1 */)
     for (int o = -r; o <= r; ++o) g[o + r] = (float)(w[o + r] / sum);
 }
 
+cudaEvent_t take_event(pgsf_plan *p)
+{
+    cudaEvent_t e = nullptr;
+    if (!p->prof_free.empty()) {
+        e = p->prof_free.back();
+        p->prof_free.pop_back();
+    } else if (cudaEventCreate(&e) != cudaSuccess) {
+        cudaGetLastError();
+        e = nullptr;
+    }
+    return e;
+}
+
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 size_t round256(size_t v) { return (v + 255u) & ~(size_t)255u; }
 
 }  // namespace
+
+namespace pgsf {
+
+LaunchScope::LaunchScope(pgsf_plan *plan, const char *name, cudaStream_t stream) : p(plan), st(stream), b(nullptr)
+{
+    p->launches += 1;
+    if (!p->prof_on) return;
+    int id = -1;
+    for (size_t i = 0; i < p->prof_acc.size(); ++i)
+        if (p->prof_acc[i].name == name) { id = (int)i; break; }
+    if (id < 0) {
+        p->prof_acc.push_back(ProfAcc{name, 0ULL, 0.0});
+        id = (int)p->prof_acc.size() - 1;
+    }
+    cudaEvent_t a = take_event(p);
+    b = take_event(p);
+    if (!a || !b) { if (a) p->prof_free.push_back(a); if (b) p->prof_free.push_back(b); b = nullptr; return; }
+    cudaEventRecord(a, st);
+    p->prof_recs.push_back(ProfRec{id, a, b});
+}
+
+LaunchScope::~LaunchScope()
+{
+    if (b) cudaEventRecord(b, st);
+}
+
+}  // namespace pgsf
 
 extern "C" {
 
@@ -114,6 +154,7 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
     p->dims.plane = (long long)desc->nx * desc->ny;
     p->dims.cube = p->dims.plane * desc->nz;
     p->launches = 0;
+    p->prof_on = false;
     p->h_d_in = nullptr;
     p->h_d_mask = nullptr;
     p->h_d_count = nullptr;
@@ -167,7 +208,49 @@ pgsf_status pgsf_plan_destroy(pgsf_plan *p)
         for (int s = 0; s < PGSF_MAX_SCALES; ++s) cudaFree(p->h_d_f[s]);
         if (p->h_stream) cudaStreamDestroy(p->h_stream);
     }
+    for (auto &r : p->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (auto e : p->prof_free) cudaEventDestroy(e);
     delete p;
+    return PGSF_OK;
+}
+
+pgsf_status pgsf_plan_set_profiling(pgsf_plan *p, int enable)
+{
+    if (!p) return PGSF_ERR_INVALID_ARG;
+    for (auto &r : p->prof_recs) { p->prof_free.push_back(r.a); p->prof_free.push_back(r.b); }
+    p->prof_recs.clear();
+    p->prof_acc.clear();
+    p->prof_on = enable != 0;
+    return PGSF_OK;
+}
+
+pgsf_status pgsf_plan_profile_collect(pgsf_plan *p, int *n_entries)
+{
+    if (!p || !n_entries) return PGSF_ERR_INVALID_ARG;
+    for (auto &r : p->prof_recs) {
+        cudaError_t e = cudaEventSynchronize(r.b);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, r.a, r.b);
+        if (e != cudaSuccess) return cuda_fail(p, e, "profile collect");
+        p->prof_acc[r.name_id].launches += 1;
+        p->prof_acc[r.name_id].ms += ms;
+        p->prof_free.push_back(r.a);
+        p->prof_free.push_back(r.b);
+    }
+    p->prof_recs.clear();
+    *n_entries = (int)p->prof_acc.size();
+    return PGSF_OK;
+}
+
+pgsf_status pgsf_plan_profile_entry(const pgsf_plan *p, int index, char *name, int cap,
+                                    unsigned long long *launches, double *ms_total)
+{
+    if (!p || index < 0 || index >= (int)p->prof_acc.size() || !name || cap < 1)
+        return PGSF_ERR_INVALID_ARG;
+    const pgsf::ProfAcc &a = p->prof_acc[index];
+    snprintf(name, cap, "%s", a.name.c_str());
+    if (launches) *launches = a.launches;
+    if (ms_total) *ms_total = a.ms;
     return PGSF_OK;
 }
 

@@ -14,6 +14,8 @@
 //
 // Preconditions (checked by the plan): nx % 4 == 0, 16-byte aligned cubes, radius in the compiled
 // set (smaller radii run in the next larger window with exact-zero padding taps).
+#include <stdio.h>
+
 #include "pgsf_internal.h"
 
 namespace pgsf {
@@ -283,24 +285,32 @@ cudaError_t fast_filter3d(pgsf_plan *p, int scale, const float *in, float *out, 
     const ScalePlan &sp = p->scales[scale];
     if (d.ny > 65535 || d.nz > 65535) return cudaErrorInvalidConfiguration;
     cudaError_t e;
-    switch (sp.rxy_c) {
-    case 3: e = launch_xy<3>(in, tmp, d, sp.txy, st); break;
-    case 6: e = launch_xy<6>(in, tmp, d, sp.txy, st); break;
-    case 9: e = launch_xy<9>(in, tmp, d, sp.txy, st); break;
-    case 12: e = launch_xy<12>(in, tmp, d, sp.txy, st); break;
-    default: return cudaErrorNotSupported;
+    char name[32];
+    snprintf(name, sizeof name, "xy_s%d", scale);
+    {
+        LaunchScope ls(p, name, st);
+        switch (sp.rxy_c) {
+        case 3: e = launch_xy<3>(in, tmp, d, sp.txy, st); break;
+        case 6: e = launch_xy<6>(in, tmp, d, sp.txy, st); break;
+        case 9: e = launch_xy<9>(in, tmp, d, sp.txy, st); break;
+        case 12: e = launch_xy<12>(in, tmp, d, sp.txy, st); break;
+        default: return cudaErrorNotSupported;
+        }
     }
     if (e != cudaSuccess) return e;
-    switch (sp.rz_c) {
-    case 6: e = launch_z<6>(tmp, out, d, sp.tz, st); break;
-    case 12: e = launch_z<12>(tmp, out, d, sp.tz, st); break;
-    case 24: e = launch_z<24>(tmp, out, d, sp.tz, st); break;
-    case 48: e = launch_z<48>(tmp, out, d, sp.tz, st); break;
-    case 72: e = launch_z<72>(tmp, out, d, sp.tz, st); break;
-    case 96: e = launch_z<96>(tmp, out, d, sp.tz, st); break;
-    default: return cudaErrorNotSupported;
+    snprintf(name, sizeof name, "z_s%d", scale);
+    {
+        LaunchScope ls(p, name, st);
+        switch (sp.rz_c) {
+        case 6: e = launch_z<6>(tmp, out, d, sp.tz, st); break;
+        case 12: e = launch_z<12>(tmp, out, d, sp.tz, st); break;
+        case 24: e = launch_z<24>(tmp, out, d, sp.tz, st); break;
+        case 48: e = launch_z<48>(tmp, out, d, sp.tz, st); break;
+        case 72: e = launch_z<72>(tmp, out, d, sp.tz, st); break;
+        case 96: e = launch_z<96>(tmp, out, d, sp.tz, st); break;
+        default: return cudaErrorNotSupported;
+        }
     }
-    p->launches += 2;
     return e;
 }
 

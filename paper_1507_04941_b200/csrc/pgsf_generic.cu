@@ -126,10 +126,9 @@ cudaError_t generic_filter3d(pgsf_plan *p, int scale, const float *in, float *ou
     const Dims &d = p->dims;
     const ScalePlan &sp = p->scales[scale];
     const unsigned g = grid_for(d.cube);
-    k_conv1d<0><<<g, kThreads, 0, st>>>(in, tmp_a, d, sp.taps[0]);
-    k_conv1d<1><<<g, kThreads, 0, st>>>(tmp_a, tmp_b, d, sp.taps[1]);
-    k_conv1d<2><<<g, kThreads, 0, st>>>(tmp_b, out, d, sp.taps[2]);
-    p->launches += 3;
+    { LaunchScope ls(p, "generic_conv_x", st); k_conv1d<0><<<g, kThreads, 0, st>>>(in, tmp_a, d, sp.taps[0]); }
+    { LaunchScope ls(p, "generic_conv_y", st); k_conv1d<1><<<g, kThreads, 0, st>>>(tmp_a, tmp_b, d, sp.taps[1]); }
+    { LaunchScope ls(p, "generic_conv_z", st); k_conv1d<2><<<g, kThreads, 0, st>>>(tmp_b, out, d, sp.taps[2]); }
     return cudaGetLastError();
 }
 
@@ -140,14 +139,16 @@ cudaError_t generic_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int o
     const unsigned g = grid_for(d.cube);
     float *x1 = tmp4, *x2 = tmp4 + d.cube, *y1 = tmp4 + 2 * d.cube, *y2 = tmp4 + 3 * d.cube;
     const int *h = p->desc.box_half;
-    k_boxsum<0, true><<<g, kThreads, 0, st>>>(f, nullptr, x1, x2, d, h[0]);
-    k_boxsum<1, false><<<g, kThreads, 0, st>>>(x1, x2, y1, y2, d, h[1]);
-    k_boxsum<2, false><<<g, kThreads, 0, st>>>(y1, y2, x1, x2, d, h[2]);
+    { LaunchScope ls(p, "generic_boxsum_x", st); k_boxsum<0, true><<<g, kThreads, 0, st>>>(f, nullptr, x1, x2, d, h[0]); }
+    { LaunchScope ls(p, "generic_boxsum_y", st); k_boxsum<1, false><<<g, kThreads, 0, st>>>(x1, x2, y1, y2, d, h[1]); }
+    { LaunchScope ls(p, "generic_boxsum_z", st); k_boxsum<2, false><<<g, kThreads, 0, st>>>(y1, y2, x1, x2, d, h[2]); }
     const float k = (float)p->desc.k;
-    k_threshold<<<g, kThreads, 0, st>>>(f, x1, x2, mask, or_into, mean, sd, count, d, h[0], h[1], h[2],
-                                        p->desc.halo[0], p->desc.halo[1], p->desc.halo[2], k,
-                                        (float)(p->desc.k * p->desc.k));
-    p->launches += 4;
+    {
+        LaunchScope ls(p, "generic_threshold", st);
+        k_threshold<<<g, kThreads, 0, st>>>(f, x1, x2, mask, or_into, mean, sd, count, d, h[0], h[1], h[2],
+                                            p->desc.halo[0], p->desc.halo[1], p->desc.halo[2], k,
+                                            (float)(p->desc.k * p->desc.k));
+    }
     return cudaGetLastError();
 }
 

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string>
+#include <vector>
 
 #include "pgsf.h"
 
@@ -48,6 +49,20 @@ struct Dims {
 
 }  // namespace pgsf
 
+namespace pgsf {
+// Optional per-kernel timing (pgsf_plan_set_profiling): one cudaEvent pair around every launch, on
+// the stream the kernel is launched on; durations are summed per kernel name on collect.
+struct ProfRec {
+    int name_id;
+    cudaEvent_t a, b;
+};
+struct ProfAcc {
+    std::string name;
+    unsigned long long launches;
+    double ms;
+};
+}  // namespace pgsf
+
 struct pgsf_plan {
     pgsf_plan_desc desc;
     double sigmas[PGSF_MAX_SCALES * 3];
@@ -61,6 +76,10 @@ struct pgsf_plan {
     size_t ws_cube_bytes;
     unsigned long long launches;
     std::string err;
+    bool prof_on;
+    std::vector<pgsf::ProfRec> prof_recs;      // pending (not yet collected) launches
+    std::vector<cudaEvent_t> prof_free;        // recycled events
+    std::vector<pgsf::ProfAcc> prof_acc;
     // plan-owned device staging for pgsf_find_multiscale_host
     float *h_d_in;
     float *h_d_f[PGSF_MAX_SCALES];
@@ -71,6 +90,15 @@ struct pgsf_plan {
 };
 
 namespace pgsf {
+
+// Counts a launch and, when profiling is on, brackets it with events on `st`.
+struct LaunchScope {
+    pgsf_plan *p;
+    cudaStream_t st;
+    cudaEvent_t b;
+    LaunchScope(pgsf_plan *plan, const char *name, cudaStream_t stream);
+    ~LaunchScope();
+};
 
 // ---- generic kernels (pgsf_generic.cu): any shape, any radius <= PGSF_MAX_RADIUS ----------------
 cudaError_t generic_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp_a,
