@@ -190,7 +190,7 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
 
     // workspace: [scratch filtered cube][filter temporaries][statistics temporaries]
     p->ws_cube_bytes = round256((size_t)p->dims.cube * sizeof(float));
-    const size_t cubes = 1 + (p->fast_filter ? 1 : 2) + (p->fast_stats ? 0 : 4);
+    const size_t cubes = 1 + (p->fast_filter ? 1 : 2) + (p->fast_stats ? 2 : 4);
     p->ws_bytes = cubes * p->ws_cube_bytes;
     *out = p;
     return PGSF_OK;
@@ -279,7 +279,7 @@ namespace {
 struct Workspace {
     float *scratch;  // 1 cube
     float *ftmp;     // 1 or 2 cubes
-    float *stmp;     // 0 or 4 cubes
+    float *stmp;     // 2 or 4 cubes
 };
 
 Workspace carve(const pgsf_plan *p, void *ws)
@@ -310,12 +310,18 @@ pgsf_status filter_one(pgsf_plan *p, int scale, const float *in, float *out, con
     return PGSF_OK;
 }
 
-pgsf_status threshold_one(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean,
-                          float *sd, unsigned long long *count, const Workspace &w, cudaStream_t st)
+// statistics + selection of `batch` consecutive cubes starting at f / mask (/ mean / sd)
+pgsf_status threshold_batch(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean,
+                            float *sd, unsigned long long *count, int batch, const Workspace &w,
+                            cudaStream_t st)
 {
-    cudaError_t e;
-    if (p->fast_stats) e = pgsf::fast_threshold(p, f, mask, or_into, mean, sd, count, st);
-    else e = pgsf::generic_threshold(p, f, mask, or_into, mean, sd, count, w.stmp, st);
+    cudaError_t e = cudaSuccess;
+    for (int bi = 0; bi < batch && e == cudaSuccess; ++bi) {
+        const size_t off = (size_t)bi * p->dims.cube;
+        float *m = mean ? mean + off : nullptr, *s = sd ? sd + off : nullptr;
+        if (p->fast_stats) e = pgsf::fast_threshold(p, f + off, mask + off, or_into, m, s, count, w.stmp, st);
+        else e = pgsf::generic_threshold(p, f + off, mask + off, or_into, m, s, count, w.stmp, st);
+    }
     if (e != cudaSuccess) return cuda_fail(p, e, "threshold launch");
     return PGSF_OK;
 }
@@ -368,13 +374,7 @@ pgsf_status pgsf_local_threshold(pgsf_plan *p, const float *d_f, uint8_t *d_mask
         e = cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), st);
         if (e != cudaSuccess) return cuda_fail(p, e, "cudaMemsetAsync(count)");
     }
-    for (int bi = 0; bi < p->desc.batch; ++bi) {
-        const size_t off = (size_t)bi * p->dims.cube;
-        s = threshold_one(p, d_f + off, d_mask + off, or_into, d_mean ? d_mean + off : nullptr,
-                          d_std ? d_std + off : nullptr, d_count, w, st);
-        if (s != PGSF_OK) return s;
-    }
-    return PGSF_OK;
+    return threshold_batch(p, d_f, d_mask, or_into, d_mean, d_std, d_count, p->desc.batch, w, st);
 }
 
 pgsf_status pgsf_find_multiscale(pgsf_plan *p, const float *d_in, float *const *d_filtered,
@@ -401,14 +401,22 @@ pgsf_status pgsf_find_multiscale(pgsf_plan *p, const float *d_in, float *const *
         e = cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), st);
         if (e != cudaSuccess) return cuda_fail(p, e, "cudaMemsetAsync(count)");
     }
-    for (int bi = 0; bi < p->desc.batch; ++bi) {
-        const size_t off = (size_t)bi * p->dims.cube;
-        for (int s = 0; s < S; ++s) {
-            float *f = (d_filtered && d_filtered[s]) ? d_filtered[s] + off : w.scratch;
+    const int B = p->desc.batch;
+    for (int s = 0; s < S; ++s) {
+        unsigned long long *cnt = (s == S - 1) ? d_count : nullptr;
+        float *keep = d_filtered ? d_filtered[s] : nullptr;
+        for (int bi = 0; bi < B; ++bi) {
+            const size_t off = (size_t)bi * p->dims.cube;
+            float *f = keep ? keep + off : w.scratch;
             rc = filter_one(p, s, d_in + off, f, w, st);
             if (rc != PGSF_OK) return rc;
-            rc = threshold_one(p, f, d_mask + off, s > 0, nullptr, nullptr,
-                               (s == S - 1) ? d_count : nullptr, w, st);
+            if (!keep) {   // one scratch cube: threshold this entry before it is overwritten
+                rc = threshold_batch(p, f, d_mask + off, s > 0, nullptr, nullptr, cnt, 1, w, st);
+                if (rc != PGSF_OK) return rc;
+            }
+        }
+        if (keep) {        // the whole batch of kept cubes in one launch
+            rc = threshold_batch(p, keep, d_mask, s > 0, nullptr, nullptr, cnt, B, w, st);
             if (rc != PGSF_OK) return rc;
         }
     }

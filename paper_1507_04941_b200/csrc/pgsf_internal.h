@@ -113,7 +113,8 @@ bool fast_z_radius(int r, int *compiled);
 cudaError_t fast_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp,
                           cudaStream_t st);
 bool fast_stats_supported(const pgsf_plan *p);
+// tmp2: 2 cubes (the z-direction window sums of f and f^2)
 cudaError_t fast_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean,
-                           float *sd, unsigned long long *count, cudaStream_t st);
+                           float *sd, unsigned long long *count, float *tmp2, cudaStream_t st);
 
 }  // namespace pgsf
