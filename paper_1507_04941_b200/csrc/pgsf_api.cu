@@ -402,21 +402,38 @@ pgsf_status pgsf_find_multiscale(pgsf_plan *p, const float *d_in, float *const *
         if (e != cudaSuccess) return cuda_fail(p, e, "cudaMemsetAsync(count)");
     }
     const int B = p->desc.batch;
-    for (int s = 0; s < S; ++s) {
-        unsigned long long *cnt = (s == S - 1) ? d_count : nullptr;
-        float *keep = d_filtered ? d_filtered[s] : nullptr;
+    bool all_kept = d_filtered != nullptr;
+    for (int s = 0; s < S && all_kept; ++s) all_kept = d_filtered[s] != nullptr;
+    if (p->fast_filter && all_kept) {
+        // x and y passes of all scales from ONE read of the input; the x/y-filtered cube of scale s
+        // is parked in the output cube of scale s+1 (the last one in the workspace), so the z passes
+        // run in order s = 0..S-1, each freeing the cube the next one writes to
+        int idx[PGSF_MAX_SCALES];
+        for (int s = 0; s < S; ++s) idx[s] = s;
         for (int bi = 0; bi < B; ++bi) {
             const size_t off = (size_t)bi * p->dims.cube;
-            float *f = keep ? keep + off : w.scratch;
-            rc = filter_one(p, s, d_in + off, f, w, st);
-            if (rc != PGSF_OK) return rc;
-            if (!keep) {   // one scratch cube: threshold this entry before it is overwritten
-                rc = threshold_batch(p, f, d_mask + off, s > 0, nullptr, nullptr, cnt, 1, w, st);
+            float *park[PGSF_MAX_SCALES];
+            for (int s = 0; s < S; ++s) park[s] = (s + 1 < S) ? d_filtered[s + 1] + off : w.ftmp;
+            cudaError_t ce = pgsf::fast_xy_multi(p, idx, S, d_in + off, park, st);
+            if (ce != cudaSuccess) return cuda_fail(p, ce, "xy filter launch");
+            for (int s = 0; s < S; ++s) {
+                ce = pgsf::fast_z(p, s, park[s], d_filtered[s] + off, st);
+                if (ce != cudaSuccess) return cuda_fail(p, ce, "z filter launch");
+                rc = threshold_batch(p, d_filtered[s] + off, d_mask + off, s > 0, nullptr, nullptr,
+                                     (s == S - 1) ? d_count : nullptr, 1, w, st);
                 if (rc != PGSF_OK) return rc;
             }
         }
-        if (keep) {        // the whole batch of kept cubes in one launch
-            rc = threshold_batch(p, keep, d_mask, s > 0, nullptr, nullptr, cnt, B, w, st);
+        return PGSF_OK;
+    }
+    for (int bi = 0; bi < B; ++bi) {
+        const size_t off = (size_t)bi * p->dims.cube;
+        for (int s = 0; s < S; ++s) {
+            float *f = (d_filtered && d_filtered[s]) ? d_filtered[s] + off : w.scratch;
+            rc = filter_one(p, s, d_in + off, f, w, st);
+            if (rc != PGSF_OK) return rc;
+            rc = threshold_batch(p, f, d_mask + off, s > 0, nullptr, nullptr, (s == S - 1) ? d_count : nullptr,
+                                 1, w, st);
             if (rc != PGSF_OK) return rc;
         }
     }

@@ -46,61 +46,65 @@ __device__ __forceinline__ void cp_async_wait_all()
     asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
 }
 
-constexpr int round4(int v) { return (v + 3) & ~3; }
+__host__ __device__ constexpr int round4(int v) { return (v + 3) & ~3; }
 
 // ------------------------------------------------------------------------------------ x/y passes
+//
+// k_xy_multi<RMAX>: one z plane tile of 128 x 32 voxels.  The input tile + RMAX halo is staged ONCE
+// (zero fill outside the cube, C-5) and the x and y passes of EVERY scale of the bank are evaluated
+// from it ("several sigma scales evaluated per input read", BASELINE.json north_star): the input cube
+// is read once for all scales instead of once per scale.
+//   y pass (Eq. 4): thread = 4 staged columns x 4 rows; walks down the staged rows (LDS.128), packed
+//                   FFMA2 over x pairs; result stored with the rows of a row PAIR interleaved,
+//                   t1[(row/2)][col][row%2], so that
+//   x pass (Eq. 3): thread = 2 rows x 8 columns; one LDS.128 yields two columns of both rows as two
+//                   (row, row+1) register pairs, i.e. the x pass is packed FFMA2 over row pairs.
 
-constexpr int XY_TX = 64;       // output tile
-constexpr int XY_TY = 32;
-constexpr int XY_THREADS = 256;
-constexpr int XY_PY = 4;        // y outputs per thread in the y pass
-constexpr int XY_QX = 8;        // x outputs per thread in the x pass
+constexpr int XM_TX = 128;
+constexpr int XM_TY = 32;
+constexpr int XM_NT = 256;
+constexpr int XM_PY = 4;        // rows per thread in the y pass
+constexpr int XM_QX = 8;        // columns per thread in the x pass (times two rows)
 
-template <int R>
-struct XYShape {
-    static constexpr int R4 = round4(R);
-    static constexpr int W = XY_TX + 2 * R4;   // staged columns
-    static constexpr int HI = XY_TY + 2 * R;   // staged rows
-    static constexpr int SMEM = (HI * W + XY_TY * W) * 4;
+struct XYMultiParams {
+    Dims d;
+    int n;                          // scales in this launch
+    int rc[PGSF_MAX_SCALES];        // compiled radius of each
+    float *out[PGSF_MAX_SCALES];    // x/y-filtered plane stack of each
+    TapsXY t[PGSF_MAX_SCALES];
 };
 
-template <int R>
-__global__ void __launch_bounds__(XY_THREADS) k_xy(const float *__restrict__ in, float *__restrict__ out,
-                                                   Dims d, TapsXY t)
+template <int RMAX>
+struct XMShape {
+    static constexpr int R4M = round4(RMAX);
+    static constexpr int W = XM_TX + 2 * R4M;                    // staged columns
+    static constexpr int HI = XM_TY + 2 * RMAX;                  // staged rows
+    static constexpr int WT = W + ((2 - W % 16) + 16) % 16;      // t1 pitch in columns, = 2 (mod 16):
+                                                                 // row pairs 4 banks apart
+    static constexpr int SMEM = (HI * W + XM_TY * WT) * 4;
+};
+
+template <int R, int RMAX>
+__device__ __forceinline__ void xy_one_scale(const float *s_in, float *s_t1, float *__restrict__ out_plane,
+                                             const TapsXY &t, const Dims &d, int x0, int y0, int tid)
 {
-    using S = XYShape<R>;
-    extern __shared__ __align__(16) float smem[];
-    float *s_in = smem;                 // [HI][W]
-    float *s_t1 = smem + S::HI * S::W;  // [TY][W]
-    const int tid = threadIdx.x;
-    const int x0 = blockIdx.x * XY_TX, y0 = blockIdx.y * XY_TY, z = blockIdx.z;
-    const float *plane_in = in + (long long)z * d.plane;
-
-    // stage the input tile + halo; anything outside the cube becomes 0 (C-5)
-    constexpr int W4 = S::W / 4;
-    for (int i = tid; i < W4 * S::HI; i += XY_THREADS) {
-        const int r = i / W4, c4 = i - r * W4;
-        const int gy = y0 - R + r, gx = x0 - S::R4 + 4 * c4;
-        const bool ok = gy >= 0 && gy < d.ny && gx >= 0 && gx < d.nx;
-        const float *src = ok ? plane_in + (long long)gy * d.nx + gx : plane_in;
-        cp_async16(s_in + r * S::W + 4 * c4, src, ok);
-    }
-    cp_async_wait_all();
-    __syncthreads();
-
-    // y pass (Eq. 4): t1[y][x] = sum_o in[y+o][x] gy[o] for every staged column; pairs along x
-    constexpr int YB = XY_TY / XY_PY;
-    for (int task = tid; task < W4 * YB; task += XY_THREADS) {
-        const int yb = task / W4, c4 = task - yb * W4;
-        float2 acc[XY_PY][2];
+    using S = XMShape<RMAX>;
+    constexpr int R4 = round4(R);
+    constexpr int C0 = S::R4M - R4;                 // first staged column this scale needs
+    constexpr int W4s = (XM_TX + 2 * R4) / 4;
+    constexpr int YB = XM_TY / XM_PY;
+    // ---- y pass
+    for (int task = tid; task < W4s * YB; task += XM_NT) {
+        const int yb = task / W4s, c4 = task - yb * W4s;
+        float2 acc[XM_PY][2];
 #pragma unroll
-        for (int p = 0; p < XY_PY; ++p) acc[p][0] = acc[p][1] = make_float2(0.f, 0.f);
-        const float *col = s_in + (yb * XY_PY) * S::W + 4 * c4;
+        for (int p = 0; p < XM_PY; ++p) acc[p][0] = acc[p][1] = make_float2(0.f, 0.f);
+        const float *col = s_in + (yb * XM_PY + (RMAX - R)) * S::W + C0 + 4 * c4;
 #pragma unroll
-        for (int j = 0; j < XY_PY + 2 * R; ++j) {
+        for (int j = 0; j < XM_PY + 2 * R; ++j) {
             const float4 v = *reinterpret_cast<const float4 *>(col + j * S::W);
 #pragma unroll
-            for (int p = 0; p < XY_PY; ++p) {
+            for (int p = 0; p < XM_PY; ++p) {
                 const int o = j - p;
                 if (o >= 0 && o <= 2 * R) {
                     acc[p][0] = ffma2(make_float2(v.x, v.y), t.gy[o], acc[p][0]);
@@ -109,38 +113,98 @@ __global__ void __launch_bounds__(XY_THREADS) k_xy(const float *__restrict__ in,
             }
         }
 #pragma unroll
-        for (int p = 0; p < XY_PY; ++p)
-            *reinterpret_cast<float4 *>(s_t1 + (yb * XY_PY + p) * S::W + 4 * c4) =
-                make_float4(acc[p][0].x, acc[p][0].y, acc[p][1].x, acc[p][1].y);
+        for (int jj = 0; jj < XM_PY / 2; ++jj) {
+            float *dst = s_t1 + ((yb * (XM_PY / 2) + jj) * S::WT + C0 + 4 * c4) * 2;
+            const float2 a0 = acc[2 * jj][0], a1 = acc[2 * jj][1], b0 = acc[2 * jj + 1][0], b1 = acc[2 * jj + 1][1];
+            *reinterpret_cast<float4 *>(dst) = make_float4(a0.x, b0.x, a0.y, b0.y);
+            *reinterpret_cast<float4 *>(dst + 4) = make_float4(a1.x, b1.x, a1.y, b1.y);
+        }
     }
     __syncthreads();
-
-    // x pass (Eq. 3): t2[y][x] = sum_o t1[y][x+o] gx[o]; each thread QX consecutive outputs
-    constexpr int XB = XY_TX / XY_QX;
-    for (int task = tid; task < XY_TY * XB; task += XY_THREADS) {
-        const int row = task / XB, xb = task - row * XB;
-        const int gy = y0 + row, gx = x0 + xb * XY_QX;
-        if (gy >= d.ny || gx >= d.nx) continue;
-        constexpr int NV = XY_QX + 2 * S::R4;
-        float v[NV];
-        const float *src = s_t1 + row * S::W + xb * XY_QX;  // staged column 0 <-> x0 - R4
+    // ---- x pass
+    {
+        const int jp = tid & (XM_TY / 2 - 1), xb = tid / (XM_TY / 2);
+        constexpr int CS = S::R4M - R;              // staged column of tap o = 0 of output column 0
+        constexpr int SH = CS & 1;                  // float4 loads start at an even column
+        constexpr int NL = (XM_QX + 2 * R + SH + 1) / 2;
+        float2 v[2 * NL];
+        const float *src = s_t1 + (jp * S::WT + (CS - SH) + XM_QX * xb) * 2;
 #pragma unroll
-        for (int j = 0; j < NV / 4; ++j) {
-            const float4 q = *reinterpret_cast<const float4 *>(src + 4 * j);
-            v[4 * j] = q.x; v[4 * j + 1] = q.y; v[4 * j + 2] = q.z; v[4 * j + 3] = q.w;
+        for (int k = 0; k < NL; ++k) {
+            const float4 q = *reinterpret_cast<const float4 *>(src + 4 * k);
+            v[2 * k] = make_float2(q.x, q.y);
+            v[2 * k + 1] = make_float2(q.z, q.w);
         }
-        float acc[XY_QX];
+        float2 acc[XM_QX];
 #pragma unroll
-        for (int i = 0; i < XY_QX; ++i) acc[i] = 0.f;
+        for (int i = 0; i < XM_QX; ++i) acc[i] = make_float2(0.f, 0.f);
 #pragma unroll
         for (int o = 0; o <= 2 * R; ++o)
 #pragma unroll
-            for (int i = 0; i < XY_QX; ++i) acc[i] = fmaf(v[i + o + (S::R4 - R)], t.gx[o], acc[i]);
-        float *dst = out + (long long)z * d.plane + (long long)gy * d.nx + gx;
-#pragma unroll
-        for (int i = 0; i < XY_QX; i += 4)
-            if (gx + i < d.nx)
-                *reinterpret_cast<float4 *>(dst + i) = make_float4(acc[i], acc[i + 1], acc[i + 2], acc[i + 3]);
+            for (int i = 0; i < XM_QX; ++i) acc[i] = ffma2(v[i + o + SH], t.gx[o], acc[i]);
+        const int gy = y0 + 2 * jp, gx = x0 + XM_QX * xb;
+        if (gx < d.nx) {
+            float *dst = out_plane + (long long)gy * d.nx + gx;
+            const bool second = gx + 4 < d.nx;
+            if (gy < d.ny) {
+                *reinterpret_cast<float4 *>(dst) = make_float4(acc[0].x, acc[1].x, acc[2].x, acc[3].x);
+                if (second) *reinterpret_cast<float4 *>(dst + 4) = make_float4(acc[4].x, acc[5].x, acc[6].x, acc[7].x);
+            }
+            if (gy + 1 < d.ny) {
+                *reinterpret_cast<float4 *>(dst + d.nx) = make_float4(acc[0].y, acc[1].y, acc[2].y, acc[3].y);
+                if (second)
+                    *reinterpret_cast<float4 *>(dst + d.nx + 4) = make_float4(acc[4].y, acc[5].y, acc[6].y, acc[7].y);
+            }
+        }
+    }
+}
+
+template <int RMAX>
+__global__ void __launch_bounds__(XM_NT) k_xy_multi(const float *__restrict__ in,
+                                                     const __grid_constant__ XYMultiParams P)
+{
+    using S = XMShape<RMAX>;
+    extern __shared__ __align__(16) float smem[];
+    float *s_in = smem;                  // [HI][W]
+    float *s_t1 = smem + S::HI * S::W;   // [TY/2][WT][2]
+    const Dims &d = P.d;
+    const int tid = threadIdx.x;
+    const int x0 = blockIdx.x * XM_TX, y0 = blockIdx.y * XM_TY, z = blockIdx.z;
+    const long long plane_off = (long long)z * d.plane;
+
+    // stage the input tile + halo: thread <-> one 16-byte column chunk, rows r0, r0 + RP, ...
+    {
+        constexpr int W4 = S::W / 4, RP = XM_NT / W4;
+        if (tid < RP * W4) {
+            const int c4 = tid % W4, r0 = tid / W4;
+            const int xx = x0 - S::R4M + 4 * c4;
+            const bool xok = xx >= 0 && xx < d.nx;
+            int yy = y0 - RMAX + r0;
+            long long off = plane_off + (long long)yy * d.nx + xx;
+            float *dst = s_in + r0 * S::W + 4 * c4;
+            for (int r = r0; r < S::HI; r += RP) {
+                const bool ok = xok && yy >= 0 && yy < d.ny;
+                cp_async16(dst, in + (ok ? off : 0), ok);
+                yy += RP;
+                off += (long long)RP * d.nx;
+                dst += RP * S::W;
+            }
+        }
+        cp_async_wait_all();
+        __syncthreads();
+    }
+
+    for (int s = 0; s < P.n; ++s) {
+        if (s > 0) __syncthreads();      // the previous scale's x pass has read s_t1
+        float *out_plane = P.out[s] + plane_off;
+        const TapsXY &t = P.t[s];
+        switch (P.rc[s]) {
+        case 3: xy_one_scale<3, RMAX>(s_in, s_t1, out_plane, t, d, x0, y0, tid); break;
+        case 6: if constexpr (RMAX >= 6) xy_one_scale<6, RMAX>(s_in, s_t1, out_plane, t, d, x0, y0, tid); break;
+        case 9: if constexpr (RMAX >= 9) xy_one_scale<9, RMAX>(s_in, s_t1, out_plane, t, d, x0, y0, tid); break;
+        case 12: if constexpr (RMAX >= 12) xy_one_scale<12, RMAX>(s_in, s_t1, out_plane, t, d, x0, y0, tid); break;
+        default: break;
+        }
     }
 }
 
@@ -228,18 +292,18 @@ __global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, f
     }
 }
 
-template <int R>
-cudaError_t launch_xy(const float *in, float *out, const Dims &d, const TapsXY &t, cudaStream_t st)
+template <int RMAX>
+cudaError_t launch_xy_multi(const float *in, const XYMultiParams &P, cudaStream_t st)
 {
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_xy<R>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             XYShape<R>::SMEM);
+        cudaError_t e = cudaFuncSetAttribute(k_xy_multi<RMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             XMShape<RMAX>::SMEM);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    dim3 grid((d.nx + XY_TX - 1) / XY_TX, (d.ny + XY_TY - 1) / XY_TY, d.nz);
-    k_xy<R><<<grid, XY_THREADS, XYShape<R>::SMEM, st>>>(in, out, d, t);
+    dim3 grid((P.d.nx + XM_TX - 1) / XM_TX, (P.d.ny + XM_TY - 1) / XM_TY, P.d.nz);
+    k_xy_multi<RMAX><<<grid, XM_NT, XMShape<RMAX>::SMEM, st>>>(in, P);
     return cudaGetLastError();
 }
 
@@ -278,40 +342,64 @@ bool fast_z_radius(int r, int *c)
     return false;
 }
 
-cudaError_t fast_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp,
+// x and y passes of the scales `scales[0..n)` of one cube: in -> out[i] (x/y-filtered cubes)
+cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *in, float *const *out,
                           cudaStream_t st)
 {
     const Dims &d = p->dims;
-    const ScalePlan &sp = p->scales[scale];
-    if (d.ny > 65535 || d.nz > 65535) return cudaErrorInvalidConfiguration;
-    cudaError_t e;
+    if (d.ny > 65535 * XM_TY || d.nz > 65535 || n < 1 || n > PGSF_MAX_SCALES) return cudaErrorInvalidConfiguration;
+    XYMultiParams P;
+    P.d = d;
+    P.n = n;
+    int rmax = 0;
+    for (int i = 0; i < n; ++i) {
+        const ScalePlan &sp = p->scales[scales[i]];
+        P.rc[i] = sp.rxy_c;
+        P.out[i] = out[i];
+        P.t[i] = sp.txy;
+        if (sp.rxy_c > rmax) rmax = sp.rxy_c;
+    }
+    for (int i = n; i < PGSF_MAX_SCALES; ++i) { P.rc[i] = 0; P.out[i] = nullptr; }
     char name[32];
-    snprintf(name, sizeof name, "xy_s%d", scale);
-    {
-        LaunchScope ls(p, name, st);
-        switch (sp.rxy_c) {
-        case 3: e = launch_xy<3>(in, tmp, d, sp.txy, st); break;
-        case 6: e = launch_xy<6>(in, tmp, d, sp.txy, st); break;
-        case 9: e = launch_xy<9>(in, tmp, d, sp.txy, st); break;
-        case 12: e = launch_xy<12>(in, tmp, d, sp.txy, st); break;
-        default: return cudaErrorNotSupported;
-        }
+    if (n == 1) snprintf(name, sizeof name, "xy_s%d", scales[0]);
+    else snprintf(name, sizeof name, "xy_all");
+    LaunchScope ls(p, name, st);
+    switch (rmax) {
+    case 3: return launch_xy_multi<3>(in, P, st);
+    case 6: return launch_xy_multi<6>(in, P, st);
+    case 9: return launch_xy_multi<9>(in, P, st);
+    case 12: return launch_xy_multi<12>(in, P, st);
+    default: return cudaErrorNotSupported;
     }
-    if (e != cudaSuccess) return e;
+}
+
+// frequency pass of one scale: in (x/y-filtered cube) -> out
+cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStream_t st)
+{
+    const Dims &d = p->dims;
+    const ScalePlan &sp = p->scales[scale];
+    if (d.ny > 65535 || d.nz > 65535 * Z_ZB) return cudaErrorInvalidConfiguration;
+    char name[32];
     snprintf(name, sizeof name, "z_s%d", scale);
-    {
-        LaunchScope ls(p, name, st);
-        switch (sp.rz_c) {
-        case 6: e = launch_z<6>(tmp, out, d, sp.tz, st); break;
-        case 12: e = launch_z<12>(tmp, out, d, sp.tz, st); break;
-        case 24: e = launch_z<24>(tmp, out, d, sp.tz, st); break;
-        case 48: e = launch_z<48>(tmp, out, d, sp.tz, st); break;
-        case 72: e = launch_z<72>(tmp, out, d, sp.tz, st); break;
-        case 96: e = launch_z<96>(tmp, out, d, sp.tz, st); break;
-        default: return cudaErrorNotSupported;
-        }
+    LaunchScope ls(p, name, st);
+    switch (sp.rz_c) {
+    case 6: return launch_z<6>(in, out, d, sp.tz, st);
+    case 12: return launch_z<12>(in, out, d, sp.tz, st);
+    case 24: return launch_z<24>(in, out, d, sp.tz, st);
+    case 48: return launch_z<48>(in, out, d, sp.tz, st);
+    case 72: return launch_z<72>(in, out, d, sp.tz, st);
+    case 96: return launch_z<96>(in, out, d, sp.tz, st);
+    default: return cudaErrorNotSupported;
     }
-    return e;
+}
+
+cudaError_t fast_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp,
+                          cudaStream_t st)
+{
+    float *outs[1] = {tmp};
+    cudaError_t e = fast_xy_multi(p, &scale, 1, in, outs, st);
+    if (e != cudaSuccess) return e;
+    return fast_z(p, scale, tmp, out, st);
 }
 
 }  // namespace pgsf

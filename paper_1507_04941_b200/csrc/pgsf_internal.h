@@ -112,6 +112,9 @@ bool fast_xy_radius(int r, int *compiled);
 bool fast_z_radius(int r, int *compiled);
 cudaError_t fast_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp,
                           cudaStream_t st);
+cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *in, float *const *out,
+                          cudaStream_t st);
+cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStream_t st);
 bool fast_stats_supported(const pgsf_plan *p);
 // tmp2: 2 cubes (the z-direction window sums of f and f^2)
 cudaError_t fast_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean,

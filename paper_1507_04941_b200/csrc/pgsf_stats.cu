@@ -206,32 +206,50 @@ __global__ void __launch_bounds__(ST_NT, 2) k_xybox(const float *__restrict__ f,
     constexpr int W = ST_TX + 2 * HX;   // staged columns
     constexpr int W4 = W / 4;
     constexpr int WP = W + 4;           // row pitch: WP/4 odd -> conflict-free 16-byte accesses down a column
+    constexpr int RP = ST_NT / W4;      // staged rows per pass of the CTA
     extern __shared__ __align__(16) float smem[];
     const int H = ST_TY + 2 * p.hy;     // staged rows
     float *s_a = smem;                  // Z1 tile + halo, then its x-direction sums
     float *s_b = s_a + H * WP;          // Z2 likewise
     float *s_f = s_b + H * WP;          // centre values f of the tile [ST_TY][ST_TX]
-    uint8_t *s_m = reinterpret_cast<uint8_t *>(s_f + ST_TY * ST_TX);   // previous mask of the tile (OR mode)
+    uint8_t *s_m = reinterpret_cast<uint8_t *>(s_f + ST_TY * ST_TX);   // mask bytes of the tile [ST_TY][ST_TX]
     const Dims &d = p.d;
     const int tid = threadIdx.x;
     const int x0 = blockIdx.x * ST_TX, y0 = blockIdx.y * ST_TY, z = blockIdx.z;
     const long long plane_off = (long long)z * d.plane;
 
-    for (int i = tid; i < W4 * H; i += ST_NT) {
-        const int r = i / W4, c4 = i - r * W4;
-        const int yy = y0 - p.hy + r, xx = x0 - HX + 4 * c4;
-        const bool ok = yy >= 0 && yy < d.ny && xx >= 0 && xx < d.nx;
-        const long long off = ok ? plane_off + (long long)yy * d.nx + xx : 0;
-        st_cp_async16(s_a + r * WP + 4 * c4, Z1 + off, ok);
-        st_cp_async16(s_b + r * WP + 4 * c4, Z2 + off, ok);
+    // stage Z1 / Z2: thread <-> one 16-byte column chunk, rows r0, r0 + RP, ...
+    if (tid < RP * W4) {
+        const int c4 = tid % W4, r0 = tid / W4;
+        const int xx = x0 - HX + 4 * c4;
+        const bool xok = xx >= 0 && xx < d.nx;
+        int yy = y0 - p.hy + r0;
+        long long off = plane_off + (long long)yy * d.nx + xx;
+        float *da = s_a + r0 * WP + 4 * c4, *db = s_b + r0 * WP + 4 * c4;
+        for (int r = r0; r < H; r += RP) {
+            const bool ok = xok && yy >= 0 && yy < d.ny;
+            const long long o = ok ? off : 0;
+            st_cp_async16(da, Z1 + o, ok);
+            st_cp_async16(db, Z2 + o, ok);
+            yy += RP;
+            off += (long long)RP * d.nx;
+            da += RP * WP;
+            db += RP * WP;
+        }
     }
-    for (int i = tid; i < (ST_TX / 4) * ST_TY; i += ST_NT) {
-        const int r = i / (ST_TX / 4), c4 = i - r * (ST_TX / 4);
-        const int yy = y0 + r, xx = x0 + 4 * c4;
-        const bool ok = yy < d.ny && xx < d.nx;
-        const long long off = ok ? plane_off + (long long)yy * d.nx + xx : 0;
-        st_cp_async16(s_f + r * ST_TX + 4 * c4, f + off, ok);
-        if (p.or_into) st_cp_async4(s_m + r * ST_TX + 4 * c4, mask + off, ok);
+    // stage the centre values (and, in OR mode, the previous mask) of the tile
+    {
+        const int c4 = tid & 31, r0 = tid >> 5;
+        const int xx = x0 + 4 * c4;
+        const bool xok = xx < d.nx;
+#pragma unroll
+        for (int k = 0; k < ST_TY / 8; ++k) {
+            const int r = r0 + 8 * k, yy = y0 + r;
+            const bool ok = xok && yy < d.ny;
+            const long long o = ok ? plane_off + (long long)yy * d.nx + xx : 0;
+            st_cp_async16(s_f + r * ST_TX + 4 * c4, f + o, ok);
+            if (p.or_into) st_cp_async4(s_m + r * ST_TX + 4 * c4, mask + o, ok);
+        }
     }
     st_cp_async_wait();
     __syncthreads();
@@ -248,35 +266,55 @@ __global__ void __launch_bounds__(ST_NT, 2) k_xybox(const float *__restrict__ f,
     __syncthreads();
 
     // y direction + selection: column cx of the tile, rows ry0 .. ry0 + ST_ROWS - 1
-    const int cx = tid & (ST_TX - 1);
-    const int ry0 = (tid >> 7) * ST_ROWS;
-    const int gx = x0 + cx;
-    unsigned my_count = 0;
-    if (gx < d.nx) {
+    {
+        const int cx = tid & (ST_TX - 1);
+        const int ry0 = (tid >> 7) * ST_ROWS;
+        const int gx = x0 + cx;
         float S1[ST_ROWS], S2[ST_ROWS];
         ybox(s_a + ry0 * WP + cx, WP, p.hy, S1);
         ybox(s_b + ry0 * WP + cx, WP, p.hy, S2);
-        const float nxz = (float)clipped_len(gx, HX, d.nx) * (float)clipped_len(z, p.hz, d.nz);
+        const float nxz = (float)clipped_len(min(gx, d.nx - 1), HX, d.nx) * (float)clipped_len(z, p.hz, d.nz);
+        const bool y_inside = y0 - p.hy >= 0 && y0 + ST_TY - 1 + p.hy < d.ny;   // no row of the tile is clipped
+        const float n_in = nxz * (float)(2 * p.hy + 1);
+        const bool halo = (p.gx | p.gy | p.gz) != 0;
         const bool core_xz = gx >= p.gx && gx < d.nx - p.gx && z >= p.gz && z < d.nz - p.gz;
+        const float *vf = s_f + ry0 * ST_TX + cx;
+        uint8_t *vm = s_m + ry0 * ST_TX + cx;
 #pragma unroll
         for (int i = 0; i < ST_ROWS; ++i) {
             const int gy = y0 + ry0 + i;
-            if (gy >= d.ny) break;
-            const long long idx = plane_off + (long long)gy * d.nx + gx;
-            const float n = nxz * (float)clipped_len(gy, p.hy, d.ny);
-            const float v = s_f[(ry0 + i) * ST_TX + cx], s1 = S1[i], s2 = S2[i];
+            const float n = y_inside ? n_in : nxz * (float)clipped_len(min(gy, d.ny - 1), p.hy, d.ny);
+            const float v = vf[i * ST_TX], s1 = S1[i], s2 = S2[i];
             const float a = fmaf(n, v, -s1);
             const float q = fmaxf(fmaf(n, s2, -s1 * s1), 0.f);
             int sel = (a > kFlatGuard * n * fabsf(v)) && (a * a > p.k2 * q);
-            const bool core = core_xz && gy >= p.gy && gy < d.ny - p.gy;
-            if (!core) sel = 0;
-            else if (p.or_into) sel |= (s_m[(ry0 + i) * ST_TX + cx] != 0);
-            mask[idx] = (uint8_t)sel;
-            my_count += sel;
-            if (mean != nullptr || sd != nullptr) {
+            if (halo && !(core_xz && gy >= p.gy && gy < d.ny - p.gy)) sel = 0;
+            else if (p.or_into) sel |= (vm[i * ST_TX] != 0);
+            vm[i * ST_TX] = (uint8_t)sel;
+            if ((mean != nullptr || sd != nullptr) && gx < d.nx && gy < d.ny) {
+                const long long idx = plane_off + (long long)gy * d.nx + gx;
                 const float m = s1 / n;
                 if (mean != nullptr) mean[idx] = m;
                 if (sd != nullptr) sd[idx] = sqrtf(fmaxf(s2 / n - m * m, 0.f));
+            }
+        }
+    }
+    __syncthreads();
+
+    // mask tile -> global, 4 bytes per thread and row pass (one 128-byte row per warp); count = popcount
+    unsigned my_count = 0;
+    {
+        const int c4 = tid & 31, r0 = tid >> 5;
+        const int xx = x0 + 4 * c4;
+        if (xx < d.nx) {
+#pragma unroll
+            for (int k = 0; k < ST_TY / 8; ++k) {
+                const int r = r0 + 8 * k, yy = y0 + r;
+                if (yy < d.ny) {
+                    const unsigned w = *reinterpret_cast<const unsigned *>(s_m + r * ST_TX + 4 * c4);
+                    *reinterpret_cast<unsigned *>(mask + plane_off + (long long)yy * d.nx + xx) = w;
+                    my_count += __popc(w);
+                }
             }
         }
     }
