@@ -89,238 +89,269 @@ __global__ void __launch_bounds__(ZB_NT) k_zbox(const float4 *__restrict__ f, fl
     }
 }
 
-// ------------------------------------------------------------------------------------ k_xybox
+// ------------------------------------------------------------------------------------ k_ymarch
+//
+// One CTA = one z plane, one x tile, one y chunk.  A thread owns G = hx/2 adjacent columns and
+// marches down y with the y-direction window sums  Y1 = sum_{|o|<=hy} Z1(y+o),  Y2 likewise  in
+// registers (row entering the window added, row leaving it subtracted; the leaving row was read
+// 2 hy + 1 steps earlier, so it comes from L2).  Y2 is Kahan-compensated for the same reason as in
+// k_zbox; Y1 only enters through the mean, whose tolerance is ~n times looser, and stays plain.
+// The x-direction window of 2 hx + 1 = 4 G + 1 columns is then exactly
+//      (suffix of the thread two to the left) + (the three threads in between) + (prefix of the
+//      thread two to the right),
+// so every thread publishes the G prefix and G suffix sums of its own columns in shared memory and
+// combines five neighbours' values: ~4 additions per voxel, every output a plain sum of the elements
+// of its own window (no cancellation).  One __syncthreads per row (double-buffered exchange).
 
-constexpr int ST_TX = 128;
-constexpr int ST_TY = 32;
-constexpr int ST_NT = 256;
-constexpr int ST_L = 32;              // x-direction outputs per thread
-constexpr int ST_ROWS = ST_TY / 2;    // y-direction outputs per thread (two threads per column)
-constexpr int ST_MAX_HY = 16;
+constexpr int YM_MAX_NT = 256;
 
-struct XyboxParams {
+struct YmParams {
     Dims d;
     int hy, hz;
     int gx, gy, gz;      // halo excluded from mask and count (C-11)
     int or_into;
     float k2;            // k^2
+    int wo;              // output columns per x tile (tiles overlap by 2 hx staged columns)
+    int ntiles;
+    int ychunk;          // rows per CTA
 };
 
-__device__ __forceinline__ void st_cp_async16(void *smem, const void *gmem, bool valid)
-{
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    const int bytes = valid ? 16 : 0;  // src-size 0 -> 16 bytes of zeros
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gmem), "r"(bytes));
-}
-__device__ __forceinline__ void st_cp_async4(void *smem, const void *gmem, bool valid)
-{
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    const int bytes = valid ? 4 : 0;
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(s), "l"(gmem), "r"(bytes));
-}
-__device__ __forceinline__ void st_cp_async_wait()
-{
-    asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
-}
+template <int G> struct VecT { using type = float4; static constexpr int L = 4; };
+template <> struct VecT<2> { using type = float2; static constexpr int L = 2; };
 
 __device__ __forceinline__ int clipped_len(int c, int h, int n)
 {
     return min(c + h, n - 1) - max(c - h, 0) + 1;
 }
 
-// x-direction window sums of one staged row segment, in place:
-//   row[i] <- sum_{e = i .. i + 2 HX} row[e],  i = 0 .. ST_L - 1   (row has ST_L + 2 HX valid elements)
-// van Herk / Gil-Werman with blocks of WN = 2 HX + 1 elements: h = suffix sum inside a block,
-// g = prefix sum inside a block, out[i] = h[i] + g[i + WN - 1] (just h[i] when i starts a block).
-// All indices are compile-time; the four segments of a row sit in one warp, hence __syncwarp
-// between the last read and the first write.
-template <int HX>
-__device__ __forceinline__ void xbox_inplace(float *row, bool active)
+template <int G>
+__device__ __forceinline__ void ld_cols(const float *__restrict__ p, bool ok, float (&v)[G])
 {
-    constexpr int WN = 2 * HX + 1;
-    constexpr int N = ST_L + 2 * HX;
-    float o[ST_L];
-    if (active) {
-        float g[N], h[N];
+    if constexpr (G == 2) {
+        const float2 t = ok ? __ldg(reinterpret_cast<const float2 *>(p)) : make_float2(0.f, 0.f);
+        v[0] = t.x; v[1] = t.y;
+    } else {
 #pragma unroll
-        for (int q = 0; q < N / 4; ++q) {
-            const float4 v = *reinterpret_cast<const float4 *>(row + 4 * q);
-            g[4 * q] = v.x; g[4 * q + 1] = v.y; g[4 * q + 2] = v.z; g[4 * q + 3] = v.w;
+        for (int q = 0; q < G / 4; ++q) {
+            const float4 t = ok ? __ldg(reinterpret_cast<const float4 *>(p) + q) : make_float4(0.f, 0.f, 0.f, 0.f);
+            v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
         }
-#pragma unroll
-        for (int e = 0; e < N; ++e) h[e] = g[e];
-#pragma unroll
-        for (int e = 1; e < N; ++e)
-            if (e % WN != 0) g[e] = g[e - 1] + g[e];
-#pragma unroll
-        for (int e = N - 2; e >= 0; --e)
-            if (e % WN != WN - 1) h[e] = h[e + 1] + h[e];
-#pragma unroll
-        for (int i = 0; i < ST_L; ++i) o[i] = (i % WN == 0) ? h[i] : h[i] + g[i + WN - 1];
-    }
-    __syncwarp();
-    if (active) {
-#pragma unroll
-        for (int q = 0; q < ST_L / 4; ++q)
-            *reinterpret_cast<float4 *>(row + 4 * q) = make_float4(o[4 * q], o[4 * q + 1], o[4 * q + 2], o[4 * q + 3]);
     }
 }
 
-// y-direction window sums down one staged column: out[r] = sum_{q = r .. r + 2 hy} col[q * pitch],
-// r = 0 .. ST_ROWS - 1.  For 2 hy + 1 >= ST_ROWS the same two-block decomposition as in x (block 0 =
-// rows 0 .. 2 hy, block 1 = the rows below); shorter windows are summed directly.
-__device__ __forceinline__ void ybox(const float *col, int pitch, int hy, float (&out)[ST_ROWS])
+template <int G>
+struct YmRow {          // everything one march step reads from global memory
+    float l1[G], l2[G];  // row entering the window
+    float t1[G], t2[G];  // row leaving it
+    float fc[G];         // centre values
+    unsigned mk[(G + 3) / 4];   // previous mask bytes (OR mode)
+};
+
+template <int G>
+__device__ __forceinline__ void ym_load(YmRow<G> &r, const float *__restrict__ f, const float *__restrict__ Z1,
+                                        const float *__restrict__ Z2, const uint8_t *__restrict__ mask,
+                                        long long col_off, int y, const YmParams &p, bool col_ok)
 {
-    const int wy = 2 * hy;
-    if (wy + 1 >= ST_ROWS) {
-        float tail = 0.f;                      // rows ST_ROWS .. 2 hy, common to every suffix
-        for (int q = wy; q >= ST_ROWS; --q) tail += col[q * pitch];
-        float h = tail;
+    const int nx = p.d.nx, ny = p.d.ny;
+    const int yl = y + p.hy, yt = y - p.hy;
+    const bool okl = col_ok && yl < ny, okt = col_ok && yt >= 0, okc = col_ok && y < ny;
+    const long long ol = okl ? col_off + (long long)yl * nx : 0;
+    const long long ot = okt ? col_off + (long long)yt * nx : 0;
+    const long long oc = okc ? col_off + (long long)y * nx : 0;
+    ld_cols<G>(Z1 + ol, okl, r.l1);
+    ld_cols<G>(Z2 + ol, okl, r.l2);
+    ld_cols<G>(Z1 + ot, okt, r.t1);
+    ld_cols<G>(Z2 + ot, okt, r.t2);
+    ld_cols<G>(f + oc, okc, r.fc);
+    if (p.or_into) {
+        if constexpr (G == 2) r.mk[0] = okc ? *reinterpret_cast<const unsigned short *>(mask + oc) : 0u;
+        else {
 #pragma unroll
-        for (int r = ST_ROWS - 1; r >= 0; --r) {
-            h += col[r * pitch];
-            out[r] = h;                        // suffix of block 0 starting at row r
-        }
-        float g = 0.f;
-#pragma unroll
-        for (int r = 1; r < ST_ROWS; ++r) {
-            g += col[(r + wy) * pitch];        // prefix of block 1 up to row r + 2 hy
-            out[r] += g;
+            for (int q = 0; q < G / 4; ++q) r.mk[q] = okc ? *reinterpret_cast<const unsigned *>(mask + oc + 4 * q) : 0u;
         }
     } else {
 #pragma unroll
-        for (int r = 0; r < ST_ROWS; ++r) {
-            float s = 0.f;
-            for (int q = 0; q <= wy; ++q) s += col[(r + q) * pitch];
-            out[r] = s;
-        }
+        for (int q = 0; q < (G + 3) / 4; ++q) r.mk[q] = 0u;
     }
 }
 
-template <int HX>
-__global__ void __launch_bounds__(ST_NT, 2) k_xybox(const float *__restrict__ f, const float *__restrict__ Z1,
-                                                   const float *__restrict__ Z2, uint8_t *__restrict__ mask,
-                                                   float *__restrict__ mean, float *__restrict__ sd,
-                                                   unsigned long long *__restrict__ count, XyboxParams p)
+template <int G>
+__global__ void __launch_bounds__(YM_MAX_NT) k_ymarch(const float *__restrict__ f, const float *__restrict__ Z1,
+                                                      const float *__restrict__ Z2, uint8_t *__restrict__ mask,
+                                                      float *__restrict__ mean, float *__restrict__ sd,
+                                                      unsigned long long *__restrict__ count, const YmParams p)
 {
-    constexpr int W = ST_TX + 2 * HX;   // staged columns
-    constexpr int W4 = W / 4;
-    constexpr int WP = W + 4;           // row pitch: WP/4 odd -> conflict-free 16-byte accesses down a column
-    constexpr int RP = ST_NT / W4;      // staged rows per pass of the CTA
-    extern __shared__ __align__(16) float smem[];
-    const int H = ST_TY + 2 * p.hy;     // staged rows
-    float *s_a = smem;                  // Z1 tile + halo, then its x-direction sums
-    float *s_b = s_a + H * WP;          // Z2 likewise
-    float *s_f = s_b + H * WP;          // centre values f of the tile [ST_TY][ST_TX]
-    uint8_t *s_m = reinterpret_cast<uint8_t *>(s_f + ST_TY * ST_TX);   // mask bytes of the tile [ST_TY][ST_TX]
+    using V = typename VecT<G>::type;
+    constexpr int VL = VecT<G>::L, NV = G / VL, HX = 2 * G;
+    extern __shared__ __align__(16) unsigned char ym_smem[];
+    V *sm = reinterpret_cast<V *>(ym_smem);
+    const int NT = blockDim.x, SL = NT + 4, tid = threadIdx.x;
+    // exchange buffers [parity][array Y1/Y2][prefix/suffix][NV][SL]; thread t lives in slot t + 2,
+    // the two slots on either side stay zero (= nothing beyond the staged columns)
+    auto buf = [&](int par, int arr, int kind, int v) -> V * { return sm + ((((par * 2 + arr) * 2 + kind) * NV + v) * SL); };
+    for (int i = tid; i < 32 * NV; i += NT) {
+        V *b = sm + (i / 4) * SL;
+        const int e = i & 3;
+        V z;
+        if constexpr (G == 2) z = make_float2(0.f, 0.f); else z = make_float4(0.f, 0.f, 0.f, 0.f);
+        b[e < 2 ? e : NT + e] = z;
+    }
     const Dims &d = p.d;
-    const int tid = threadIdx.x;
-    const int x0 = blockIdx.x * ST_TX, y0 = blockIdx.y * ST_TY, z = blockIdx.z;
-    const long long plane_off = (long long)z * d.plane;
+    const int z = blockIdx.z;
+    const int out_lo = (p.ntiles == 1) ? 0 : blockIdx.x * p.wo;
+    const int out_hi = (p.ntiles == 1) ? d.nx : min(d.nx, out_lo + p.wo);
+    const int xs = (p.ntiles == 1) ? 0 : out_lo - HX;
+    const int c0 = xs + G * tid;                       // first of this thread's G columns
+    const bool col_ok = c0 >= 0 && c0 + G <= d.nx;     // (extents are multiples of the vector width)
+    const long long col_off = (long long)z * d.plane + (col_ok ? c0 : 0);
+    const int ya = blockIdx.y * p.ychunk, yb = min(ya + p.ychunk, d.ny);
+    const bool is_out = col_ok && c0 >= out_lo && c0 < out_hi;
 
-    // stage Z1 / Z2: thread <-> one 16-byte column chunk, rows r0, r0 + RP, ...
-    if (tid < RP * W4) {
-        const int c4 = tid % W4, r0 = tid / W4;
-        const int xx = x0 - HX + 4 * c4;
-        const bool xok = xx >= 0 && xx < d.nx;
-        int yy = y0 - p.hy + r0;
-        long long off = plane_off + (long long)yy * d.nx + xx;
-        float *da = s_a + r0 * WP + 4 * c4, *db = s_b + r0 * WP + 4 * c4;
-        for (int r = r0; r < H; r += RP) {
-            const bool ok = xok && yy >= 0 && yy < d.ny;
-            const long long o = ok ? off : 0;
-            st_cp_async16(da, Z1 + o, ok);
-            st_cp_async16(db, Z2 + o, ok);
-            yy += RP;
-            off += (long long)RP * d.nx;
-            da += RP * WP;
-            db += RP * WP;
+    float nxz[G];                                      // clipped window lengths along x times along z
+    unsigned core_x = 0;                               // bit j: column j is outside the x/z halo
+    {
+        const float nzc = (float)clipped_len(z, p.hz, d.nz);
+        const bool core_z = z >= p.gz && z < d.nz - p.gz;
+#pragma unroll
+        for (int j = 0; j < G; ++j) {
+            const int c = min(max(c0 + j, 0), d.nx - 1);
+            nxz[j] = (float)clipped_len(c, HX, d.nx) * nzc;
+            if (core_z && c0 + j >= p.gx && c0 + j < d.nx - p.gx) core_x |= 1u << j;
         }
     }
-    // stage the centre values (and, in OR mode, the previous mask) of the tile
-    {
-        const int c4 = tid & 31, r0 = tid >> 5;
-        const int xx = x0 + 4 * c4;
-        const bool xok = xx < d.nx;
+
+    float s1[G], s2[G], e2[G];
 #pragma unroll
-        for (int k = 0; k < ST_TY / 8; ++k) {
-            const int r = r0 + 8 * k, yy = y0 + r;
-            const bool ok = xok && yy < d.ny;
-            const long long o = ok ? plane_off + (long long)yy * d.nx + xx : 0;
-            st_cp_async16(s_f + r * ST_TX + 4 * c4, f + o, ok);
-            if (p.or_into) st_cp_async4(s_m + r * ST_TX + 4 * c4, mask + o, ok);
+    for (int j = 0; j < G; ++j) s1[j] = s2[j] = e2[j] = 0.f;
+    // rows ya-hy .. ya+hy-1 of the first window (clipped to the cube, C-7)
+    for (int r = max(ya - p.hy, 0); r < min(ya + p.hy, d.ny); ++r) {
+        float a1[G], a2[G];
+        ld_cols<G>(Z1 + col_off + (long long)r * d.nx, col_ok, a1);
+        ld_cols<G>(Z2 + col_off + (long long)r * d.nx, col_ok, a2);
+#pragma unroll
+        for (int j = 0; j < G; ++j) {
+            s1[j] += a1[j];
+            kahan_add(s2[j], e2[j], a2[j]);
         }
     }
-    st_cp_async_wait();
-    __syncthreads();
+    __syncthreads();   // zero padding of the exchange buffers is in place
 
-    // x direction: one row segment of 32 outputs per thread (8 consecutive rows per quarter warp)
-    {
-        const int warp = tid >> 5, lane = tid & 31;
-        const int xr = warp * 8 + (lane & 7), xs = lane >> 3;
-        const bool act = xr < H;
-        const int o = act ? xr * WP + xs * ST_L : 0;
-        xbox_inplace<HX>(s_a + o, act);
-        xbox_inplace<HX>(s_b + o, act);
-    }
-    __syncthreads();
-
-    // y direction + selection: column cx of the tile, rows ry0 .. ry0 + ST_ROWS - 1
-    {
-        const int cx = tid & (ST_TX - 1);
-        const int ry0 = (tid >> 7) * ST_ROWS;
-        const int gx = x0 + cx;
-        float S1[ST_ROWS], S2[ST_ROWS];
-        ybox(s_a + ry0 * WP + cx, WP, p.hy, S1);
-        ybox(s_b + ry0 * WP + cx, WP, p.hy, S2);
-        const float nxz = (float)clipped_len(min(gx, d.nx - 1), HX, d.nx) * (float)clipped_len(z, p.hz, d.nz);
-        const bool y_inside = y0 - p.hy >= 0 && y0 + ST_TY - 1 + p.hy < d.ny;   // no row of the tile is clipped
-        const float n_in = nxz * (float)(2 * p.hy + 1);
-        const bool halo = (p.gx | p.gy | p.gz) != 0;
-        const bool core_xz = gx >= p.gx && gx < d.nx - p.gx && z >= p.gz && z < d.nz - p.gz;
-        const float *vf = s_f + ry0 * ST_TX + cx;
-        uint8_t *vm = s_m + ry0 * ST_TX + cx;
+    unsigned my_count = 0;
+    YmRow<G> cur, nxt;
+    ym_load<G>(cur, f, Z1, Z2, mask, col_off, ya, p, col_ok);
+    const float guard = kFlatGuard;
+#pragma unroll 2
+    for (int y = ya; y < yb; ++y) {
+        if (y + 1 < yb) ym_load<G>(nxt, f, Z1, Z2, mask, col_off, y + 1, p, col_ok);
+        const int par = (y - ya) & 1;
+        // window sums along y of this thread's columns; prefix / suffix sums across its columns
+        float P1[G], Q1[G], P2[G], Q2[G];
 #pragma unroll
-        for (int i = 0; i < ST_ROWS; ++i) {
-            const int gy = y0 + ry0 + i;
-            const float n = y_inside ? n_in : nxz * (float)clipped_len(min(gy, d.ny - 1), p.hy, d.ny);
-            const float v = vf[i * ST_TX], s1 = S1[i], s2 = S2[i];
-            const float a = fmaf(n, v, -s1);
-            const float q = fmaxf(fmaf(n, s2, -s1 * s1), 0.f);
-            int sel = (a > kFlatGuard * n * fabsf(v)) && (a * a > p.k2 * q);
-            if (halo && !(core_xz && gy >= p.gy && gy < d.ny - p.gy)) sel = 0;
-            else if (p.or_into) sel |= (vm[i * ST_TX] != 0);
-            vm[i * ST_TX] = (uint8_t)sel;
-            if ((mean != nullptr || sd != nullptr) && gx < d.nx && gy < d.ny) {
-                const long long idx = plane_off + (long long)gy * d.nx + gx;
-                const float m = s1 / n;
-                if (mean != nullptr) mean[idx] = m;
-                if (sd != nullptr) sd[idx] = sqrtf(fmaxf(s2 / n - m * m, 0.f));
+        for (int j = 0; j < G; ++j) {
+            s1[j] += cur.l1[j];
+            kahan_add(s2[j], e2[j], cur.l2[j]);
+            P1[j] = Q1[j] = s1[j];
+            P2[j] = Q2[j] = s2[j] - e2[j];
+        }
+#pragma unroll
+        for (int j = 1; j < G; ++j) { P1[j] += P1[j - 1]; P2[j] += P2[j - 1]; }
+#pragma unroll
+        for (int j = G - 2; j >= 0; --j) { Q1[j] += Q1[j + 1]; Q2[j] += Q2[j + 1]; }
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            if constexpr (G == 2) {
+                buf(par, 0, 0, v)[tid + 2] = make_float2(P1[0], P1[1]);
+                buf(par, 0, 1, v)[tid + 2] = make_float2(Q1[0], Q1[1]);
+                buf(par, 1, 0, v)[tid + 2] = make_float2(P2[0], P2[1]);
+                buf(par, 1, 1, v)[tid + 2] = make_float2(Q2[0], Q2[1]);
+            } else {
+                buf(par, 0, 0, v)[tid + 2] = make_float4(P1[4 * v], P1[4 * v + 1], P1[4 * v + 2], P1[4 * v + 3]);
+                buf(par, 0, 1, v)[tid + 2] = make_float4(Q1[4 * v], Q1[4 * v + 1], Q1[4 * v + 2], Q1[4 * v + 3]);
+                buf(par, 1, 0, v)[tid + 2] = make_float4(P2[4 * v], P2[4 * v + 1], P2[4 * v + 2], P2[4 * v + 3]);
+                buf(par, 1, 1, v)[tid + 2] = make_float4(Q2[4 * v], Q2[4 * v + 1], Q2[4 * v + 2], Q2[4 * v + 3]);
             }
         }
-    }
-    __syncthreads();
-
-    // mask tile -> global, 4 bytes per thread and row pass (one 128-byte row per warp); count = popcount
-    unsigned my_count = 0;
-    {
-        const int c4 = tid & 31, r0 = tid >> 5;
-        const int xx = x0 + 4 * c4;
-        if (xx < d.nx) {
+        // the row leaving the window (after this output)
 #pragma unroll
-            for (int k = 0; k < ST_TY / 8; ++k) {
-                const int r = r0 + 8 * k, yy = y0 + r;
-                if (yy < d.ny) {
-                    const unsigned w = *reinterpret_cast<const unsigned *>(s_m + r * ST_TX + 4 * c4);
-                    *reinterpret_cast<unsigned *>(mask + plane_off + (long long)yy * d.nx + xx) = w;
-                    my_count += __popc(w);
+        for (int j = 0; j < G; ++j) {
+            s1[j] -= cur.t1[j];
+            kahan_add(s2[j], e2[j], -cur.t2[j]);
+        }
+        __syncthreads();
+        // x-direction window: suffix(t-2) + total(t-1) + total(t) + total(t+1) + prefix(t+2)
+        float S1[G], S2[G];
+        {
+            const float m1 = reinterpret_cast<const float *>(buf(par, 0, 1, 0) + tid + 1)[0] + P1[G - 1] +
+                             reinterpret_cast<const float *>(buf(par, 0, 1, 0) + tid + 3)[0];
+            const float m2 = reinterpret_cast<const float *>(buf(par, 1, 1, 0) + tid + 1)[0] + P2[G - 1] +
+                             reinterpret_cast<const float *>(buf(par, 1, 1, 0) + tid + 3)[0];
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                const V a1 = buf(par, 0, 1, v)[tid], b1 = buf(par, 0, 0, v)[tid + 4];
+                const V a2 = buf(par, 1, 1, v)[tid], b2 = buf(par, 1, 0, v)[tid + 4];
+                const float *pa1 = reinterpret_cast<const float *>(&a1), *pb1 = reinterpret_cast<const float *>(&b1);
+                const float *pa2 = reinterpret_cast<const float *>(&a2), *pb2 = reinterpret_cast<const float *>(&b2);
+#pragma unroll
+                for (int e = 0; e < VL; ++e) {
+                    S1[VL * v + e] = m1 + (pa1[e] + pb1[e]);
+                    S2[VL * v + e] = m2 + (pa2[e] + pb2[e]);
                 }
             }
         }
+        // selection (division-free form, see pgsf_generic.cu), halo, OR, mask bytes
+        const float nyc = (float)clipped_len(y, p.hy, d.ny);
+        const bool core_y = y >= p.gy && y < d.ny - p.gy;
+        unsigned bits = 0;
+#pragma unroll
+        for (int j = 0; j < G; ++j) {
+            const float n = nxz[j] * nyc;
+            const float v = cur.fc[j];
+            const float a = fmaf(n, v, -S1[j]);
+            const float q = fmaxf(fmaf(n, S2[j], -S1[j] * S1[j]), 0.f);
+            const bool sel = (a > guard * n * fabsf(v)) && (a * a > p.k2 * q);
+            if (sel) bits |= 1u << j;
+        }
+        if (p.or_into) {   // previous mask: any non-zero byte counts as set
+            if constexpr (G == 2) {
+                bits |= ((cur.mk[0] & 0xffu) ? 1u : 0u) | ((cur.mk[0] & 0xff00u) ? 2u : 0u);
+            } else {
+#pragma unroll
+                for (int q4 = 0; q4 < G / 4; ++q4) {
+                    const unsigned old = cur.mk[q4];
+                    const unsigned nz = ((old | ((old & 0x7f7f7f7fu) + 0x7f7f7f7fu)) >> 7) & 0x01010101u;
+                    bits |= ((nz & 1u) | ((nz >> 7) & 2u) | ((nz >> 14) & 4u) | ((nz >> 21) & 8u)) << (4 * q4);
+                }
+            }
+        }
+        bits = core_y ? (bits & core_x) : 0u;
+        if (is_out) {
+            const long long idx = col_off + (long long)y * d.nx;
+            my_count += __popc(bits);
+            if constexpr (G == 2) {
+                *reinterpret_cast<unsigned short *>(mask + idx) = (unsigned short)((bits & 1u) | ((bits & 2u) << 7));
+            } else {
+#pragma unroll
+                for (int q4 = 0; q4 < G / 4; ++q4) {
+                    const unsigned b4 = (bits >> (4 * q4)) & 15u;
+                    *reinterpret_cast<unsigned *>(mask + idx + 4 * q4) =
+                        (b4 & 1u) | ((b4 & 2u) << 7) | ((b4 & 4u) << 14) | ((b4 & 8u) << 21);
+                }
+            }
+            if (mean != nullptr || sd != nullptr) {
+#pragma unroll
+                for (int j = 0; j < G; ++j) {
+                    const float n = nxz[j] * nyc;
+                    const float m = S1[j] / n;
+                    if (mean != nullptr) mean[idx + j] = m;
+                    if (sd != nullptr) sd[idx + j] = sqrtf(fmaxf(S2[j] / n - m * m, 0.f));
+                }
+            }
+        }
+        cur = nxt;
     }
 
     if (count != nullptr) {
-        __shared__ unsigned wsum[ST_NT / 32];
+        __shared__ unsigned wsum[YM_MAX_NT / 32];
         unsigned c = my_count;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
@@ -328,26 +359,46 @@ __global__ void __launch_bounds__(ST_NT, 2) k_xybox(const float *__restrict__ f,
         __syncthreads();
         if (tid == 0) {
             unsigned t = 0;
-            for (int w = 0; w < ST_NT / 32; ++w) t += wsum[w];
+            for (int w = 0; w < NT / 32; ++w) t += wsum[w];
             if (t) atomicAdd(count, (unsigned long long)t);
         }
     }
 }
 
-template <int HX>
-cudaError_t launch_xybox(const float *f, const float *Z1, const float *Z2, uint8_t *mask, float *mean,
-                         float *sd, unsigned long long *count, const XyboxParams &p, cudaStream_t st)
+template <int G>
+cudaError_t launch_ymarch(const pgsf_plan *pl, const float *f, const float *Z1, const float *Z2, uint8_t *mask,
+                          float *mean, float *sd, unsigned long long *count, YmParams p, cudaStream_t st)
 {
-    const int H = ST_TY + 2 * p.hy;
-    const int smem = 2 * H * (ST_TX + 2 * HX + 4) * (int)sizeof(float) + ST_TY * ST_TX * 5;
+    constexpr int VL = VecT<G>::L;
+    const Dims &d = p.d;
+    // threads: cover the whole row when it fits in one CTA, else tiles overlapping by 2 hx columns
+    int nt = ((d.nx + G - 1) / G + 31) / 32 * 32;
+    if (nt <= YM_MAX_NT) {
+        p.ntiles = 1;
+        p.wo = d.nx;
+    } else {
+        nt = YM_MAX_NT;
+        p.wo = nt * G - 4 * G;
+        p.ntiles = (d.nx + p.wo - 1) / p.wo;
+    }
+    // y chunks: enough CTAs for a few waves; a chunk start re-reads 2 hy rows
+    const long long resident = (long long)pl->sm_count * (nt <= 128 ? 4 : 2);
+    const long long base = (long long)p.ntiles * d.nz;
+    int nch = (int)((4 * resident + base - 1) / base);
+    const int min_rows = 8 * p.hy > 64 ? 8 * p.hy : 64;
+    if (nch > (d.ny + min_rows - 1) / min_rows) nch = (d.ny + min_rows - 1) / min_rows;
+    if (nch < 1) nch = 1;
+    p.ychunk = (d.ny + nch - 1) / nch;
+    nch = (d.ny + p.ychunk - 1) / p.ychunk;
+    const int smem = 8 * (G / VL) * (nt + 4) * VL * (int)sizeof(float);
     static int configured = 0;
-    if (configured < smem) {
-        cudaError_t e = cudaFuncSetAttribute(k_xybox<HX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (smem > 48 * 1024 && configured < smem) {
+        cudaError_t e = cudaFuncSetAttribute(k_ymarch<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    dim3 grid((p.d.nx + ST_TX - 1) / ST_TX, (p.d.ny + ST_TY - 1) / ST_TY, p.d.nz);
-    k_xybox<HX><<<grid, ST_NT, smem, st>>>(f, Z1, Z2, mask, mean, sd, count, p);
+    dim3 grid(p.ntiles, nch, d.nz);
+    k_ymarch<G><<<grid, nt, smem, st>>>(f, Z1, Z2, mask, mean, sd, count, p);
     return cudaGetLastError();
 }
 
@@ -355,10 +406,11 @@ cudaError_t launch_xybox(const float *f, const float *Z1, const float *Z2, uint8
 
 bool fast_stats_supported(const pgsf_plan *p)
 {
-    const int hx = p->desc.box_half[0], hy = p->desc.box_half[1];
+    const int hx = p->desc.box_half[0];
     if (p->desc.nx % 4 != 0) return false;
-    if (hx % 4 != 0 || hx > 16 || hy > ST_MAX_HY) return false;
-    return (p->desc.ny + ST_TY - 1) / ST_TY <= 65535 && p->desc.nz <= 65535;
+    if (hx != 4 && hx != 8 && hx != 16) return false;
+    if (p->desc.nx % (hx / 2) != 0) return false;   // a thread owns hx/2 whole columns
+    return p->desc.nz <= 65535;
 }
 
 cudaError_t fast_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean, float *sd,
@@ -388,22 +440,21 @@ cudaError_t fast_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_i
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
-    XyboxParams xp;
-    xp.d = d;
-    xp.hy = p->desc.box_half[1];
-    xp.hz = p->desc.box_half[2];
-    xp.gx = p->desc.halo[0];
-    xp.gy = p->desc.halo[1];
-    xp.gz = p->desc.halo[2];
-    xp.or_into = or_into;
-    xp.k2 = (float)(p->desc.k * p->desc.k);
+    YmParams yp;
+    yp.d = d;
+    yp.hy = p->desc.box_half[1];
+    yp.hz = p->desc.box_half[2];
+    yp.gx = p->desc.halo[0];
+    yp.gy = p->desc.halo[1];
+    yp.gz = p->desc.halo[2];
+    yp.or_into = or_into;
+    yp.k2 = (float)(p->desc.k * p->desc.k);
+    yp.wo = yp.ntiles = yp.ychunk = 0;
     LaunchScope ls(p, "stats_xybox", st);
     switch (p->desc.box_half[0]) {
-    case 0: return launch_xybox<0>(f, Z1, Z2, mask, mean, sd, count, xp, st);
-    case 4: return launch_xybox<4>(f, Z1, Z2, mask, mean, sd, count, xp, st);
-    case 8: return launch_xybox<8>(f, Z1, Z2, mask, mean, sd, count, xp, st);
-    case 12: return launch_xybox<12>(f, Z1, Z2, mask, mean, sd, count, xp, st);
-    case 16: return launch_xybox<16>(f, Z1, Z2, mask, mean, sd, count, xp, st);
+    case 4: return launch_ymarch<2>(p, f, Z1, Z2, mask, mean, sd, count, yp, st);
+    case 8: return launch_ymarch<4>(p, f, Z1, Z2, mask, mean, sd, count, yp, st);
+    case 16: return launch_ymarch<8>(p, f, Z1, Z2, mask, mean, sd, count, yp, st);
     default: return cudaErrorNotSupported;
     }
 }
