@@ -195,8 +195,9 @@ def _kernel_work(name: str, w, taps, n_vox: int):
     the separable method must do, not what the implementation happens to move."""
     S = len(taps)
     kind, _, tail = name.partition("_")
-    if kind == "xy" and tail == "all":       # x and y passes of every scale from one read of the input
-        return 2 * sum(t[0] + t[1] for t in taps) * n_vox, (4 + 4 * S) * n_vox
+    if kind == "xy" and tail.startswith("m"):  # x and y passes of the scales in the bit mask, one read of the input
+        grp = [t for i, t in enumerate(taps) if (int(tail[1:]) >> i) & 1]
+        return 2 * sum(t[0] + t[1] for t in grp) * n_vox, (4 + 4 * len(grp)) * n_vox
     if kind == "xy" and tail.startswith("s"):
         t = taps[int(tail[1:])]
         return 2 * (t[0] + t[1]) * n_vox, 8 * n_vox

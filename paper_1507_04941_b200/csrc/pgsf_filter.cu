@@ -50,161 +50,201 @@ __host__ __device__ constexpr int round4(int v) { return (v + 3) & ~3; }
 
 // ------------------------------------------------------------------------------------ x/y passes
 //
-// k_xy_multi<RMAX>: one z plane tile of 128 x 32 voxels.  The input tile + RMAX halo is staged ONCE
-// (zero fill outside the cube, C-5) and the x and y passes of EVERY scale of the bank are evaluated
-// from it ("several sigma scales evaluated per input read", BASELINE.json north_star): the input cube
-// is read once for all scales instead of once per scale.
-//   y pass (Eq. 4): thread = 4 staged columns x 4 rows; walks down the staged rows (LDS.128), packed
-//                   FFMA2 over x pairs; result stored with the rows of a row PAIR interleaved,
-//                   t1[(row/2)][col][row%2], so that
-//   x pass (Eq. 3): thread = 2 rows x 8 columns; one LDS.128 yields two columns of both rows as two
-//                   (row, row+1) register pairs, i.e. the x pass is packed FFMA2 over row pairs.
+// k_xym<NS, RA..RD>: one CTA = one z plane, a strip of 256 columns, one chunk of rows; it marches
+// down y in batches of 8 row PAIRS and evaluates the x and y passes of up to four scales from ONE
+// read of the input ("several sigma scales evaluated per input read", BASELINE.json north_star).
+//   x pass (Eq. 3): warp w stages row pair w of the batch (+16 columns either side, zero fill outside
+//                   the cube = C-5) with the two rows interleaved, so one LDS.128 yields two columns
+//                   of both rows; a lane owns 8 columns x 2 rows and gathers its taps as packed
+//                   FFMA2 over the row pair.  Results u go to shared memory, one slab per scale.
+//   y pass (Eq. 4): a thread owns ONE column and keeps the R + 1 unfinished output row pairs of
+//                   every scale in registers.  Each new pair (u[2k], u[2k+1]) is scattered into
+//                   them with FFMA2 (even taps use the pair as loaded, odd taps the pair shifted by
+//                   one row), the accumulators rotate through the destination register of the
+//                   FFMA2 (no moves), and the pair that has seen all its taps is stored.
+// Both passes are pure FFMA2 streams with uniform-register taps; no y halo is recomputed and the
+// only shared-memory traffic is the x pass' operand reads.
 
-constexpr int XM_TX = 128;
-constexpr int XM_TY = 32;
-constexpr int XM_NT = 256;
-constexpr int XM_PY = 4;        // rows per thread in the y pass
-constexpr int XM_QX = 8;        // columns per thread in the x pass (times two rows)
+constexpr int XM_NT = 256;          // threads = columns per CTA
+constexpr int XM_NB = 8;            // row pairs per batch (= warps)
+constexpr int XM_HALO = 16;         // staged columns either side (>= largest x radius, multiple of 4)
+constexpr int XM_SW = XM_NT + 2 * XM_HALO;
+constexpr int XM_GP = 10;           // pitch in pairs of an 8-column group (spreads the banks)
+constexpr int XM_SIN = (XM_SW / 8) * XM_GP;   // pairs of one staged row pair
+constexpr int XM_U = (XM_NT / 8) * XM_GP;     // pairs of one x-filtered row pair
+constexpr int XM_MAXS = 4;
 
-struct XYMultiParams {
+struct XymParams {
     Dims d;
-    int n;                          // scales in this launch
-    int rc[PGSF_MAX_SCALES];        // compiled radius of each
-    float *out[PGSF_MAX_SCALES];    // x/y-filtered plane stack of each
-    TapsXY t[PGSF_MAX_SCALES];
+    int ychunk;                       // output rows per CTA (multiple of 16)
+    float *out[XM_MAXS];              // x/y-filtered cube of each scale
+    TapsXY t[XM_MAXS];
 };
 
-template <int RMAX>
-struct XMShape {
-    static constexpr int R4M = round4(RMAX);
-    static constexpr int W = XM_TX + 2 * R4M;                    // staged columns
-    static constexpr int HI = XM_TY + 2 * RMAX;                  // staged rows
-    static constexpr int WT = W + ((2 - W % 16) + 16) % 16;      // t1 pitch in columns, = 2 (mod 16):
-                                                                 // row pairs 4 banks apart
-    static constexpr int SMEM = (HI * W + XM_TY * WT) * 4;
-};
-
-template <int R, int RMAX>
-__device__ __forceinline__ void xy_one_scale(const float *s_in, float *s_t1, float *__restrict__ out_plane,
-                                             const TapsXY &t, const Dims &d, int x0, int y0, int tid)
+__device__ __forceinline__ float2 fmul2(float2 a, float g)
 {
-    using S = XMShape<RMAX>;
-    constexpr int R4 = round4(R);
-    constexpr int C0 = S::R4M - R4;                 // first staged column this scale needs
-    constexpr int W4s = (XM_TX + 2 * R4) / 4;
-    constexpr int YB = XM_TY / XM_PY;
-    // ---- y pass
-    for (int task = tid; task < W4s * YB; task += XM_NT) {
-        const int yb = task / W4s, c4 = task - yb * W4s;
-        float2 acc[XM_PY][2];
-#pragma unroll
-        for (int p = 0; p < XM_PY; ++p) acc[p][0] = acc[p][1] = make_float2(0.f, 0.f);
-        const float *col = s_in + (yb * XM_PY + (RMAX - R)) * S::W + C0 + 4 * c4;
-#pragma unroll
-        for (int j = 0; j < XM_PY + 2 * R; ++j) {
-            const float4 v = *reinterpret_cast<const float4 *>(col + j * S::W);
-#pragma unroll
-            for (int p = 0; p < XM_PY; ++p) {
-                const int o = j - p;
-                if (o >= 0 && o <= 2 * R) {
-                    acc[p][0] = ffma2(make_float2(v.x, v.y), t.gy[o], acc[p][0]);
-                    acc[p][1] = ffma2(make_float2(v.z, v.w), t.gy[o], acc[p][1]);
-                }
-            }
-        }
-#pragma unroll
-        for (int jj = 0; jj < XM_PY / 2; ++jj) {
-            float *dst = s_t1 + ((yb * (XM_PY / 2) + jj) * S::WT + C0 + 4 * c4) * 2;
-            const float2 a0 = acc[2 * jj][0], a1 = acc[2 * jj][1], b0 = acc[2 * jj + 1][0], b1 = acc[2 * jj + 1][1];
-            *reinterpret_cast<float4 *>(dst) = make_float4(a0.x, b0.x, a0.y, b0.y);
-            *reinterpret_cast<float4 *>(dst + 4) = make_float4(a1.x, b1.x, a1.y, b1.y);
-        }
-    }
-    __syncthreads();
-    // ---- x pass
-    {
-        const int jp = tid & (XM_TY / 2 - 1), xb = tid / (XM_TY / 2);
-        constexpr int CS = S::R4M - R;              // staged column of tap o = 0 of output column 0
-        constexpr int SH = CS & 1;                  // float4 loads start at an even column
-        constexpr int NL = (XM_QX + 2 * R + SH + 1) / 2;
-        float2 v[2 * NL];
-        const float *src = s_t1 + (jp * S::WT + (CS - SH) + XM_QX * xb) * 2;
-#pragma unroll
-        for (int k = 0; k < NL; ++k) {
-            const float4 q = *reinterpret_cast<const float4 *>(src + 4 * k);
-            v[2 * k] = make_float2(q.x, q.y);
-            v[2 * k + 1] = make_float2(q.z, q.w);
-        }
-        float2 acc[XM_QX];
-#pragma unroll
-        for (int i = 0; i < XM_QX; ++i) acc[i] = make_float2(0.f, 0.f);
-#pragma unroll
-        for (int o = 0; o <= 2 * R; ++o)
-#pragma unroll
-            for (int i = 0; i < XM_QX; ++i) acc[i] = ffma2(v[i + o + SH], t.gx[o], acc[i]);
-        const int gy = y0 + 2 * jp, gx = x0 + XM_QX * xb;
-        if (gx < d.nx) {
-            float *dst = out_plane + (long long)gy * d.nx + gx;
-            const bool second = gx + 4 < d.nx;
-            if (gy < d.ny) {
-                *reinterpret_cast<float4 *>(dst) = make_float4(acc[0].x, acc[1].x, acc[2].x, acc[3].x);
-                if (second) *reinterpret_cast<float4 *>(dst + 4) = make_float4(acc[4].x, acc[5].x, acc[6].x, acc[7].x);
-            }
-            if (gy + 1 < d.ny) {
-                *reinterpret_cast<float4 *>(dst + d.nx) = make_float4(acc[0].y, acc[1].y, acc[2].y, acc[3].y);
-                if (second)
-                    *reinterpret_cast<float4 *>(dst + d.nx + 4) = make_float4(acc[4].y, acc[5].y, acc[6].y, acc[7].y);
-            }
-        }
-    }
+    const float2 gg = make_float2(g, g);
+    unsigned long long ra = *reinterpret_cast<const unsigned long long *>(&a);
+    unsigned long long rb = *reinterpret_cast<const unsigned long long *>(&gg);
+    unsigned long long rd;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(rd) : "l"(ra), "l"(rb));
+    return *reinterpret_cast<float2 *>(&rd);
 }
 
-template <int RMAX>
-__global__ void __launch_bounds__(XM_NT) k_xy_multi(const float *__restrict__ in,
-                                                     const __grid_constant__ XYMultiParams P)
+// x pass of one scale for the warp's staged row pair: lane -> columns 8 lane .. 8 lane + 7
+template <int R>
+__device__ __forceinline__ void xm_xpass(const float2 *__restrict__ s_in, float2 *__restrict__ s_u,
+                                         const float (&gx)[32], int lane)
 {
-    using S = XMShape<RMAX>;
-    extern __shared__ __align__(16) float smem[];
-    float *s_in = smem;                  // [HI][W]
-    float *s_t1 = smem + S::HI * S::W;   // [TY/2][WT][2]
-    const Dims &d = P.d;
-    const int tid = threadIdx.x;
-    const int x0 = blockIdx.x * XM_TX, y0 = blockIdx.y * XM_TY, z = blockIdx.z;
-    const long long plane_off = (long long)z * d.plane;
-
-    // stage the input tile + halo: thread <-> one 16-byte column chunk, rows r0, r0 + RP, ...
-    {
-        constexpr int W4 = S::W / 4, RP = XM_NT / W4;
-        if (tid < RP * W4) {
-            const int c4 = tid % W4, r0 = tid / W4;
-            const int xx = x0 - S::R4M + 4 * c4;
-            const bool xok = xx >= 0 && xx < d.nx;
-            int yy = y0 - RMAX + r0;
-            long long off = plane_off + (long long)yy * d.nx + xx;
-            float *dst = s_in + r0 * S::W + 4 * c4;
-            for (int r = r0; r < S::HI; r += RP) {
-                const bool ok = xok && yy >= 0 && yy < d.ny;
-                cp_async16(dst, in + (ok ? off : 0), ok);
-                yy += RP;
-                off += (long long)RP * d.nx;
-                dst += RP * S::W;
+    constexpr int C0 = XM_HALO - R;     // staged column of tap -R of output column 0
+    constexpr int SH = C0 & 1;          // 16-byte loads start at an even staged column
+    constexpr int NL = (8 + 2 * R + SH + 1) / 2;
+    float2 acc[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc[i] = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int l = 0; l < NL; ++l) {
+        const int sc = C0 - SH + 2 * l;                 // relative to 8 lane; compile time
+        const float4 q = *reinterpret_cast<const float4 *>(s_in + (lane + (sc >> 3)) * XM_GP + (sc & 7));
+        const float2 v[2] = {make_float2(q.x, q.y), make_float2(q.z, q.w)};
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int j = 2 * l + e - SH;               // input index relative to tap -R of output 0
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const int o = j - i;
+                if (j >= 0 && o >= 0 && o <= 2 * R) acc[i] = ffma2(v[e], gx[o], acc[i]);
             }
         }
-        cp_async_wait_all();
-        __syncthreads();
     }
+    float4 *dst = reinterpret_cast<float4 *>(s_u + lane * XM_GP);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) dst[i] = make_float4(acc[2 * i].x, acc[2 * i].y, acc[2 * i + 1].x, acc[2 * i + 1].y);
+}
 
-    for (int s = 0; s < P.n; ++s) {
-        if (s > 0) __syncthreads();      // the previous scale's x pass has read s_t1
-        float *out_plane = P.out[s] + plane_off;
-        const TapsXY &t = P.t[s];
-        switch (P.rc[s]) {
-        case 3: xy_one_scale<3, RMAX>(s_in, s_t1, out_plane, t, d, x0, y0, tid); break;
-        case 6: if constexpr (RMAX >= 6) xy_one_scale<6, RMAX>(s_in, s_t1, out_plane, t, d, x0, y0, tid); break;
-        case 9: if constexpr (RMAX >= 9) xy_one_scale<9, RMAX>(s_in, s_t1, out_plane, t, d, x0, y0, tid); break;
-        case 12: if constexpr (RMAX >= 12) xy_one_scale<12, RMAX>(s_in, s_t1, out_plane, t, d, x0, y0, tid); break;
-        default: break;
+// y pass state of one scale and one column: B[j] = unfinished output pair m = k + dmin + j
+template <int R>
+struct XmY {
+    float2 B[R];
+    float prev;     // u[2k - 1]
+    __device__ __forceinline__ void init()
+    {
+#pragma unroll
+        for (int j = 0; j < R; ++j) B[j] = make_float2(0.f, 0.f);
+        prev = 0.f;
+    }
+    // scatter the pair U = (u[2k], u[2k+1]); returns the finished pair of rows 2m, 2m+1, m = k - ceil(R/2)
+    __device__ __forceinline__ float2 step(float2 U, const float (&gy)[32])
+    {
+        constexpr int dmin = -((R + 1) / 2), dmax = R / 2;
+        const float2 Uo = make_float2(prev, U.x);
+        prev = U.y;
+        float2 out = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int d = dmin; d <= dmax; ++d) {
+            const int oe = -2 * d, oo = -2 * d - 1;     // taps fed by U and by Uo
+            const bool he = oe >= -R && oe <= R, ho = oo >= -R && oo <= R;
+            float2 t;
+            if (d < dmax) {
+                t = B[d - dmin];
+                if (he) t = ffma2(U, gy[oe + R], t);
+                if (ho) t = ffma2(Uo, gy[oo + R], t);
+            } else {                                    // newest pair: first contribution(s)
+                if (he) { t = fmul2(U, gy[oe + R]); if (ho) t = ffma2(Uo, gy[oo + R], t); }
+                else t = fmul2(Uo, gy[oo + R]);
+            }
+            if (d == dmin) out = t;
+            else B[d - 1 - dmin] = t;
         }
+        return out;
+    }
+};
+
+template <int NS, int RA, int RB, int RC, int RD>
+__global__ void __launch_bounds__(XM_NT, 2) k_xym(const float *__restrict__ in, const __grid_constant__ XymParams P)
+{
+    extern __shared__ __align__(16) float2 xm_smem[];
+    float2 *s_in = xm_smem;                        // [8 warps][XM_SIN]
+    float2 *s_u = xm_smem + XM_NB * XM_SIN;        // [8 row pairs][NS][XM_U]
+    const Dims &d = P.d;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int x0 = blockIdx.x * XM_NT, z = blockIdx.z;
+    const int ya = blockIdx.y * P.ychunk, yb = min(ya + P.ychunk, d.ny);
+    const int ys = ya - 16;                        // first input row of the first batch (even)
+    const int nbatch = (yb + 12 - ys + 15) / 16;
+    const long long plane_off = (long long)z * d.plane;
+    const int gx = x0 + tid;
+    const bool col_ok = gx < d.nx;
+    float *o0 = P.out[0] + plane_off + gx;
+    float *o1 = NS > 1 ? P.out[NS > 1 ? 1 : 0] + plane_off + gx : nullptr;
+    float *o2 = NS > 2 ? P.out[NS > 2 ? 2 : 0] + plane_off + gx : nullptr;
+    float *o3 = NS > 3 ? P.out[NS > 3 ? 3 : 0] + plane_off + gx : nullptr;
+
+    XmY<RA> sa; XmY<RB> sb; XmY<RC> sc; XmY<RD> sd;
+    sa.init(); sb.init(); sc.init(); sd.init();
+
+    // this warp's row pair of batch b: rows ys + 16 b + 2 w (+1); lane loads float4 columns lane, lane+32, lane+64
+    float4 pf[2][3];
+    auto prefetch = [&](int b) {
+        const int r0 = ys + 16 * b + 2 * w;
+#pragma unroll
+        for (int rr = 0; rr < 2; ++rr) {
+            const int r = r0 + rr;
+            const bool rok = r >= 0 && r < d.ny;
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                const int idx = lane + 32 * q;
+                const int xx = x0 - XM_HALO + 4 * idx;
+                const bool ok = rok && idx < XM_SW / 4 && xx >= 0 && xx < d.nx;
+                pf[rr][q] = ok ? __ldg(reinterpret_cast<const float4 *>(in + plane_off + (long long)r * d.nx + xx))
+                               : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+        }
+    };
+    prefetch(0);
+    for (int b = 0; b < nbatch; ++b) {
+        // ---- x phase: stage the row pair interleaved, then the x pass of every scale
+        {
+            float2 *sw = s_in + w * XM_SIN;
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                const int idx = lane + 32 * q;
+                if (idx < XM_SW / 4) {
+                    float4 *dst = reinterpret_cast<float4 *>(sw + (idx >> 1) * XM_GP + (idx & 1) * 4);
+                    const float4 a = pf[0][q], c = pf[1][q];
+                    dst[0] = make_float4(a.x, c.x, a.y, c.y);
+                    dst[1] = make_float4(a.z, c.z, a.w, c.w);
+                }
+            }
+            __syncwarp();
+            float2 *su = s_u + (w * NS) * XM_U;
+            xm_xpass<RA>(sw, su, P.t[0].gx, lane);
+            if constexpr (NS > 1) xm_xpass<RB>(sw, su + XM_U, P.t[NS > 1 ? 1 : 0].gx, lane);
+            if constexpr (NS > 2) xm_xpass<RC>(sw, su + 2 * XM_U, P.t[NS > 2 ? 2 : 0].gx, lane);
+            if constexpr (NS > 3) xm_xpass<RD>(sw, su + 3 * XM_U, P.t[NS > 3 ? 3 : 0].gx, lane);
+        }
+        if (b + 1 < nbatch) prefetch(b + 1);
+        __syncthreads();
+        // ---- y phase: 8 steps of the march
+        const int kbase = ys / 2 + XM_NB * b;      // ys is even
+        const int pi = (tid >> 3) * XM_GP + (tid & 7);
+#pragma unroll 2
+        for (int kk = 0; kk < XM_NB; ++kk) {
+            const float2 *su = s_u + (kk * NS) * XM_U + pi;
+            const int k = kbase + kk;
+            auto emit = [&](float *o, float2 v, int m) {
+                const int r0 = 2 * m;
+                if (col_ok) {
+                    if (r0 >= ya && r0 < yb) o[(long long)r0 * d.nx] = v.x;
+                    if (r0 + 1 >= ya && r0 + 1 < yb) o[(long long)(r0 + 1) * d.nx] = v.y;
+                }
+            };
+            emit(o0, sa.step(su[0], P.t[0].gy), k - (RA + 1) / 2);
+            if constexpr (NS > 1) emit(o1, sb.step(su[XM_U], P.t[NS > 1 ? 1 : 0].gy), k - (RB + 1) / 2);
+            if constexpr (NS > 2) emit(o2, sc.step(su[2 * XM_U], P.t[NS > 2 ? 2 : 0].gy), k - (RC + 1) / 2);
+            if constexpr (NS > 3) emit(o3, sd.step(su[3 * XM_U], P.t[NS > 3 ? 3 : 0].gy), k - (RD + 1) / 2);
+        }
+        __syncthreads();
     }
 }
 
@@ -292,18 +332,19 @@ __global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, f
     }
 }
 
-template <int RMAX>
-cudaError_t launch_xy_multi(const float *in, const XYMultiParams &P, cudaStream_t st)
+template <int NS, int RA, int RB, int RC, int RD>
+cudaError_t launch_xym(const float *in, const XymParams &P, int sm_count, cudaStream_t st)
 {
+    constexpr int SMEM = (XM_NB * XM_SIN + XM_NB * NS * XM_U) * (int)sizeof(float2);
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_xy_multi<RMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             XMShape<RMAX>::SMEM);
+        cudaError_t e = cudaFuncSetAttribute(k_xym<NS, RA, RB, RC, RD>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    dim3 grid((P.d.nx + XM_TX - 1) / XM_TX, (P.d.ny + XM_TY - 1) / XM_TY, P.d.nz);
-    k_xy_multi<RMAX><<<grid, XM_NT, XMShape<RMAX>::SMEM, st>>>(in, P);
+    (void)sm_count;
+    dim3 grid((P.d.nx + XM_NT - 1) / XM_NT, (P.d.ny + P.ychunk - 1) / P.ychunk, P.d.nz);
+    k_xym<NS, RA, RB, RC, RD><<<grid, XM_NT, SMEM, st>>>(in, P);
     return cudaGetLastError();
 }
 
@@ -342,35 +383,92 @@ bool fast_z_radius(int r, int *c)
     return false;
 }
 
-// x and y passes of the scales `scales[0..n)` of one cube: in -> out[i] (x/y-filtered cubes)
+// One launch of k_xym for the (already radius-sorted) scales g[0..n): true if that radius tuple is compiled.
+static bool xym_dispatch(int n, const int *rc, const float *in, const XymParams &P, int sm_count, cudaStream_t st,
+                         bool probe, cudaError_t *err)
+{
+#define XYM_CASE(NS, A, B, C, D)                                                              \
+    if (n == NS && rc[0] == A && (NS < 2 || rc[1] == B) && (NS < 3 || rc[2] == C) && (NS < 4 || rc[3] == D)) { \
+        if (!probe) *err = launch_xym<NS, A, (NS > 1 ? B : 3), (NS > 2 ? C : 3), (NS > 3 ? D : 3)>(in, P, sm_count, st); \
+        return true;                                                                          \
+    }
+    XYM_CASE(4, 3, 6, 9, 12)
+    XYM_CASE(3, 3, 6, 9, 0)
+    XYM_CASE(3, 3, 6, 6, 0)
+    XYM_CASE(3, 6, 9, 9, 0)
+    XYM_CASE(2, 3, 3, 0, 0)
+    XYM_CASE(2, 3, 6, 0, 0)
+    XYM_CASE(2, 3, 9, 0, 0)
+    XYM_CASE(2, 3, 12, 0, 0)
+    XYM_CASE(2, 6, 6, 0, 0)
+    XYM_CASE(2, 6, 9, 0, 0)
+    XYM_CASE(2, 6, 12, 0, 0)
+    XYM_CASE(2, 9, 9, 0, 0)
+    XYM_CASE(2, 9, 12, 0, 0)
+    XYM_CASE(2, 12, 12, 0, 0)
+    XYM_CASE(1, 3, 0, 0, 0)
+    XYM_CASE(1, 6, 0, 0, 0)
+    XYM_CASE(1, 9, 0, 0, 0)
+    XYM_CASE(1, 12, 0, 0, 0)
+#undef XYM_CASE
+    return false;
+}
+
+// x and y passes of the scales `scales[0..n)` of one cube: in -> out[i] (x/y-filtered cubes).  The
+// scales are sorted by compiled radius and cut into the largest groups a k_xym instance exists for;
+// every group reads the input once.
 cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *in, float *const *out,
                           cudaStream_t st)
 {
     const Dims &d = p->dims;
-    if (d.ny > 65535 * XM_TY || d.nz > 65535 || n < 1 || n > PGSF_MAX_SCALES) return cudaErrorInvalidConfiguration;
-    XYMultiParams P;
-    P.d = d;
-    P.n = n;
-    int rmax = 0;
-    for (int i = 0; i < n; ++i) {
-        const ScalePlan &sp = p->scales[scales[i]];
-        P.rc[i] = sp.rxy_c;
-        P.out[i] = out[i];
-        P.t[i] = sp.txy;
-        if (sp.rxy_c > rmax) rmax = sp.rxy_c;
+    if (d.nz > 65535 || n < 1 || n > PGSF_MAX_SCALES) return cudaErrorInvalidConfiguration;
+    int order[PGSF_MAX_SCALES];
+    for (int i = 0; i < n; ++i) order[i] = i;
+    for (int i = 1; i < n; ++i)          // insertion sort by compiled radius (stable)
+        for (int j = i; j > 0 && p->scales[scales[order[j]]].rxy_c < p->scales[scales[order[j - 1]]].rxy_c; --j) {
+            const int t = order[j]; order[j] = order[j - 1]; order[j - 1] = t;
+        }
+    // rows per CTA: a few waves of CTAs; a chunk start recomputes 16 + 12 rows
+    int nch = 1;
+    {
+        const long long base = (long long)((d.nx + XM_NT - 1) / XM_NT) * d.nz;
+        const long long want = 6LL * p->sm_count * 2;
+        nch = (int)((want + base - 1) / base);
+        const int maxch = (d.ny + 127) / 128;
+        if (nch > maxch) nch = maxch;
+        if (nch < 1) nch = 1;
     }
-    for (int i = n; i < PGSF_MAX_SCALES; ++i) { P.rc[i] = 0; P.out[i] = nullptr; }
-    char name[32];
-    if (n == 1) snprintf(name, sizeof name, "xy_s%d", scales[0]);
-    else snprintf(name, sizeof name, "xy_all");
-    LaunchScope ls(p, name, st);
-    switch (rmax) {
-    case 3: return launch_xy_multi<3>(in, P, st);
-    case 6: return launch_xy_multi<6>(in, P, st);
-    case 9: return launch_xy_multi<9>(in, P, st);
-    case 12: return launch_xy_multi<12>(in, P, st);
-    default: return cudaErrorNotSupported;
+    int ychunk = ((d.ny + nch - 1) / nch + 15) / 16 * 16;
+    if ((d.ny + ychunk - 1) / ychunk > 65535) return cudaErrorInvalidConfiguration;
+    int pos = 0;
+    while (pos < n) {
+        int take = n - pos < XM_MAXS ? n - pos : XM_MAXS;
+        int rc[XM_MAXS];
+        XymParams P;
+        for (; take >= 1; --take) {
+            for (int i = 0; i < take; ++i) rc[i] = p->scales[scales[order[pos + i]]].rxy_c;
+            if (xym_dispatch(take, rc, nullptr, P, 0, st, true, nullptr)) break;
+        }
+        if (take < 1) return cudaErrorNotSupported;
+        P.d = d;
+        P.ychunk = ychunk;
+        unsigned mask = 0;
+        for (int i = 0; i < XM_MAXS; ++i) {
+            const int j = i < take ? i : 0;
+            const int sidx = scales[order[pos + j]];
+            P.out[i] = out[order[pos + j]];
+            P.t[i] = p->scales[sidx].txy;
+            if (i < take) mask |= 1u << sidx;
+        }
+        char name[32];
+        snprintf(name, sizeof name, "xy_m%u", mask);
+        LaunchScope ls(p, name, st);
+        cudaError_t e = cudaSuccess;
+        xym_dispatch(take, rc, in, P, p->sm_count, st, false, &e);
+        if (e != cudaSuccess) return e;
+        pos += take;
     }
+    return cudaSuccess;
 }
 
 // frequency pass of one scale: in (x/y-filtered cube) -> out
