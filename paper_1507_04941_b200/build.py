@@ -11,7 +11,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpgsf.so")
-SOURCES = ["pgsf_api.cu", "pgsf_generic.cu", "pgsf_filter.cu", "pgsf_stats.cu"]
+SOURCES = ["pgsf_z_r96.cu", "pgsf_z_r72.cu", "pgsf_z_r48.cu", "pgsf_z_r24.cu", "pgsf_z_r12.cu", "pgsf_z_r6.cu",
+           "pgsf_api.cu", "pgsf_generic.cu", "pgsf_filter.cu", "pgsf_stats.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--use_fast_math=false",
@@ -42,14 +43,20 @@ def build(force: bool = False, verbose: bool = False) -> str:
     flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
     objs = []
     procs = []
+    hdrs = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".h", ".cuh"))]
+    hdrs += [os.path.join(ROOT, "include", "pgsf.h"), os.path.abspath(__file__)]
+    newest_hdr = max(os.path.getmtime(h) for h in hdrs)
     for src in SOURCES:
         obj = os.path.join(objdir, src.replace(".cu", ".o"))
+        objs.append(obj)
+        if (not force and os.path.exists(obj)
+                and os.path.getmtime(obj) > max(newest_hdr, os.path.getmtime(os.path.join(CSRC, src)))):
+            continue   # object is newer than its source and every header
         cmd = [_nvcc(), *flags, "-I", os.path.join(ROOT, "include"), "-I", CSRC, "-c",
                os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
-        objs.append(obj)
     for cmd, pr in procs:
         out, _ = pr.communicate()
         if verbose or pr.returncode != 0:

@@ -417,6 +417,16 @@ pgsf_status pgsf_find_multiscale(pgsf_plan *p, const float *d_in, float *const *
             cudaError_t ce = pgsf::fast_xy_multi(p, idx, S, d_in + off, park, st);
             if (ce != cudaSuccess) return cuda_fail(p, ce, "xy filter launch");
             for (int s = 0; s < S; ++s) {
+                if (p->fast_stats) {
+                    // frequency pass and z-direction window sums in one march; then the x/y window sums
+                    float *Z1 = w.stmp, *Z2 = w.stmp + p->dims.cube;
+                    ce = pgsf::fast_zm(p, s, park[s], d_filtered[s] + off, Z1, Z2, st);
+                    if (ce != cudaSuccess) return cuda_fail(p, ce, "z filter + window launch");
+                    ce = pgsf::fast_threshold_xy(p, d_filtered[s] + off, Z1, Z2, d_mask + off, s > 0, nullptr,
+                                                 nullptr, (s == S - 1) ? d_count : nullptr, st);
+                    if (ce != cudaSuccess) return cuda_fail(p, ce, "threshold launch");
+                    continue;
+                }
                 ce = pgsf::fast_z(p, s, park[s], d_filtered[s] + off, st);
                 if (ce != cudaSuccess) return cuda_fail(p, ce, "z filter launch");
                 rc = threshold_batch(p, d_filtered[s] + off, d_mask + off, s > 0, nullptr, nullptr,

@@ -1,0 +1,44 @@
+// Device helpers shared by the filter kernels (internal; not part of the ABI).
+#pragma once
+#include "pgsf_internal.h"
+
+namespace pgsf {
+namespace {
+
+__device__ __forceinline__ float2 ffma2(float2 a, float g, float2 c)
+{
+    // d = a * {g, g} + c, both halves in one instruction
+    const float2 gg = make_float2(g, g);
+    unsigned long long ra = *reinterpret_cast<const unsigned long long *>(&a);
+    unsigned long long rb = *reinterpret_cast<const unsigned long long *>(&gg);
+    unsigned long long rc = *reinterpret_cast<const unsigned long long *>(&c);
+    unsigned long long rd;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(rd) : "l"(ra), "l"(rb), "l"(rc));
+    return *reinterpret_cast<float2 *>(&rd);
+}
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem, bool valid)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    const int bytes = valid ? 16 : 0;  // src-size 0 -> 16 bytes of zeros
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gmem), "r"(bytes));
+}
+__device__ __forceinline__ void cp_async_wait_all()
+{
+    asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
+}
+
+// Kahan-compensated s += v (e holds the running low-order error)
+__device__ __forceinline__ void kahan_add(float &s, float &e, float v)
+{
+    const float y = v - e;
+    const float t = s + y;
+    e = (t - s) - y;
+    s = t;
+}
+
+__host__ __device__ constexpr int round4(int v) { return (v + 3) & ~3; }
+
+
+}  // namespace
+}  // namespace pgsf

@@ -17,36 +17,24 @@
 #include <stdio.h>
 
 #include "pgsf_internal.h"
+#include "pgsf_device.cuh"
 
 namespace pgsf {
+// per-radius entry points of the frequency-axis kernels (pgsf_z_r*.cu)
+cudaError_t launch_z_r6(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
+cudaError_t launch_zm_r6(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, cudaStream_t st);
+cudaError_t launch_z_r12(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
+cudaError_t launch_zm_r12(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, cudaStream_t st);
+cudaError_t launch_z_r24(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
+cudaError_t launch_zm_r24(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, cudaStream_t st);
+cudaError_t launch_z_r48(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
+cudaError_t launch_zm_r48(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, cudaStream_t st);
+cudaError_t launch_z_r72(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
+cudaError_t launch_zm_r72(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, cudaStream_t st);
+cudaError_t launch_z_r96(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
+cudaError_t launch_zm_r96(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, cudaStream_t st);
+
 namespace {
-
-// ------------------------------------------------------------------------------------ helpers
-
-__device__ __forceinline__ float2 ffma2(float2 a, float g, float2 c)
-{
-    // d = a * {g, g} + c, both halves in one instruction
-    const float2 gg = make_float2(g, g);
-    unsigned long long ra = *reinterpret_cast<const unsigned long long *>(&a);
-    unsigned long long rb = *reinterpret_cast<const unsigned long long *>(&gg);
-    unsigned long long rc = *reinterpret_cast<const unsigned long long *>(&c);
-    unsigned long long rd;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(rd) : "l"(ra), "l"(rb), "l"(rc));
-    return *reinterpret_cast<float2 *>(&rd);
-}
-
-__device__ __forceinline__ void cp_async16(void *smem, const void *gmem, bool valid)
-{
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    const int bytes = valid ? 16 : 0;  // src-size 0 -> 16 bytes of zeros
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gmem), "r"(bytes));
-}
-__device__ __forceinline__ void cp_async_wait_all()
-{
-    asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
-}
-
-__host__ __device__ constexpr int round4(int v) { return (v + 3) & ~3; }
 
 // ------------------------------------------------------------------------------------ x/y passes
 //
@@ -248,90 +236,6 @@ __global__ void __launch_bounds__(XM_NT, 2) k_xym(const float *__restrict__ in, 
     }
 }
 
-// ------------------------------------------------------------------------------------ z pass
-
-constexpr int Z_XT = 128;       // columns per CTA (32 float4 lanes = one warp per plane row)
-constexpr int Z_PZ = 8;         // channels per thread
-constexpr int Z_WARPS = 8;      // z groups per CTA
-constexpr int Z_THREADS = 32 * Z_WARPS;
-constexpr int Z_ZB = Z_PZ * Z_WARPS;   // 64 output channels per CTA
-
-template <int RZ>
-struct ZShape {
-    static constexpr int PLANES = Z_ZB + 2 * RZ;
-    static constexpr int SMEM = PLANES * Z_XT * 4;
-};
-
-template <int RZ>
-__global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, float *__restrict__ out,
-                                                 Dims d, Taps t)
-{
-    using S = ZShape<RZ>;
-    extern __shared__ __align__(16) float smem[];  // [PLANES][Z_XT]
-    const int tid = threadIdx.x, lane = tid & 31, wz = tid >> 5;
-    const int z0 = blockIdx.x * Z_ZB, x0 = blockIdx.y * Z_XT, y = blockIdx.z;
-    const int gx = x0 + 4 * lane;
-    const bool col_ok = gx < d.nx;
-    const float *col_in = in + (long long)y * d.nx + (col_ok ? gx : 0);
-
-    // stage channels z0-RZ .. z0+ZB+RZ-1 of this 128-column strip; outside the cube -> 0 (C-5)
-    for (int pz = wz; pz < S::PLANES; pz += Z_WARPS) {
-        const int gz = z0 - RZ + pz;
-        const bool ok = col_ok && gz >= 0 && gz < d.nz;
-        cp_async16(smem + pz * Z_XT + 4 * lane, ok ? col_in + (long long)gz * d.plane : in, ok);
-    }
-    cp_async_wait_all();
-    __syncthreads();
-
-    // Eq. 5: f[z] = sum_o t2[z+o] gz[o]; the thread walks along z, PZ accumulators x 4 columns.
-    // Taps are stored at g[o + kTapPad] with kTapPad zeros on both sides.
-    float2 acc[Z_PZ][2];
-#pragma unroll
-    for (int p = 0; p < Z_PZ; ++p) acc[p][0] = acc[p][1] = make_float2(0.f, 0.f);
-    const float *base = smem + (wz * Z_PZ) * Z_XT + 4 * lane;
-    if constexpr (RZ <= 48) {
-        // fully unrolled: every tap index is a compile-time constant-bank offset
-#pragma unroll
-        for (int j = 0; j < Z_PZ + 2 * RZ; ++j) {
-            const float4 v = *reinterpret_cast<const float4 *>(base + j * Z_XT);
-#pragma unroll
-            for (int p = 0; p < Z_PZ; ++p) {
-                const int o = j - p;
-                if (o >= 0 && o <= 2 * RZ) {
-                    acc[p][0] = ffma2(make_float2(v.x, v.y), t.g[o + kTapPad], acc[p][0]);
-                    acc[p][1] = ffma2(make_float2(v.z, v.w), t.g[o + kTapPad], acc[p][1]);
-                }
-            }
-        }
-    } else {
-        // too long to unroll: walk the PZ + 2 RZ staged channels in chunks of 8; the zero padding of
-        // the tap array makes the ramp-up / ramp-down iterations the same code as the steady state
-        static_assert((Z_PZ + 2 * RZ) % 8 == 0 && kTapPad >= Z_PZ - 1, "chunking");
-#pragma unroll 1
-        for (int jc = 0; jc < Z_PZ + 2 * RZ; jc += 8) {
-#pragma unroll
-            for (int jj = 0; jj < 8; ++jj) {
-                const float4 v = *reinterpret_cast<const float4 *>(base + (jc + jj) * Z_XT);
-#pragma unroll
-                for (int p = 0; p < Z_PZ; ++p) {
-                    const float g = t.g[jc + jj - p + kTapPad];
-                    acc[p][0] = ffma2(make_float2(v.x, v.y), g, acc[p][0]);
-                    acc[p][1] = ffma2(make_float2(v.z, v.w), g, acc[p][1]);
-                }
-            }
-        }
-    }
-    if (!col_ok) return;
-    float *col_out = out + (long long)y * d.nx + gx;
-#pragma unroll
-    for (int p = 0; p < Z_PZ; ++p) {
-        const int gz = z0 + wz * Z_PZ + p;
-        if (gz < d.nz)
-            *reinterpret_cast<float4 *>(col_out + (long long)gz * d.plane) =
-                make_float4(acc[p][0].x, acc[p][0].y, acc[p][1].x, acc[p][1].y);
-    }
-}
-
 template <int NS, int RA, int RB, int RC, int RD>
 cudaError_t launch_xym(const float *in, const XymParams &P, int sm_count, cudaStream_t st)
 {
@@ -345,21 +249,6 @@ cudaError_t launch_xym(const float *in, const XymParams &P, int sm_count, cudaSt
     (void)sm_count;
     dim3 grid((P.d.nx + XM_NT - 1) / XM_NT, (P.d.ny + P.ychunk - 1) / P.ychunk, P.d.nz);
     k_xym<NS, RA, RB, RC, RD><<<grid, XM_NT, SMEM, st>>>(in, P);
-    return cudaGetLastError();
-}
-
-template <int RZ>
-cudaError_t launch_z(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st)
-{
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_z<RZ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             ZShape<RZ>::SMEM);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
-    dim3 grid((d.nz + Z_ZB - 1) / Z_ZB, (d.nx + Z_XT - 1) / Z_XT, d.ny);
-    k_z<RZ><<<grid, Z_THREADS, ZShape<RZ>::SMEM, st>>>(in, out, d, t);
     return cudaGetLastError();
 }
 
@@ -476,17 +365,39 @@ cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStr
 {
     const Dims &d = p->dims;
     const ScalePlan &sp = p->scales[scale];
-    if (d.ny > 65535 || d.nz > 65535 * Z_ZB) return cudaErrorInvalidConfiguration;
+    if (d.ny > 65535 || d.nz > 65535 * 64) return cudaErrorInvalidConfiguration;
     char name[32];
     snprintf(name, sizeof name, "z_s%d", scale);
     LaunchScope ls(p, name, st);
     switch (sp.rz_c) {
-    case 6: return launch_z<6>(in, out, d, sp.tz, st);
-    case 12: return launch_z<12>(in, out, d, sp.tz, st);
-    case 24: return launch_z<24>(in, out, d, sp.tz, st);
-    case 48: return launch_z<48>(in, out, d, sp.tz, st);
-    case 72: return launch_z<72>(in, out, d, sp.tz, st);
-    case 96: return launch_z<96>(in, out, d, sp.tz, st);
+    case 6: return launch_z_r6(in, out, d, sp.tz, st);
+    case 12: return launch_z_r12(in, out, d, sp.tz, st);
+    case 24: return launch_z_r24(in, out, d, sp.tz, st);
+    case 48: return launch_z_r48(in, out, d, sp.tz, st);
+    case 72: return launch_z_r72(in, out, d, sp.tz, st);
+    case 96: return launch_z_r96(in, out, d, sp.tz, st);
+    default: return cudaErrorNotSupported;
+    }
+}
+
+// frequency pass of one scale fused with the z-direction window sums of the statistics:
+// in (x/y-filtered cube) -> out (filtered cube), Z1, Z2
+cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, cudaStream_t st)
+{
+    const Dims &d = p->dims;
+    const ScalePlan &sp = p->scales[scale];
+    if (d.ny > 65535) return cudaErrorInvalidConfiguration;
+    const int hz = p->desc.box_half[2];
+    char name[32];
+    snprintf(name, sizeof name, "zm_s%d", scale);
+    LaunchScope ls(p, name, st);
+    switch (sp.rz_c) {
+    case 6: return launch_zm_r6(in, out, Z1, Z2, d, hz, sp.tz, st);
+    case 12: return launch_zm_r12(in, out, Z1, Z2, d, hz, sp.tz, st);
+    case 24: return launch_zm_r24(in, out, Z1, Z2, d, hz, sp.tz, st);
+    case 48: return launch_zm_r48(in, out, Z1, Z2, d, hz, sp.tz, st);
+    case 72: return launch_zm_r72(in, out, Z1, Z2, d, hz, sp.tz, st);
+    case 96: return launch_zm_r96(in, out, Z1, Z2, d, hz, sp.tz, st);
     default: return cudaErrorNotSupported;
     }
 }

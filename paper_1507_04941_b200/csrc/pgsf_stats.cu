@@ -440,6 +440,13 @@ cudaError_t fast_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_i
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
+    return fast_threshold_xy(p, f, Z1, Z2, mask, or_into, mean, sd, count, st);
+}
+
+cudaError_t fast_threshold_xy(pgsf_plan *p, const float *f, const float *Z1, const float *Z2, uint8_t *mask,
+                              int or_into, float *mean, float *sd, unsigned long long *count, cudaStream_t st)
+{
+    const Dims &d = p->dims;
     YmParams yp;
     yp.d = d;
     yp.hy = p->desc.box_half[1];

@@ -1,0 +1,293 @@
+// Frequency-axis kernels of the separable form of Eq. 2 (Eq. 5), as templates on the compiled
+// radius RZ.  Every radius is instantiated in its own translation unit (pgsf_z_r*.cu) so that the long,
+// fully unrolled tap walks compile in parallel.
+#pragma once
+#include "pgsf_device.cuh"
+
+namespace pgsf {
+namespace {
+
+// ------------------------------------------------------------------------------------ z pass
+
+constexpr int Z_XT = 128;       // columns per CTA (32 float4 lanes = one warp per plane row)
+constexpr int Z_PZ = 8;         // channels per thread
+constexpr int Z_WARPS = 8;      // z groups per CTA
+constexpr int Z_THREADS = 32 * Z_WARPS;
+constexpr int Z_ZB = Z_PZ * Z_WARPS;   // 64 output channels per CTA
+
+template <int RZ>
+struct ZShape {
+    static constexpr int PLANES = Z_ZB + 2 * RZ;
+    static constexpr int SMEM = PLANES * Z_XT * 4;
+};
+
+// Eq. 5 for one thread: PZ consecutive channels x 4 columns from the staged slab (`base` = the
+// thread's first staged channel, i.e. tap -RZ of its first output).  Taps are stored at
+// g[o + kTapPad] with kTapPad zeros on both sides.  The walk over the PZ + 2 RZ staged channels is
+// unrolled by template recursion for RZ <= 48 (a `#pragma unroll` of 104 iterations is not honoured), so
+// every tap is a compile-time constant-bank offset and the body is LDS.128 + 16 FFMA2 per channel.
+template <int RZ, int J>
+__device__ __forceinline__ void z_step(const float *__restrict__ base, const Taps &t, float2 (&acc)[Z_PZ][2])
+{
+    const float4 v = *reinterpret_cast<const float4 *>(base + J * Z_XT);
+#pragma unroll
+    for (int p = 0; p < Z_PZ; ++p) {
+        const int o = J - p;
+        if (o >= 0 && o <= 2 * RZ) {
+            acc[p][0] = ffma2(make_float2(v.x, v.y), t.g[o + kTapPad], acc[p][0]);
+            acc[p][1] = ffma2(make_float2(v.z, v.w), t.g[o + kTapPad], acc[p][1]);
+        }
+    }
+}
+
+template <int RZ, int J0, int N>
+__device__ __forceinline__ void z_steps(const float *__restrict__ base, const Taps &t, float2 (&acc)[Z_PZ][2])
+{
+    if constexpr (N == 1) {
+        z_step<RZ, J0>(base, t, acc);
+    } else {
+        z_steps<RZ, J0, N / 2>(base, t, acc);
+        z_steps<RZ, J0 + N / 2, N - N / 2>(base, t, acc);
+    }
+}
+
+template <int RZ>
+__device__ __forceinline__ void z_accumulate(const float *__restrict__ base, const Taps &t, float2 (&acc)[Z_PZ][2])
+{
+#pragma unroll
+    for (int p = 0; p < Z_PZ; ++p) acc[p][0] = acc[p][1] = make_float2(0.f, 0.f);
+    if constexpr (RZ <= 48) {
+        z_steps<RZ, 0, Z_PZ + 2 * RZ>(base, t, acc);
+    } else {
+        // 150 - 200 channels: walk them in chunks of 8 with the tap index in a uniform register; the zero
+        // padding of the tap array makes the ramp-up / ramp-down iterations the same code as the steady state
+        static_assert((Z_PZ + 2 * RZ) % 8 == 0 && kTapPad >= Z_PZ - 1, "chunking");
+#pragma unroll 1
+        for (int jc = 0; jc < Z_PZ + 2 * RZ; jc += 8) {
+#pragma unroll
+            for (int jj = 0; jj < 8; ++jj) {
+                const float4 v = *reinterpret_cast<const float4 *>(base + (jc + jj) * Z_XT);
+#pragma unroll
+                for (int p = 0; p < Z_PZ; ++p) {
+                    const float g = t.g[jc + jj - p + kTapPad];
+                    acc[p][0] = ffma2(make_float2(v.x, v.y), g, acc[p][0]);
+                    acc[p][1] = ffma2(make_float2(v.z, v.w), g, acc[p][1]);
+                }
+            }
+        }
+    }
+}
+
+template <int RZ>
+__global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, float *__restrict__ out,
+                                                 Dims d, Taps t)
+{
+    using S = ZShape<RZ>;
+    extern __shared__ __align__(16) float smem[];  // [PLANES][Z_XT]
+    const int tid = threadIdx.x, lane = tid & 31, wz = tid >> 5;
+    const int z0 = blockIdx.x * Z_ZB, x0 = blockIdx.y * Z_XT, y = blockIdx.z;
+    const int gx = x0 + 4 * lane;
+    const bool col_ok = gx < d.nx;
+    const float *col_in = in + (long long)y * d.nx + (col_ok ? gx : 0);
+
+    // stage channels z0-RZ .. z0+ZB+RZ-1 of this 128-column strip; outside the cube -> 0 (C-5)
+    for (int pz = wz; pz < S::PLANES; pz += Z_WARPS) {
+        const int gz = z0 - RZ + pz;
+        const bool ok = col_ok && gz >= 0 && gz < d.nz;
+        cp_async16(smem + pz * Z_XT + 4 * lane, ok ? col_in + (long long)gz * d.plane : in, ok);
+    }
+    cp_async_wait_all();
+    __syncthreads();
+
+    // Eq. 5: f[z] = sum_o t2[z+o] gz[o]; the thread walks along z, PZ accumulators x 4 columns.
+    float2 acc[Z_PZ][2];
+    z_accumulate<RZ>(smem + (wz * Z_PZ) * Z_XT + 4 * lane, t, acc);
+    if (!col_ok) return;
+    float *col_out = out + (long long)y * d.nx + gx;
+#pragma unroll
+    for (int p = 0; p < Z_PZ; ++p) {
+        const int gz = z0 + wz * Z_PZ + p;
+        if (gz < d.nz)
+            *reinterpret_cast<float4 *>(col_out + (long long)gz * d.plane) =
+                make_float4(acc[p][0].x, acc[p][0].y, acc[p][1].x, acc[p][1].y);
+    }
+}
+
+// ------------------------------------------------------------------------------------ z pass + z window sums
+//
+// k_zm<RZ>: the frequency pass of k_z FUSED with the frequency-direction window sums of the local
+// statistics ("three directional sums"; the z direction first).  A CTA owns a strip of 128
+// columns of one row and marches along the WHOLE frequency axis in steps of 64 channels:
+//   filter phase  as k_z: slab of 64 + 2 RZ channels of t2 staged in shared memory, every thread
+//                 4 columns x 8 channels of Eq. 5; f goes to HBM (it is an output) and to a 64-channel
+//                 slab in shared memory;
+//   window phase  thread (column c, quantity q in {f, f^2}) walks the 64 new channels: the channel
+//                 entering the window [z - hz, z + hz] comes from the shared-memory slab, the one
+//                 leaving it is re-read from the f this CTA wrote 2 hz + 1 channels earlier -- the
+//                 strip is narrow, so that plane is still in L2 (ld.global.cg); running sums are
+//                 Kahan-compensated as in k_zbox.  Writes Z1 = sum f, Z2 = sum f^2 (window clipped to
+//                 the cube, C-7).
+// Against k_z + k_zbox this saves one HBM read of t2's halo, both HBM reads of f by k_zbox and one
+// launch: 8 + 8 + 16 GB instead of 17 + 35 GB per scale at config 3.
+
+// n steps of the compensated sliding window of one (column, quantity): add the entering channel, write
+// the window sum, subtract the leaving channel.  lead / trail advance by one staged channel per step.
+template <bool SQ>
+__device__ __forceinline__ float *window_run(float &s, float &e, const float *__restrict__ lead,
+                                             const float *__restrict__ trail, float *__restrict__ zp, long long plane, int n)
+{
+#pragma unroll 8
+    for (int j = 0; j < n; ++j) {
+        const float a = lead[j * Z_XT], b = trail[j * Z_XT];
+        kahan_add(s, e, SQ ? a * a : a);
+        *zp = s - e;
+        zp += plane;
+        kahan_add(s, e, SQ ? -(b * b) : -b);
+    }
+    return zp;
+}
+
+template <int RZ>
+struct ZmShape {
+    static constexpr int PLANES = Z_ZB + 2 * RZ;           // t2 slab; its first Z_ZB planes are reused as the f slab
+    static constexpr int SMEM = (PLANES + Z_ZB) * Z_XT * 4; // + slab of the channels leaving the window
+};
+
+template <int RZ>
+__global__ void __launch_bounds__(Z_THREADS) k_zm(const float *__restrict__ in, float *out, float *__restrict__ Z1,
+                                                  float *__restrict__ Z2, Dims d, int hz, Taps t)
+{
+    using S = ZmShape<RZ>;
+    extern __shared__ __align__(16) float smem[];  // [PLANES][Z_XT] t2 slab / f slab, [Z_ZB][Z_XT] leaving slab
+    float *fs = smem;                              // f of this step (written after the filter phase)
+    float *ts = smem + S::PLANES * Z_XT;           // f of the channels leaving the window in this step
+    const int tid = threadIdx.x, lane = tid & 31, wz = tid >> 5;
+    const int x0 = blockIdx.x * Z_XT, y = blockIdx.y;
+    const int gx = x0 + 4 * lane;
+    const bool col_ok = gx < d.nx;
+    const float *col_in = in + (long long)y * d.nx + (col_ok ? gx : 0);
+    float *col_out = out + (long long)y * d.nx + (col_ok ? gx : 0);
+    // window phase: one thread per (column, quantity)
+    const int c = tid & (Z_XT - 1);
+    const bool sq = tid >= Z_XT;
+    const bool c_ok = x0 + c < d.nx;
+    const long long cb = (long long)y * d.nx + x0 + c;
+    float *Zq = sq ? Z2 : Z1;
+    float s = 0.f, e = 0.f;
+    const int nz = d.nz;
+    const int nsteps = (nz + hz + Z_ZB - 1) / Z_ZB;   // entering channels 0 .. nz + hz - 1 (the tail drains the window)
+
+    for (int k = 0; k < nsteps; ++k) {
+        const int z0 = k * Z_ZB;
+        // channels leaving the window in this step: z0 - 2 hz + j, j = 0..63.  Those written in EARLIER steps
+        // (by this CTA: still in L2) are fetched now, together with the t2 slab; those of this step's own
+        // f block (2 hz < 64) are read from the f slab instead.
+        for (int pz = wz; pz < Z_ZB; pz += Z_WARPS) {
+            const int zt = z0 - 2 * hz + pz;
+            const bool ok = col_ok && zt >= 0 && zt < z0;
+            cp_async16(ts + pz * Z_XT + 4 * lane, ok ? col_out + (long long)zt * d.plane : in, ok);
+        }
+        if (z0 < nz) {
+            // stage channels z0-RZ .. z0+ZB+RZ-1 of t2; outside the cube -> 0 (C-5)
+            for (int pz = wz; pz < S::PLANES; pz += Z_WARPS) {
+                const int gz = z0 - RZ + pz;
+                const bool ok = col_ok && gz >= 0 && gz < nz;
+                cp_async16(smem + pz * Z_XT + 4 * lane, ok ? col_in + (long long)gz * d.plane : in, ok);
+            }
+        }
+        cp_async_wait_all();
+        __syncthreads();
+        if (z0 < nz) {
+            float2 acc[Z_PZ][2];
+            z_accumulate<RZ>(smem + (wz * Z_PZ) * Z_XT + 4 * lane, t, acc);
+            __syncthreads();   // every warp is done with the t2 slab: its head becomes the f slab
+#pragma unroll
+            for (int p = 0; p < Z_PZ; ++p) {
+                const int gz = z0 + wz * Z_PZ + p;
+                const float4 v = make_float4(acc[p][0].x, acc[p][0].y, acc[p][1].x, acc[p][1].y);
+                *reinterpret_cast<float4 *>(fs + (wz * Z_PZ + p) * Z_XT + 4 * lane) = v;
+                if (col_ok && gz < nz) *reinterpret_cast<float4 *>(col_out + (long long)gz * d.plane) = v;
+            }
+            __syncthreads();   // f slab complete
+        }
+        if (c_ok) {
+            if (z0 >= hz && z0 + Z_ZB <= nz) {
+                // interior step: all 64 entering channels and all 64 outputs are inside the cube
+                const int jsplit = min(2 * hz, Z_ZB);   // leaving channel: ts[j] for j < jsplit, else fs[j - 2 hz]
+                float *zp = Zq + (long long)(z0 - hz) * d.plane + cb;
+                if (sq) {
+                    zp = window_run<true>(s, e, fs + c, ts + c, zp, d.plane, jsplit);
+                    window_run<true>(s, e, fs + jsplit * Z_XT + c, fs + c, zp, d.plane, Z_ZB - jsplit);
+                } else {
+                    zp = window_run<false>(s, e, fs + c, ts + c, zp, d.plane, jsplit);
+                    window_run<false>(s, e, fs + jsplit * Z_XT + c, fs + c, zp, d.plane, Z_ZB - jsplit);
+                }
+            } else {
+                for (int j = 0; j < Z_ZB; ++j) {
+                    const int zl = z0 + j;          // channel entering the window of output zo
+                    const int zo = zl - hz;
+                    if (zl < nz) {
+                        const float v = fs[j * Z_XT + c];
+                        kahan_add(s, e, sq ? v * v : v);
+                    }
+                    if (zo >= 0 && zo < nz) {
+                        Zq[(long long)zo * d.plane + cb] = s - e;
+                        const int jt = j - 2 * hz;  // the channel leaving after this output, relative to z0
+                        const float v = jt >= 0 ? fs[jt * Z_XT + c] : ts[j * Z_XT + c];   // (zero where zt < 0)
+                        kahan_add(s, e, sq ? -(v * v) : -v);
+                    }
+                }
+            }
+        }
+        __syncthreads();   // slabs are overwritten by the next step
+    }
+}
+
+template <int RZ>
+cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t,
+                      cudaStream_t st)
+{
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_zm<RZ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             ZmShape<RZ>::SMEM);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dim3 grid((d.nx + Z_XT - 1) / Z_XT, d.ny);
+    k_zm<RZ><<<grid, Z_THREADS, ZmShape<RZ>::SMEM, st>>>(in, out, Z1, Z2, d, hz, t);
+    return cudaGetLastError();
+}
+
+template <int RZ>
+cudaError_t launch_z(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st)
+{
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_z<RZ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             ZShape<RZ>::SMEM);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dim3 grid((d.nz + Z_ZB - 1) / Z_ZB, (d.nx + Z_XT - 1) / Z_XT, d.ny);
+    k_z<RZ><<<grid, Z_THREADS, ZShape<RZ>::SMEM, st>>>(in, out, d, t);
+    return cudaGetLastError();
+}
+
+
+}  // namespace
+}  // namespace pgsf
+
+// one pair of plain entry points per radius
+#define PGSF_INSTANTIATE_Z(RZ)                                                                              \
+    namespace pgsf {                                                                                        \
+    cudaError_t launch_z_r##RZ(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st)  \
+    {                                                                                                       \
+        return launch_z<RZ>(in, out, d, t, st);                                                             \
+    }                                                                                                       \
+    cudaError_t launch_zm_r##RZ(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz,   \
+                                const Taps &t, cudaStream_t st)                                             \
+    {                                                                                                       \
+        return launch_zm<RZ>(in, out, Z1, Z2, d, hz, t, st);                                                \
+    }                                                                                                       \
+    }
