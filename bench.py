@@ -26,6 +26,7 @@ if ROOT not in sys.path:
 METRIC = "Gvoxel/s per Gaussian scale (filter+threshold)"
 UNIT = "Gvoxel-scales/s"
 STATS_FLOPS = 21            # statistics + threshold per voxel per scale
+STATS_Z_FLOPS = 5           # of which the z-direction window: 2 x (add + subtract) + 1 square
 FP32_LANES_PER_SM = 128     # B200_PROFILING.md unit counts: 148 SMs, 1965 MHz max SM clock
 
 
@@ -204,6 +205,11 @@ def _kernel_work(name: str, w, taps, n_vox: int):
     if kind == "z" and tail.startswith("s"):
         t = taps[int(tail[1:])]
         return 2 * t[2] * n_vox, 8 * n_vox
+    if kind == "zm" and tail.startswith("s"):   # z pass + z-direction window sums (5 of the 21 statistics flops)
+        t = taps[int(tail[1:])]
+        return (2 * t[2] + STATS_Z_FLOPS) * n_vox, 8 * n_vox
+    if kind == "stats" and tail == "xybox":     # x/y window sums + selection after a fused zm launch
+        return (STATS_FLOPS - STATS_Z_FLOPS) * n_vox, 5 * n_vox
     if kind == "stats" and tail == "all":    # statistics of every scale, one mask write
         return STATS_FLOPS * S * n_vox, (4 * S + 1) * n_vox
     if kind == "stats":

@@ -163,10 +163,15 @@ __global__ void __launch_bounds__(XM_NT, 2) k_xym(const float *__restrict__ in, 
     const long long plane_off = (long long)z * d.plane;
     const int gx = x0 + tid;
     const bool col_ok = gx < d.nx;
-    float *o0 = P.out[0] + plane_off + gx;
-    float *o1 = NS > 1 ? P.out[NS > 1 ? 1 : 0] + plane_off + gx : nullptr;
-    float *o2 = NS > 2 ? P.out[NS > 2 ? 2 : 0] + plane_off + gx : nullptr;
-    float *o3 = NS > 3 ? P.out[NS > 3 ? 3 : 0] + plane_off + gx : nullptr;
+    // running output pointers: row 2 m of scale s for the current march step k, m = k - ceil(R_s / 2)
+    constexpr int RMAX = NS > 3 ? RD : NS > 2 ? RC : NS > 1 ? RB : RA;   // (the scales are sorted by radius)
+    constexpr int RMIN = RA;
+    const long long col0 = plane_off + (col_ok ? gx : 0);
+    const int k0 = ys / 2;
+    float *o0 = P.out[0] + col0 + (long long)(2 * (k0 - (RA + 1) / 2)) * d.nx;
+    float *o1 = NS > 1 ? P.out[NS > 1 ? 1 : 0] + col0 + (long long)(2 * (k0 - (RB + 1) / 2)) * d.nx : nullptr;
+    float *o2 = NS > 2 ? P.out[NS > 2 ? 2 : 0] + col0 + (long long)(2 * (k0 - (RC + 1) / 2)) * d.nx : nullptr;
+    float *o3 = NS > 3 ? P.out[NS > 3 ? 3 : 0] + col0 + (long long)(2 * (k0 - (RD + 1) / 2)) * d.nx : nullptr;
 
     XmY<RA> sa; XmY<RB> sb; XmY<RC> sc; XmY<RD> sd;
     sa.init(); sb.init(); sc.init(); sd.init();
@@ -220,17 +225,38 @@ __global__ void __launch_bounds__(XM_NT, 2) k_xym(const float *__restrict__ in, 
         for (int kk = 0; kk < XM_NB; ++kk) {
             const float2 *su = s_u + (kk * NS) * XM_U + pi;
             const int k = kbase + kk;
-            auto emit = [&](float *o, float2 v, int m) {
-                const int r0 = 2 * m;
+            const float2 va = sa.step(su[0], P.t[0].gy);
+            float2 vb, vc, vd;
+            if constexpr (NS > 1) vb = sb.step(su[XM_U], P.t[NS > 1 ? 1 : 0].gy);
+            if constexpr (NS > 2) vc = sc.step(su[2 * XM_U], P.t[NS > 2 ? 2 : 0].gy);
+            if constexpr (NS > 3) vd = sd.step(su[3 * XM_U], P.t[NS > 3 ? 3 : 0].gy);
+            // rows 2 m, 2 m + 1 with m = k - ceil(R/2) per scale; the common case (all of them inside the
+            // chunk) stores through the running row pointers without any test
+            const bool all_in = 2 * (k - (RMAX + 1) / 2) >= ya && 2 * (k - (RMIN + 1) / 2) + 1 < yb;
+            if (all_in) {
                 if (col_ok) {
-                    if (r0 >= ya && r0 < yb) o[(long long)r0 * d.nx] = v.x;
-                    if (r0 + 1 >= ya && r0 + 1 < yb) o[(long long)(r0 + 1) * d.nx] = v.y;
+                    o0[0] = va.x; o0[d.nx] = va.y;
+                    if constexpr (NS > 1) { o1[0] = vb.x; o1[d.nx] = vb.y; }
+                    if constexpr (NS > 2) { o2[0] = vc.x; o2[d.nx] = vc.y; }
+                    if constexpr (NS > 3) { o3[0] = vd.x; o3[d.nx] = vd.y; }
                 }
-            };
-            emit(o0, sa.step(su[0], P.t[0].gy), k - (RA + 1) / 2);
-            if constexpr (NS > 1) emit(o1, sb.step(su[XM_U], P.t[NS > 1 ? 1 : 0].gy), k - (RB + 1) / 2);
-            if constexpr (NS > 2) emit(o2, sc.step(su[2 * XM_U], P.t[NS > 2 ? 2 : 0].gy), k - (RC + 1) / 2);
-            if constexpr (NS > 3) emit(o3, sd.step(su[3 * XM_U], P.t[NS > 3 ? 3 : 0].gy), k - (RD + 1) / 2);
+            } else {
+                auto emit = [&](float *o, float2 v, int m) {
+                    const int r0 = 2 * m;
+                    if (col_ok) {
+                        if (r0 >= ya && r0 < yb) o[0] = v.x;
+                        if (r0 + 1 >= ya && r0 + 1 < yb) o[d.nx] = v.y;
+                    }
+                };
+                emit(o0, va, k - (RA + 1) / 2);
+                if constexpr (NS > 1) emit(o1, vb, k - (RB + 1) / 2);
+                if constexpr (NS > 2) emit(o2, vc, k - (RC + 1) / 2);
+                if constexpr (NS > 3) emit(o3, vd, k - (RD + 1) / 2);
+            }
+            o0 += 2 * d.nx;
+            if constexpr (NS > 1) o1 += 2 * d.nx;
+            if constexpr (NS > 2) o2 += 2 * d.nx;
+            if constexpr (NS > 3) o3 += 2 * d.nx;
         }
         __syncthreads();
     }

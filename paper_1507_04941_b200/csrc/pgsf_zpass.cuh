@@ -26,10 +26,10 @@ struct ZShape {
 // g[o + kTapPad] with kTapPad zeros on both sides.  The walk over the PZ + 2 RZ staged channels is
 // unrolled by template recursion for RZ <= 48 (a `#pragma unroll` of 104 iterations is not honoured), so
 // every tap is a compile-time constant-bank offset and the body is LDS.128 + 16 FFMA2 per channel.
-template <int RZ, int J>
+template <int RZ, int J, int XT>
 __device__ __forceinline__ void z_step(const float *__restrict__ base, const Taps &t, float2 (&acc)[Z_PZ][2])
 {
-    const float4 v = *reinterpret_cast<const float4 *>(base + J * Z_XT);
+    const float4 v = *reinterpret_cast<const float4 *>(base + J * XT);
 #pragma unroll
     for (int p = 0; p < Z_PZ; ++p) {
         const int o = J - p;
@@ -40,24 +40,24 @@ __device__ __forceinline__ void z_step(const float *__restrict__ base, const Tap
     }
 }
 
-template <int RZ, int J0, int N>
+template <int RZ, int J0, int N, int XT>
 __device__ __forceinline__ void z_steps(const float *__restrict__ base, const Taps &t, float2 (&acc)[Z_PZ][2])
 {
     if constexpr (N == 1) {
-        z_step<RZ, J0>(base, t, acc);
+        z_step<RZ, J0, XT>(base, t, acc);
     } else {
-        z_steps<RZ, J0, N / 2>(base, t, acc);
-        z_steps<RZ, J0 + N / 2, N - N / 2>(base, t, acc);
+        z_steps<RZ, J0, N / 2, XT>(base, t, acc);
+        z_steps<RZ, J0 + N / 2, N - N / 2, XT>(base, t, acc);
     }
 }
 
-template <int RZ>
+template <int RZ, int XT = Z_XT>
 __device__ __forceinline__ void z_accumulate(const float *__restrict__ base, const Taps &t, float2 (&acc)[Z_PZ][2])
 {
 #pragma unroll
     for (int p = 0; p < Z_PZ; ++p) acc[p][0] = acc[p][1] = make_float2(0.f, 0.f);
     if constexpr (RZ <= 48) {
-        z_steps<RZ, 0, Z_PZ + 2 * RZ>(base, t, acc);
+        z_steps<RZ, 0, Z_PZ + 2 * RZ, XT>(base, t, acc);
     } else {
         // 150 - 200 channels: walk them in chunks of 8 with the tap index in a uniform register; the zero
         // padding of the tap array makes the ramp-up / ramp-down iterations the same code as the steady state
@@ -66,7 +66,7 @@ __device__ __forceinline__ void z_accumulate(const float *__restrict__ base, con
         for (int jc = 0; jc < Z_PZ + 2 * RZ; jc += 8) {
 #pragma unroll
             for (int jj = 0; jj < 8; ++jj) {
-                const float4 v = *reinterpret_cast<const float4 *>(base + (jc + jj) * Z_XT);
+                const float4 v = *reinterpret_cast<const float4 *>(base + (jc + jj) * XT);
 #pragma unroll
                 for (int p = 0; p < Z_PZ; ++p) {
                     const float g = t.g[jc + jj - p + kTapPad];
@@ -132,13 +132,13 @@ __global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, f
 
 // n steps of the compensated sliding window of one (column, quantity): add the entering channel, write
 // the window sum, subtract the leaving channel.  lead / trail advance by one staged channel per step.
-template <bool SQ>
+template <bool SQ, int XT>
 __device__ __forceinline__ float *window_run(float &s, float &e, const float *__restrict__ lead,
                                              const float *__restrict__ trail, float *__restrict__ zp, long long plane, int n)
 {
 #pragma unroll 8
     for (int j = 0; j < n; ++j) {
-        const float a = lead[j * Z_XT], b = trail[j * Z_XT];
+        const float a = lead[j * XT], b = trail[j * XT];
         kahan_add(s, e, SQ ? a * a : a);
         *zp = s - e;
         zp += plane;
@@ -147,29 +147,35 @@ __device__ __forceinline__ float *window_run(float &s, float &e, const float *__
     return zp;
 }
 
-template <int RZ>
+constexpr int ZM_XT = 64;       // columns per CTA of the marching kernel (16 float4 lanes per channel row)
+
+template <int RZ, int XT>
 struct ZmShape {
-    static constexpr int PLANES = Z_ZB + 2 * RZ;           // t2 slab; its first Z_ZB planes are reused as the f slab
-    static constexpr int SMEM = (PLANES + Z_ZB) * Z_XT * 4; // + slab of the channels leaving the window
+    static constexpr int LX = XT / 4;                       // lanes per channel row
+    static constexpr int GROUPS = Z_ZB / Z_PZ;              // 8 groups of 8 channels per step
+    static constexpr int THREADS = LX * GROUPS;             // = 2 XT: one thread per (column, quantity) in the window phase
+    static constexpr int PLANES = Z_ZB + 2 * RZ;            // t2 slab; its first Z_ZB planes are reused as the f slab
+    static constexpr int SMEM = (PLANES + Z_ZB) * XT * 4;   // + slab of the channels leaving the window
 };
 
-template <int RZ>
-__global__ void __launch_bounds__(Z_THREADS) k_zm(const float *__restrict__ in, float *out, float *__restrict__ Z1,
-                                                  float *__restrict__ Z2, Dims d, int hz, Taps t)
+template <int RZ, int XT>
+__global__ void __launch_bounds__(ZmShape<RZ, XT>::THREADS) k_zm(const float *__restrict__ in, float *out,
+                                                                float *__restrict__ Z1, float *__restrict__ Z2,
+                                                                Dims d, int hz, Taps t)
 {
-    using S = ZmShape<RZ>;
-    extern __shared__ __align__(16) float smem[];  // [PLANES][Z_XT] t2 slab / f slab, [Z_ZB][Z_XT] leaving slab
+    using S = ZmShape<RZ, XT>;
+    extern __shared__ __align__(16) float smem[];  // [PLANES][XT] t2 slab / f slab, [Z_ZB][XT] leaving slab
     float *fs = smem;                              // f of this step (written after the filter phase)
-    float *ts = smem + S::PLANES * Z_XT;           // f of the channels leaving the window in this step
-    const int tid = threadIdx.x, lane = tid & 31, wz = tid >> 5;
-    const int x0 = blockIdx.x * Z_XT, y = blockIdx.y;
-    const int gx = x0 + 4 * lane;
+    float *ts = smem + S::PLANES * XT;             // f of the channels leaving the window in this step
+    const int tid = threadIdx.x, lx = tid % S::LX, wz = tid / S::LX;
+    const int x0 = blockIdx.x * XT, y = blockIdx.y;
+    const int gx = x0 + 4 * lx;
     const bool col_ok = gx < d.nx;
     const float *col_in = in + (long long)y * d.nx + (col_ok ? gx : 0);
     float *col_out = out + (long long)y * d.nx + (col_ok ? gx : 0);
     // window phase: one thread per (column, quantity)
-    const int c = tid & (Z_XT - 1);
-    const bool sq = tid >= Z_XT;
+    const int c = tid % XT;
+    const bool sq = tid >= XT;
     const bool c_ok = x0 + c < d.nx;
     const long long cb = (long long)y * d.nx + x0 + c;
     float *Zq = sq ? Z2 : Z1;
@@ -182,30 +188,30 @@ __global__ void __launch_bounds__(Z_THREADS) k_zm(const float *__restrict__ in, 
         // channels leaving the window in this step: z0 - 2 hz + j, j = 0..63.  Those written in EARLIER steps
         // (by this CTA: still in L2) are fetched now, together with the t2 slab; those of this step's own
         // f block (2 hz < 64) are read from the f slab instead.
-        for (int pz = wz; pz < Z_ZB; pz += Z_WARPS) {
+        for (int pz = wz; pz < Z_ZB; pz += S::GROUPS) {
             const int zt = z0 - 2 * hz + pz;
             const bool ok = col_ok && zt >= 0 && zt < z0;
-            cp_async16(ts + pz * Z_XT + 4 * lane, ok ? col_out + (long long)zt * d.plane : in, ok);
+            cp_async16(ts + pz * XT + 4 * lx, ok ? col_out + (long long)zt * d.plane : in, ok);
         }
         if (z0 < nz) {
             // stage channels z0-RZ .. z0+ZB+RZ-1 of t2; outside the cube -> 0 (C-5)
-            for (int pz = wz; pz < S::PLANES; pz += Z_WARPS) {
+            for (int pz = wz; pz < S::PLANES; pz += S::GROUPS) {
                 const int gz = z0 - RZ + pz;
                 const bool ok = col_ok && gz >= 0 && gz < nz;
-                cp_async16(smem + pz * Z_XT + 4 * lane, ok ? col_in + (long long)gz * d.plane : in, ok);
+                cp_async16(smem + pz * XT + 4 * lx, ok ? col_in + (long long)gz * d.plane : in, ok);
             }
         }
         cp_async_wait_all();
         __syncthreads();
         if (z0 < nz) {
             float2 acc[Z_PZ][2];
-            z_accumulate<RZ>(smem + (wz * Z_PZ) * Z_XT + 4 * lane, t, acc);
+            z_accumulate<RZ, XT>(smem + (wz * Z_PZ) * XT + 4 * lx, t, acc);
             __syncthreads();   // every warp is done with the t2 slab: its head becomes the f slab
 #pragma unroll
             for (int p = 0; p < Z_PZ; ++p) {
                 const int gz = z0 + wz * Z_PZ + p;
                 const float4 v = make_float4(acc[p][0].x, acc[p][0].y, acc[p][1].x, acc[p][1].y);
-                *reinterpret_cast<float4 *>(fs + (wz * Z_PZ + p) * Z_XT + 4 * lane) = v;
+                *reinterpret_cast<float4 *>(fs + (wz * Z_PZ + p) * XT + 4 * lx) = v;
                 if (col_ok && gz < nz) *reinterpret_cast<float4 *>(col_out + (long long)gz * d.plane) = v;
             }
             __syncthreads();   // f slab complete
@@ -216,24 +222,24 @@ __global__ void __launch_bounds__(Z_THREADS) k_zm(const float *__restrict__ in, 
                 const int jsplit = min(2 * hz, Z_ZB);   // leaving channel: ts[j] for j < jsplit, else fs[j - 2 hz]
                 float *zp = Zq + (long long)(z0 - hz) * d.plane + cb;
                 if (sq) {
-                    zp = window_run<true>(s, e, fs + c, ts + c, zp, d.plane, jsplit);
-                    window_run<true>(s, e, fs + jsplit * Z_XT + c, fs + c, zp, d.plane, Z_ZB - jsplit);
+                    zp = window_run<true, XT>(s, e, fs + c, ts + c, zp, d.plane, jsplit);
+                    window_run<true, XT>(s, e, fs + jsplit * XT + c, fs + c, zp, d.plane, Z_ZB - jsplit);
                 } else {
-                    zp = window_run<false>(s, e, fs + c, ts + c, zp, d.plane, jsplit);
-                    window_run<false>(s, e, fs + jsplit * Z_XT + c, fs + c, zp, d.plane, Z_ZB - jsplit);
+                    zp = window_run<false, XT>(s, e, fs + c, ts + c, zp, d.plane, jsplit);
+                    window_run<false, XT>(s, e, fs + jsplit * XT + c, fs + c, zp, d.plane, Z_ZB - jsplit);
                 }
             } else {
                 for (int j = 0; j < Z_ZB; ++j) {
                     const int zl = z0 + j;          // channel entering the window of output zo
                     const int zo = zl - hz;
                     if (zl < nz) {
-                        const float v = fs[j * Z_XT + c];
+                        const float v = fs[j * XT + c];
                         kahan_add(s, e, sq ? v * v : v);
                     }
                     if (zo >= 0 && zo < nz) {
                         Zq[(long long)zo * d.plane + cb] = s - e;
                         const int jt = j - 2 * hz;  // the channel leaving after this output, relative to z0
-                        const float v = jt >= 0 ? fs[jt * Z_XT + c] : ts[j * Z_XT + c];   // (zero where zt < 0)
+                        const float v = jt >= 0 ? fs[jt * XT + c] : ts[j * XT + c];   // (zero where zt < 0)
                         kahan_add(s, e, sq ? -(v * v) : -v);
                     }
                 }
@@ -241,22 +247,6 @@ __global__ void __launch_bounds__(Z_THREADS) k_zm(const float *__restrict__ in, 
         }
         __syncthreads();   // slabs are overwritten by the next step
     }
-}
-
-template <int RZ>
-cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t,
-                      cudaStream_t st)
-{
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_zm<RZ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             ZmShape<RZ>::SMEM);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
-    dim3 grid((d.nx + Z_XT - 1) / Z_XT, d.ny);
-    k_zm<RZ><<<grid, Z_THREADS, ZmShape<RZ>::SMEM, st>>>(in, out, Z1, Z2, d, hz, t);
-    return cudaGetLastError();
 }
 
 template <int RZ>
@@ -274,6 +264,21 @@ cudaError_t launch_z(const float *in, float *out, const Dims &d, const Taps &t, 
     return cudaGetLastError();
 }
 
+template <int RZ>
+cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t,
+                      cudaStream_t st)
+{
+    using S = ZmShape<RZ, ZM_XT>;
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_zm<RZ, ZM_XT>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dim3 grid((d.nx + ZM_XT - 1) / ZM_XT, d.ny);
+    k_zm<RZ, ZM_XT><<<grid, S::THREADS, S::SMEM, st>>>(in, out, Z1, Z2, d, hz, t);
+    return cudaGetLastError();
+}
 
 }  // namespace
 }  // namespace pgsf
