@@ -191,6 +191,28 @@ def run_reference(args, w):
 
 # ------------------------------------------------------------------------------------ B200 arm
 
+def replica_workload(w, rank: int):
+    """Replicas only: rank r runs its own copy of the workload, seed offset by 100 r."""
+    from dataclasses import replace
+    return replace(w, seed=w.seed + 100 * rank) if rank else w
+
+
+def max_over_ranks(ms: float, world: int, device) -> float:
+    """Step time of the job = the slowest rank's (all-reduce MAX over the process group)."""
+    if world <= 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(n_vox: int, n_scales: int, world: int, ms_step: float) -> float:
+    """Whole-job G voxel-scales/s: every rank processed n_vox x n_scales in ms_step."""
+    return n_vox * n_scales * world / (ms_step * 1e-3) / 1e9
+
+
 def _kernel_work(name: str, w, taps, n_vox: int):
     """Algorithmic (flops, bytes) of ONE launch of the kernel `name`: the work
     the separable method must do, not what the implementation happens to move."""
@@ -240,9 +262,7 @@ def run_b200(args, w):
     peaks = _peaks()
 
     # every rank runs its own replica of the workload (seed offset by rank)
-    from dataclasses import replace
-    wr = replace(w, seed=w.seed + 100 * rank) if rank else w
-    d = synth.make_workload(wr, dev)
+    d = synth.make_workload(replica_workload(w, rank), dev)
     n_vox = w.voxels
     S = len(w.sigmas)
     taps = _taps(w)
@@ -280,12 +300,9 @@ def run_b200(args, w):
     plan.pgsf_plan_set_profiling(False)
     clocks = sampler.stop()
     count = int(cnt.item())
-    if world > 1:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, world, dev)
     ms_step = ms_total / args.steps
-    value = n_vox * S * world / (ms_step * 1e-3) / 1e9
+    value = aggregate_value(n_vox, S, world, ms_step)
 
     # ---- roofline of the dominant kernel + of the whole path
     alu_peak = _alu_peak_tflops(props.multi_processor_count, peaks["sm_max_mhz"])
@@ -363,10 +380,7 @@ def run_e2e(args, w, ctx):
         _, count = plan.pgsf_find_multiscale_host(h_in, h_mask)   # synchronises before returning
     torch.cuda.synchronize()
     sec = (time.perf_counter() - t0) / steps
-    if world > 1:
-        t = torch.tensor([sec], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        sec = float(t.item())
+    sec = max_over_ranks(sec, world, dev)
     assert count == expect, f"host entry point count {count} != device path count {expect}"
     return {"value": w.voxels * S * world / sec / 1e9, "unit": UNIT, "ms_per_step": sec * 1e3, "steps": steps,
             "h2d_bytes_per_step": w.voxels * 4, "d2h_bytes_per_step": w.voxels + 8,

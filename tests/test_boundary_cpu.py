@@ -155,3 +155,45 @@ def test_synth_is_seeded_and_config_shaped():
     c = synth.make_workload(w4, "cpu")
     assert c.shape == (3, 32, 24, 24) and not torch.equal(c[0], c[1])
     assert synth.WORKLOADS[5].sigmas[-1] == (3.0, 3.0, 32.0) and synth.WORKLOADS[2].voxels == 2 ** 28
+
+
+# ---------------------------------------------------------------------------------- N > 1: replicas only
+
+def _replica_worker(rank, world, port, out):
+    import os
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    from paper_1507_04941_b200 import synth
+    w = bench.replica_workload(synth.WORKLOADS[1], rank)
+    ms = bench.max_over_ranks(10.0 + 5.0 * rank, world, "cpu")       # rank 1 is the slow one
+    out.put((rank, w.seed, ms, bench.aggregate_value(w.voxels, len(w.sigmas), world, ms)))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_replicas_world_size_2_gloo():
+    """bench.py --gpus N runs N independent replicas: seeds differ per rank, the step
+    time is the max over ranks, the value is the whole-job aggregate.  No data-path collective exists."""
+    import socket
+    import torch.multiprocessing as mp
+    from paper_1507_04941_b200 import synth
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_replica_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    w = synth.WORKLOADS[1]
+    assert [r[1] for r in res] == [w.seed, w.seed + 100]
+    assert all(abs(r[2] - 15.0) < 1e-12 for r in res)                # max over ranks on every rank
+    expect = w.voxels * len(w.sigmas) * 2 / 15e-3 / 1e9
+    assert all(abs(r[3] - expect) < 1e-9 * expect for r in res)
