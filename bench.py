@@ -40,6 +40,20 @@ def _peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback (B200_PROFILING.md)"}
 
 
+def _dram_traffic(workload: str, kernel: str):
+    """DRAM bytes per launch of `kernel` from the committed ncu capture (profiles/r01_dram_traffic.csv),
+    or None when no capture exists for this workload / kernel."""
+    path = os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    import csv
+    with open(path) as fh:
+        for row in csv.DictReader(fh):
+            if row["workload"] == workload and row["kernel"] == kernel:
+                return float(row["dram_bytes_per_launch"])
+    return None
+
+
 def _alu_peak_tflops(sm_count: int, sm_mhz: float) -> float:
     """FP32 CUDA-core peak: SMs x 128 lanes x 2 flop x clock."""
     return sm_count * FP32_LANES_PER_SM * 2 * sm_mhz * 1e6 / 1e12
@@ -326,7 +340,7 @@ def run_b200(args, w):
             ach = k0["bytes"] / sec / 1e9
             roofline = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak}
         roofline.update({"kernel": k0["name"], "ms_per_launch": k0["ms_per_launch"], "share_of_step": k0["share"],
-                         "traffic": None, "peak_source": ("148 SM x 128 lanes x 2 x sm_max_mhz" if t_alu >= t_hbm
+                         "traffic": _dram_traffic(w.name, k0["name"]), "peak_source": ("148 SM x 128 lanes x 2 x sm_max_mhz" if t_alu >= t_hbm
                                                           else peaks["source"])})
     path_flops = sum(2 * sum(t) + STATS_FLOPS for t in taps) * n_vox
     path_bytes = (4 + 4 * S + 1) * n_vox
