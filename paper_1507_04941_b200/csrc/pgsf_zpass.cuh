@@ -51,12 +51,12 @@ __device__ __forceinline__ void z_steps(const float *__restrict__ base, const Ta
     }
 }
 
-template <int RZ, int XT = Z_XT>
+template <int RZ, int XT = Z_XT, bool FULL = (RZ <= 48)>
 __device__ __forceinline__ void z_accumulate(const float *__restrict__ base, const Taps &t, float2 (&acc)[Z_PZ][2])
 {
 #pragma unroll
     for (int p = 0; p < Z_PZ; ++p) acc[p][0] = acc[p][1] = make_float2(0.f, 0.f);
-    if constexpr (RZ <= 48) {
+    if constexpr (FULL) {
         z_steps<RZ, 0, Z_PZ + 2 * RZ, XT>(base, t, acc);
     } else {
         // 150 - 200 channels: walk them in chunks of 8 with the tap index in a uniform register; the zero
@@ -149,22 +149,22 @@ __device__ __forceinline__ float *window_run(float &s, float &e, const float *__
 
 constexpr int ZM_XT = 64;       // columns per CTA of the marching kernel (16 float4 lanes per channel row)
 
-template <int RZ, int XT>
+template <int RZ, int XT, int ZB>
 struct ZmShape {
     static constexpr int LX = XT / 4;                       // lanes per channel row
-    static constexpr int GROUPS = Z_ZB / Z_PZ;              // 8 groups of 8 channels per step
-    static constexpr int THREADS = LX * GROUPS;             // = 2 XT: one thread per (column, quantity) in the window phase
-    static constexpr int PLANES = Z_ZB + 2 * RZ;            // t2 slab; its first Z_ZB planes are reused as the f slab
-    static constexpr int SMEM = (PLANES + Z_ZB) * XT * 4;   // + slab of the channels leaving the window
+    static constexpr int GROUPS = ZB / Z_PZ;                // groups of 8 channels per step
+    static constexpr int THREADS = LX * GROUPS;             // >= 2 XT; the first 2 XT threads run the window phase
+    static constexpr int PLANES = ZB + 2 * RZ;            // t2 slab; its first ZB planes are reused as the f slab
+    static constexpr int SMEM = (PLANES + ZB) * XT * 4;   // + slab of the channels leaving the window
 };
 
-template <int RZ, int XT>
-__global__ void __launch_bounds__(ZmShape<RZ, XT>::THREADS) k_zm(const float *__restrict__ in, float *out,
+template <int RZ, int XT, int ZB>
+__global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float *__restrict__ in, float *out,
                                                                 float *__restrict__ Z1, float *__restrict__ Z2,
                                                                 Dims d, int hz, Taps t)
 {
-    using S = ZmShape<RZ, XT>;
-    extern __shared__ __align__(16) float smem[];  // [PLANES][XT] t2 slab / f slab, [Z_ZB][XT] leaving slab
+    using S = ZmShape<RZ, XT, ZB>;
+    extern __shared__ __align__(16) float smem[];  // [PLANES][XT] t2 slab / f slab, [ZB][XT] leaving slab
     float *fs = smem;                              // f of this step (written after the filter phase)
     float *ts = smem + S::PLANES * XT;             // f of the channels leaving the window in this step
     const int tid = threadIdx.x, lx = tid % S::LX, wz = tid / S::LX;
@@ -176,19 +176,19 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT>::THREADS) k_zm(const float *__
     // window phase: one thread per (column, quantity)
     const int c = tid % XT;
     const bool sq = tid >= XT;
-    const bool c_ok = x0 + c < d.nx;
+    const bool c_ok = x0 + c < d.nx && tid < 2 * XT;
     const long long cb = (long long)y * d.nx + x0 + c;
     float *Zq = sq ? Z2 : Z1;
     float s = 0.f, e = 0.f;
     const int nz = d.nz;
-    const int nsteps = (nz + hz + Z_ZB - 1) / Z_ZB;   // entering channels 0 .. nz + hz - 1 (the tail drains the window)
+    const int nsteps = (nz + hz + ZB - 1) / ZB;   // entering channels 0 .. nz + hz - 1 (the tail drains the window)
 
     for (int k = 0; k < nsteps; ++k) {
-        const int z0 = k * Z_ZB;
+        const int z0 = k * ZB;
         // channels leaving the window in this step: z0 - 2 hz + j, j = 0..63.  Those written in EARLIER steps
         // (by this CTA: still in L2) are fetched now, together with the t2 slab; those of this step's own
         // f block (2 hz < 64) are read from the f slab instead.
-        for (int pz = wz; pz < Z_ZB; pz += S::GROUPS) {
+        for (int pz = wz; pz < ZB; pz += S::GROUPS) {
             const int zt = z0 - 2 * hz + pz;
             const bool ok = col_ok && zt >= 0 && zt < z0;
             cp_async16(ts + pz * XT + 4 * lx, ok ? col_out + (long long)zt * d.plane : in, ok);
@@ -205,7 +205,7 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT>::THREADS) k_zm(const float *__
         __syncthreads();
         if (z0 < nz) {
             float2 acc[Z_PZ][2];
-            z_accumulate<RZ, XT>(smem + (wz * Z_PZ) * XT + 4 * lx, t, acc);
+            z_accumulate<RZ, XT, true>(smem + (wz * Z_PZ) * XT + 4 * lx, t, acc);
             __syncthreads();   // every warp is done with the t2 slab: its head becomes the f slab
 #pragma unroll
             for (int p = 0; p < Z_PZ; ++p) {
@@ -217,19 +217,19 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT>::THREADS) k_zm(const float *__
             __syncthreads();   // f slab complete
         }
         if (c_ok) {
-            if (z0 >= hz && z0 + Z_ZB <= nz) {
+            if (z0 >= hz && z0 + ZB <= nz) {
                 // interior step: all 64 entering channels and all 64 outputs are inside the cube
-                const int jsplit = min(2 * hz, Z_ZB);   // leaving channel: ts[j] for j < jsplit, else fs[j - 2 hz]
+                const int jsplit = min(2 * hz, ZB);   // leaving channel: ts[j] for j < jsplit, else fs[j - 2 hz]
                 float *zp = Zq + (long long)(z0 - hz) * d.plane + cb;
                 if (sq) {
                     zp = window_run<true, XT>(s, e, fs + c, ts + c, zp, d.plane, jsplit);
-                    window_run<true, XT>(s, e, fs + jsplit * XT + c, fs + c, zp, d.plane, Z_ZB - jsplit);
+                    window_run<true, XT>(s, e, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit);
                 } else {
                     zp = window_run<false, XT>(s, e, fs + c, ts + c, zp, d.plane, jsplit);
-                    window_run<false, XT>(s, e, fs + jsplit * XT + c, fs + c, zp, d.plane, Z_ZB - jsplit);
+                    window_run<false, XT>(s, e, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit);
                 }
             } else {
-                for (int j = 0; j < Z_ZB; ++j) {
+                for (int j = 0; j < ZB; ++j) {
                     const int zl = z0 + j;          // channel entering the window of output zo
                     const int zo = zl - hz;
                     if (zl < nz) {
@@ -264,19 +264,25 @@ cudaError_t launch_z(const float *in, float *out, const Dims &d, const Taps &t, 
     return cudaGetLastError();
 }
 
+// channels per march step: 64 (4 warps per CTA) up to RZ = 48; 128 (8 warps) above, where the slab of
+// 64 + 2 RZ channels would leave room for two 4-warp CTAs only
+template <int RZ>
+constexpr int zm_step_channels() { return RZ >= 96 ? 128 : 64; }
+
 template <int RZ>
 cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t,
                       cudaStream_t st)
 {
-    using S = ZmShape<RZ, ZM_XT>;
+    constexpr int ZB = zm_step_channels<RZ>();
+    using S = ZmShape<RZ, ZM_XT, ZB>;
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_zm<RZ, ZM_XT>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM);
+        cudaError_t e = cudaFuncSetAttribute(k_zm<RZ, ZM_XT, ZB>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM);
         if (e != cudaSuccess) return e;
         configured = true;
     }
     dim3 grid((d.nx + ZM_XT - 1) / ZM_XT, d.ny);
-    k_zm<RZ, ZM_XT><<<grid, S::THREADS, S::SMEM, st>>>(in, out, Z1, Z2, d, hz, t);
+    k_zm<RZ, ZM_XT, ZB><<<grid, S::THREADS, S::SMEM, st>>>(in, out, Z1, Z2, d, hz, t);
     return cudaGetLastError();
 }
 
