@@ -322,8 +322,13 @@ def run_b200(args, w):
     alu_peak = _alu_peak_tflops(props.multi_processor_count, peaks["sm_max_mhz"])
     hbm_peak = peaks["hbm_gbs"]
     kern = []
+    cube = w.dims[0] * w.dims[1] * w.dims[2]
     for name, (n, ms) in prof.items():
-        fl, by = _kernel_work(name, w, taps, w.dims[0] * w.dims[1] * w.dims[2])
+        # voxels per launch: a batch goes through in groups of cubes; a name shared by all scales
+        # (stats_*) is launched once per scale and group
+        per_step = S if name.startswith("stats_") else 1
+        vox_launch = cube * w.batch * per_step * args.steps / max(n, 1)
+        fl, by = _kernel_work(name, w, taps, vox_launch)
         kern.append({"name": name, "launches": n, "ms_per_launch": ms / max(n, 1), "share": ms / max(ms_total, 1e-9),
                      "flops": fl, "bytes": by})
     kern.sort(key=lambda k: -k["share"])

@@ -190,7 +190,16 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
 
     // workspace: [scratch filtered cube][filter temporaries][statistics temporaries]
     p->ws_cube_bytes = round256((size_t)p->dims.cube * sizeof(float));
-    const size_t cubes = 1 + (p->fast_filter ? 1 : 2) + (p->fast_stats ? 2 : 4);
+    // Batches: the fast path of pgsf_find_multiscale runs `group` cubes per launch (the kernels of one
+    // 60-M-voxel sub-cube do not fill the machine), bounded by 2^32 voxels and by grid.z <= 65535 planes.
+    p->group = 1;
+    if (p->fast_filter && p->fast_stats && desc->batch > 1) {
+        long long g = (1LL << 32) / p->dims.cube;
+        if (g > 65535 / desc->nz) g = 65535 / desc->nz;
+        if (g > desc->batch) g = desc->batch;
+        p->group = g < 1 ? 1 : (int)g;
+    }
+    const size_t cubes = 1 + (p->fast_filter ? (size_t)p->group : 2) + (p->fast_stats ? 2 * (size_t)p->group : 4);
     p->ws_bytes = cubes * p->ws_cube_bytes;
     *out = p;
     return PGSF_OK;
@@ -288,7 +297,7 @@ Workspace carve(const pgsf_plan *p, void *ws)
     char *b = static_cast<char *>(ws);
     w.scratch = reinterpret_cast<float *>(b);
     w.ftmp = reinterpret_cast<float *>(b + p->ws_cube_bytes);
-    w.stmp = reinterpret_cast<float *>(b + p->ws_cube_bytes * (1 + (p->fast_filter ? 1 : 2)));
+    w.stmp = reinterpret_cast<float *>(b + p->ws_cube_bytes * (1 + (p->fast_filter ? (size_t)p->group : 2)));
     return w;
 }
 
@@ -407,23 +416,26 @@ pgsf_status pgsf_find_multiscale(pgsf_plan *p, const float *d_in, float *const *
     if (p->fast_filter && all_kept) {
         // x and y passes of all scales from ONE read of the input; the x/y-filtered cube of scale s
         // is parked in the output cube of scale s+1 (the last one in the workspace), so the z passes
-        // run in order s = 0..S-1, each freeing the cube the next one writes to
+        // run in order s = 0..S-1, each freeing the cube the next one writes to.  Batches go through in
+        // groups of p->group cubes per launch.
         int idx[PGSF_MAX_SCALES];
         for (int s = 0; s < S; ++s) idx[s] = s;
-        for (int bi = 0; bi < B; ++bi) {
-            const size_t off = (size_t)bi * p->dims.cube;
+        const int G = p->fast_stats ? p->group : 1;
+        for (int b0 = 0; b0 < B; b0 += G) {
+            const int nb = B - b0 < G ? B - b0 : G;
+            const size_t off = (size_t)b0 * p->dims.cube;
             float *park[PGSF_MAX_SCALES];
             for (int s = 0; s < S; ++s) park[s] = (s + 1 < S) ? d_filtered[s + 1] + off : w.ftmp;
-            cudaError_t ce = pgsf::fast_xy_multi(p, idx, S, d_in + off, park, st);
+            cudaError_t ce = pgsf::fast_xy_multi(p, idx, S, d_in + off, park, nb, st);
             if (ce != cudaSuccess) return cuda_fail(p, ce, "xy filter launch");
             for (int s = 0; s < S; ++s) {
                 if (p->fast_stats) {
                     // frequency pass and z-direction window sums in one march; then the x/y window sums
-                    float *Z1 = w.stmp, *Z2 = w.stmp + p->dims.cube;
-                    ce = pgsf::fast_zm(p, s, park[s], d_filtered[s] + off, Z1, Z2, st);
+                    float *Z1 = w.stmp, *Z2 = w.stmp + (size_t)p->group * p->dims.cube;
+                    ce = pgsf::fast_zm(p, s, park[s], d_filtered[s] + off, Z1, Z2, nb, st);
                     if (ce != cudaSuccess) return cuda_fail(p, ce, "z filter + window launch");
                     ce = pgsf::fast_threshold_xy(p, d_filtered[s] + off, Z1, Z2, d_mask + off, s > 0, nullptr,
-                                                 nullptr, (s == S - 1) ? d_count : nullptr, st);
+                                                 nullptr, (s == S - 1) ? d_count : nullptr, nb, st);
                     if (ce != cudaSuccess) return cuda_fail(p, ce, "threshold launch");
                     continue;
                 }

@@ -22,17 +22,17 @@
 namespace pgsf {
 // per-radius entry points of the frequency-axis kernels (pgsf_z_r*.cu)
 cudaError_t launch_z_r6(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r6(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, cudaStream_t st);
+cudaError_t launch_zm_r6(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
 cudaError_t launch_z_r12(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r12(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, cudaStream_t st);
+cudaError_t launch_zm_r12(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
 cudaError_t launch_z_r24(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r24(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, cudaStream_t st);
+cudaError_t launch_zm_r24(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
 cudaError_t launch_z_r48(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r48(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, cudaStream_t st);
+cudaError_t launch_zm_r48(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
 cudaError_t launch_z_r72(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r72(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, cudaStream_t st);
+cudaError_t launch_zm_r72(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
 cudaError_t launch_z_r96(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r96(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, cudaStream_t st);
+cudaError_t launch_zm_r96(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
 
 namespace {
 
@@ -332,10 +332,13 @@ static bool xym_dispatch(int n, const int *rc, const float *in, const XymParams 
 // x and y passes of the scales `scales[0..n)` of one cube: in -> out[i] (x/y-filtered cubes).  The
 // scales are sorted by compiled radius and cut into the largest groups a k_xym instance exists for;
 // every group reads the input once.
-cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *in, float *const *out,
+cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *in, float *const *out, int ncubes,
                           cudaStream_t st)
 {
-    const Dims &d = p->dims;
+    // the x and y passes do not couple planes: `ncubes` consecutive cubes are one stack of ncubes * nz planes
+    Dims d = p->dims;
+    d.nz *= ncubes;
+    d.cube *= ncubes;
     if (d.nz > 65535 || n < 1 || n > PGSF_MAX_SCALES) return cudaErrorInvalidConfiguration;
     int order[PGSF_MAX_SCALES];
     for (int i = 0; i < n; ++i) order[i] = i;
@@ -408,22 +411,23 @@ cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStr
 
 // frequency pass of one scale fused with the z-direction window sums of the statistics:
 // in (x/y-filtered cube) -> out (filtered cube), Z1, Z2
-cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, cudaStream_t st)
+cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, int ncubes,
+                    cudaStream_t st)
 {
     const Dims &d = p->dims;
     const ScalePlan &sp = p->scales[scale];
-    if (d.ny > 65535) return cudaErrorInvalidConfiguration;
+    if (d.ny > 65535 || ncubes < 1 || ncubes > 65535) return cudaErrorInvalidConfiguration;
     const int hz = p->desc.box_half[2];
     char name[32];
     snprintf(name, sizeof name, "zm_s%d", scale);
     LaunchScope ls(p, name, st);
     switch (sp.rz_c) {
-    case 6: return launch_zm_r6(in, out, Z1, Z2, d, hz, sp.tz, st);
-    case 12: return launch_zm_r12(in, out, Z1, Z2, d, hz, sp.tz, st);
-    case 24: return launch_zm_r24(in, out, Z1, Z2, d, hz, sp.tz, st);
-    case 48: return launch_zm_r48(in, out, Z1, Z2, d, hz, sp.tz, st);
-    case 72: return launch_zm_r72(in, out, Z1, Z2, d, hz, sp.tz, st);
-    case 96: return launch_zm_r96(in, out, Z1, Z2, d, hz, sp.tz, st);
+    case 6: return launch_zm_r6(in, out, Z1, Z2, d, hz, sp.tz, ncubes, st);
+    case 12: return launch_zm_r12(in, out, Z1, Z2, d, hz, sp.tz, ncubes, st);
+    case 24: return launch_zm_r24(in, out, Z1, Z2, d, hz, sp.tz, ncubes, st);
+    case 48: return launch_zm_r48(in, out, Z1, Z2, d, hz, sp.tz, ncubes, st);
+    case 72: return launch_zm_r72(in, out, Z1, Z2, d, hz, sp.tz, ncubes, st);
+    case 96: return launch_zm_r96(in, out, Z1, Z2, d, hz, sp.tz, ncubes, st);
     default: return cudaErrorNotSupported;
     }
 }
@@ -432,7 +436,7 @@ cudaError_t fast_filter3d(pgsf_plan *p, int scale, const float *in, float *out, 
                           cudaStream_t st)
 {
     float *outs[1] = {tmp};
-    cudaError_t e = fast_xy_multi(p, &scale, 1, in, outs, st);
+    cudaError_t e = fast_xy_multi(p, &scale, 1, in, outs, 1, st);
     if (e != cudaSuccess) return e;
     return fast_z(p, scale, tmp, out, st);
 }

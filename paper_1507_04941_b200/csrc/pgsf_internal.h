@@ -74,6 +74,7 @@ struct pgsf_plan {
     bool fast_stats;
     size_t ws_bytes;     // total workspace
     size_t ws_cube_bytes;
+    int group;           // cubes of a batch that the fast path of pgsf_find_multiscale processes per launch
     unsigned long long launches;
     std::string err;
     bool prof_on;
@@ -112,14 +113,17 @@ bool fast_xy_radius(int r, int *compiled);
 bool fast_z_radius(int r, int *compiled);
 cudaError_t fast_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp,
                           cudaStream_t st);
-cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *in, float *const *out,
+// `ncubes` consecutive cubes (stride dims.cube) per call, for the entry points that take it
+cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *in, float *const *out, int ncubes,
                           cudaStream_t st);
 cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStream_t st);
-cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, cudaStream_t st);
+cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, int ncubes,
+                    cudaStream_t st);
 bool fast_stats_supported(const pgsf_plan *p);
 // x/y window sums + selection from precomputed z-direction window sums Z1, Z2 (of fast_zm / k_zbox)
 cudaError_t fast_threshold_xy(pgsf_plan *p, const float *f, const float *Z1, const float *Z2, uint8_t *mask,
-                              int or_into, float *mean, float *sd, unsigned long long *count, cudaStream_t st);
+                              int or_into, float *mean, float *sd, unsigned long long *count, int ncubes,
+                              cudaStream_t st);
 // tmp2: 2 cubes (the z-direction window sums of f and f^2)
 cudaError_t fast_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean,
                            float *sd, unsigned long long *count, float *tmp2, cudaStream_t st);

@@ -197,13 +197,14 @@ __global__ void __launch_bounds__(YM_MAX_NT) k_ymarch(const float *__restrict__ 
         b[e < 2 ? e : NT + e] = z;
     }
     const Dims &d = p.d;
-    const int z = blockIdx.z;
+    const int zz = blockIdx.z;                         // plane of the stack of cubes
+    const int z = zz % d.nz;                           // channel inside its cube
     const int out_lo = (p.ntiles == 1) ? 0 : blockIdx.x * p.wo;
     const int out_hi = (p.ntiles == 1) ? d.nx : min(d.nx, out_lo + p.wo);
     const int xs = (p.ntiles == 1) ? 0 : out_lo - HX;
     const int c0 = xs + G * tid;                       // first of this thread's G columns
     const bool col_ok = c0 >= 0 && c0 + G <= d.nx;     // (extents are multiples of the vector width)
-    const long long col_off = (long long)z * d.plane + (col_ok ? c0 : 0);
+    const long long col_off = (long long)zz * d.plane + (col_ok ? c0 : 0);
     const int ya = blockIdx.y * p.ychunk, yb = min(ya + p.ychunk, d.ny);
     const bool is_out = col_ok && c0 >= out_lo && c0 < out_hi;
 
@@ -367,7 +368,7 @@ __global__ void __launch_bounds__(YM_MAX_NT) k_ymarch(const float *__restrict__ 
 
 template <int G>
 cudaError_t launch_ymarch(const pgsf_plan *pl, const float *f, const float *Z1, const float *Z2, uint8_t *mask,
-                          float *mean, float *sd, unsigned long long *count, YmParams p, cudaStream_t st)
+                          float *mean, float *sd, unsigned long long *count, YmParams p, int ncubes, cudaStream_t st)
 {
     constexpr int VL = VecT<G>::L;
     const Dims &d = p.d;
@@ -383,7 +384,7 @@ cudaError_t launch_ymarch(const pgsf_plan *pl, const float *f, const float *Z1, 
     }
     // y chunks: enough CTAs for a few waves; a chunk start re-reads 2 hy rows
     const long long resident = (long long)pl->sm_count * (nt <= 128 ? 4 : 2);
-    const long long base = (long long)p.ntiles * d.nz;
+    const long long base = (long long)p.ntiles * d.nz * ncubes;
     int nch = (int)((4 * resident + base - 1) / base);
     const int min_rows = 8 * p.hy > 64 ? 8 * p.hy : 64;
     if (nch > (d.ny + min_rows - 1) / min_rows) nch = (d.ny + min_rows - 1) / min_rows;
@@ -397,7 +398,8 @@ cudaError_t launch_ymarch(const pgsf_plan *pl, const float *f, const float *Z1, 
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    dim3 grid(p.ntiles, nch, d.nz);
+    if ((long long)d.nz * ncubes > 65535) return cudaErrorInvalidConfiguration;
+    dim3 grid(p.ntiles, nch, d.nz * ncubes);
     k_ymarch<G><<<grid, nt, smem, st>>>(f, Z1, Z2, mask, mean, sd, count, p);
     return cudaGetLastError();
 }
@@ -440,11 +442,12 @@ cudaError_t fast_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_i
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
-    return fast_threshold_xy(p, f, Z1, Z2, mask, or_into, mean, sd, count, st);
+    return fast_threshold_xy(p, f, Z1, Z2, mask, or_into, mean, sd, count, 1, st);
 }
 
 cudaError_t fast_threshold_xy(pgsf_plan *p, const float *f, const float *Z1, const float *Z2, uint8_t *mask,
-                              int or_into, float *mean, float *sd, unsigned long long *count, cudaStream_t st)
+                              int or_into, float *mean, float *sd, unsigned long long *count, int ncubes,
+                              cudaStream_t st)
 {
     const Dims &d = p->dims;
     YmParams yp;
@@ -459,9 +462,9 @@ cudaError_t fast_threshold_xy(pgsf_plan *p, const float *f, const float *Z1, con
     yp.wo = yp.ntiles = yp.ychunk = 0;
     LaunchScope ls(p, "stats_xybox", st);
     switch (p->desc.box_half[0]) {
-    case 4: return launch_ymarch<2>(p, f, Z1, Z2, mask, mean, sd, count, yp, st);
-    case 8: return launch_ymarch<4>(p, f, Z1, Z2, mask, mean, sd, count, yp, st);
-    case 16: return launch_ymarch<8>(p, f, Z1, Z2, mask, mean, sd, count, yp, st);
+    case 4: return launch_ymarch<2>(p, f, Z1, Z2, mask, mean, sd, count, yp, ncubes, st);
+    case 8: return launch_ymarch<4>(p, f, Z1, Z2, mask, mean, sd, count, yp, ncubes, st);
+    case 16: return launch_ymarch<8>(p, f, Z1, Z2, mask, mean, sd, count, yp, ncubes, st);
     default: return cudaErrorNotSupported;
     }
 }

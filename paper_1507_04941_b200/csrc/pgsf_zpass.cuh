@@ -169,6 +169,10 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
     float *ts = smem + S::PLANES * XT;             // f of the channels leaving the window in this step
     const int tid = threadIdx.x, lx = tid % S::LX, wz = tid / S::LX;
     const int x0 = blockIdx.x * XT, y = blockIdx.y;
+    {   // one cube of the group per blockIdx.z
+        const long long cube_off = (long long)blockIdx.z * d.cube;
+        in += cube_off; out += cube_off; Z1 += cube_off; Z2 += cube_off;
+    }
     const int gx = x0 + 4 * lx;
     const bool col_ok = gx < d.nx;
     const float *col_in = in + (long long)y * d.nx + (col_ok ? gx : 0);
@@ -271,7 +275,7 @@ constexpr int zm_step_channels() { return RZ >= 96 ? 128 : 64; }
 
 template <int RZ>
 cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t,
-                      cudaStream_t st)
+                      int ncubes, cudaStream_t st)
 {
     constexpr int ZB = zm_step_channels<RZ>();
     using S = ZmShape<RZ, ZM_XT, ZB>;
@@ -281,7 +285,7 @@ cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const D
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    dim3 grid((d.nx + ZM_XT - 1) / ZM_XT, d.ny);
+    dim3 grid((d.nx + ZM_XT - 1) / ZM_XT, d.ny, ncubes);
     k_zm<RZ, ZM_XT, ZB><<<grid, S::THREADS, S::SMEM, st>>>(in, out, Z1, Z2, d, hz, t);
     return cudaGetLastError();
 }
@@ -297,8 +301,8 @@ cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const D
         return launch_z<RZ>(in, out, d, t, st);                                                             \
     }                                                                                                       \
     cudaError_t launch_zm_r##RZ(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz,   \
-                                const Taps &t, cudaStream_t st)                                             \
+                                const Taps &t, int ncubes, cudaStream_t st)                                 \
     {                                                                                                       \
-        return launch_zm<RZ>(in, out, Z1, Z2, d, hz, t, st);                                                \
+        return launch_zm<RZ>(in, out, Z1, Z2, d, hz, t, ncubes, st);                                        \
     }                                                                                                       \
     }
