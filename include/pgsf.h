@@ -60,6 +60,8 @@ typedef enum {
 
 /* plan flags */
 #define PGSF_FLAG_FORCE_GENERIC 0x1u /* use only the generic (any shape / any radius) kernels */
+#define PGSF_FLAG_SMALL_GROUPS  0x2u /* test aid: pgsf_find_multiscale takes a batch two cubes per launch group
+                                        (by default as many as fit 2^32 voxels), so that ragged last groups run */
 
 #define PGSF_MAX_SCALES 8
 #define PGSF_MAX_RADIUS 96 /* largest supported ceil(truncate*sigma) on any axis */

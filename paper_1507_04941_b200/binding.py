@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libpgsf.so")
 
 PGSF_OK, PGSF_ERR_INVALID_ARG, PGSF_ERR_UNSUPPORTED, PGSF_ERR_OOM, PGSF_ERR_CUDA = range(5)
 PGSF_FLAG_FORCE_GENERIC = 0x1
+PGSF_FLAG_SMALL_GROUPS = 0x2
 PGSF_MAX_SCALES = 8
 PGSF_MAX_RADIUS = 96
 _STATUS = {0: "PGSF_OK", 1: "PGSF_ERR_INVALID_ARG", 2: "PGSF_ERR_UNSUPPORTED", 3: "PGSF_ERR_OOM",

@@ -196,6 +196,7 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
     if (p->fast_filter && p->fast_stats && desc->batch > 1) {
         long long g = (1LL << 32) / p->dims.cube;
         if (g > 65535 / desc->nz) g = 65535 / desc->nz;
+        if ((desc->flags & PGSF_FLAG_SMALL_GROUPS) && g > 2) g = 2;
         if (g > desc->batch) g = desc->batch;
         p->group = g < 1 ? 1 : (int)g;
     }

@@ -115,6 +115,20 @@ def test_batch_with_halo(pg, synth, oracle, flags):
     assert count > 0
 
 
+def test_batch_in_ragged_groups(pg, synth, oracle):
+    """A batch of 3 taken two cubes per launch group (groups of 2 and 1): same result as one group."""
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[4], (96, 80, 112), batch=3, n_sources=6), halo=(16, 12, 20), k=3.0)
+    d = synth.make_workload(w, "cuda")
+    rep, count = _full_compare(pg, oracle, w, d, pg.PGSF_FLAG_SMALL_GROUPS, check_stats=False)
+    with _plan(pg, w) as plan:
+        mask1, cnt1, _ = plan.pgsf_find_multiscale(d, keep_filtered=True)
+    with _plan(pg, w, pg.PGSF_FLAG_SMALL_GROUPS) as plan:
+        mask2, cnt2, _ = plan.pgsf_find_multiscale(d, keep_filtered=True)
+    torch.cuda.synchronize()
+    assert torch.equal(mask1, mask2) and int(cnt1.item()) == int(cnt2.item()) == count
+
+
 # ------------------------------------------------------------------------------------ degenerate cases
 
 @pytest.mark.parametrize("flags", IMPLS)
