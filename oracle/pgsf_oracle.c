@@ -18,7 +18,9 @@
  * Memory order (reading C-0): linear index = x + nx*(y + ny*z); x is unit stride.
  * All accumulation is double.  Input cubes are float (the paper stores fp32).
  *
- * Pins: tests/test_oracle_pins.py (S1-S15 of DESIGN.md).  Nothing here is "parity unpinned"
+ * Also here: Eq. 1, the weighted convolution (NEXT-1 of SURVEY.md 8(f)), at both levels.
+ *
+ * Pins: tests/test_oracle_pins.py (S1-S15 and W1-W6 of DESIGN.md).  Nothing here is "parity unpinned"
  * except agreement with the authors' own PGSF output on their simulated cube, which is not
  * available (no code, no data).
  */
@@ -337,5 +339,95 @@ int pgsf_oracle_threshold_region(const double *csub, const int *clo, const int *
     }
     (void)wz;
     free(A1); free(A2); free(B1); free(B2);
+    return 0;
+}
+
+/* ---------------------------------------------------------------- weighted convolution (Eq. 1) */
+
+/*
+ * Eq. 1 as printed, with i = (x+ox, y+oy, z+oz) running over the filter support inside the cube:
+ *
+ *      c_w[x][y][z] =  sum_o d[i] f[o] w[i]  /  sum_o w[i]
+ *
+ * (reading C-16 of DESIGN.md).  The printed denominator carries no f: with w == 1 it yields
+ * c_u / (number of support voxels), not c_u.  mode 1 is the normalisation by sum_o f[o] w[i] that makes
+ * w == 1 reproduce c_u (offered as a flag; the paper prints mode 0).  Positions outside the cube contribute
+ * to neither sum (C-5); a zero denominator gives 0.  L0: direct six-deep loops.
+ */
+void pgsf_oracle_wfilter_direct(const float *d, const float *w, int nx, int ny, int nz,
+                                const double *gx, int rx, const double *gy, int ry,
+                                const double *gz, int rz, int mode, double *c)
+{
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                double num = 0.0, den = 0.0;
+                for (int oz = -rz; oz <= rz; ++oz) {
+                    int iz = z + oz;
+                    if (iz < 0 || iz >= nz) continue;
+                    for (int oy = -ry; oy <= ry; ++oy) {
+                        int iy = y + oy;
+                        if (iy < 0 || iy >= ny) continue;
+                        for (int ox = -rx; ox <= rx; ++ox) {
+                            int ix = x + ox;
+                            if (ix < 0 || ix >= nx) continue;
+                            const i64 i = (i64)ix + (i64)nx * ((i64)iy + (i64)ny * iz);
+                            const double f = gx[ox + rx] * gy[oy + ry] * gz[oz + rz];
+                            num += (double)d[i] * f * (double)w[i];
+                            den += mode ? f * (double)w[i] : (double)w[i];
+                        }
+                    }
+                }
+                c[(i64)x + (i64)nx * ((i64)y + (i64)ny * z)] = den != 0.0 ? num / den : 0.0;
+            }
+}
+
+/* one 1-D pass along `axis` over a dense double cube: out[v] = sum_{|o|<=r} in[v + o e_axis] g[o + r]
+ * (g == NULL: plain sum, the box of the printed denominator), positions outside the cube skipped */
+static void pass1d(const double *in, double *out, int nx, int ny, int nz, int axis, const double *g, int r)
+{
+    const int n[3] = {nx, ny, nz};
+    const i64 stride[3] = {1, nx, (i64)nx * ny};
+#pragma omp parallel for schedule(static)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                const int c[3] = {x, y, z};
+                const i64 i = (i64)x + (i64)nx * ((i64)y + (i64)ny * z);
+                double s = 0.0;
+                for (int o = -r; o <= r; ++o) {
+                    const int j = c[axis] + o;
+                    if (j < 0 || j >= n[axis]) continue;
+                    s += in[i + o * stride[axis]] * (g ? g[o + r] : 1.0);
+                }
+                out[i] = s;
+            }
+}
+
+/*
+ * L1: Eq. 1 through the separable form.  For an outer-product f the numerator is Eq. 2 applied to the
+ * product cube d*w (three 1-D passes, as pgsf_oracle_filter_region); the printed denominator is the sum
+ * of w over the box of the support (three 1-D plain sums), the mode-1 denominator Eq. 2 applied to w.
+ * Returns 0, or -2 when out of memory.
+ */
+int pgsf_oracle_wfilter(const float *d, const float *w, int nx, int ny, int nz,
+                        const double *gx, int rx, const double *gy, int ry, const double *gz, int rz,
+                        int mode, double *c)
+{
+    const i64 n = (i64)nx * ny * nz;
+    double *a = (double *)malloc(sizeof(double) * (size_t)n);
+    double *b = (double *)malloc(sizeof(double) * (size_t)n);
+    double *den = (double *)malloc(sizeof(double) * (size_t)n);
+    if (!a || !b || !den) { free(a); free(b); free(den); return -2; }
+    for (i64 i = 0; i < n; ++i) a[i] = (double)d[i] * (double)w[i];
+    pass1d(a, b, nx, ny, nz, 0, gx, rx);
+    pass1d(b, a, nx, ny, nz, 1, gy, ry);
+    pass1d(a, c, nx, ny, nz, 2, gz, rz);          /* numerator in c */
+    for (i64 i = 0; i < n; ++i) a[i] = (double)w[i];
+    pass1d(a, b, nx, ny, nz, 0, mode ? gx : NULL, rx);
+    pass1d(b, a, nx, ny, nz, 1, mode ? gy : NULL, ry);
+    pass1d(a, den, nx, ny, nz, 2, mode ? gz : NULL, rz);
+    for (i64 i = 0; i < n; ++i) c[i] = den[i] != 0.0 ? c[i] / den[i] : 0.0;
+    free(a); free(b); free(den);
     return 0;
 }

@@ -59,6 +59,12 @@ def _load():
             ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
             c_dbl_p, c_dbl_p, c_dbl_p, c_u8_p]
         lib.pgsf_oracle_threshold_brute.restype = None
+        lib.pgsf_oracle_wfilter_direct.argtypes = [
+            c_flt_p, c_flt_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, c_dbl_p, ctypes.c_int, c_dbl_p,
+            ctypes.c_int, c_dbl_p, ctypes.c_int, ctypes.c_int, c_dbl_p]
+        lib.pgsf_oracle_wfilter_direct.restype = None
+        lib.pgsf_oracle_wfilter.argtypes = lib.pgsf_oracle_wfilter_direct.argtypes
+        lib.pgsf_oracle_wfilter.restype = ctypes.c_int
         lib.pgsf_oracle_filter_region.argtypes = [
             c_flt_p, c_int_p, c_int_p, c_int_p,
             c_dbl_p, ctypes.c_int, c_dbl_p, ctypes.c_int, c_dbl_p, ctypes.c_int,
@@ -136,6 +142,32 @@ def threshold_brute(c: np.ndarray, box_half: Sequence[int], k: float) -> Stats:
 
 
 # --------------------------------------------------------------------------- L1: separable, regions
+
+def _wfilter(fn, d, w, sigma3, mode, truncate):
+    d = np.ascontiguousarray(d, dtype=np.float32)
+    w = np.ascontiguousarray(w, dtype=np.float32)
+    assert d.shape == w.shape and d.ndim == 3
+    nz, ny, nx = d.shape
+    g = [taps(s, truncate) for s in sigma3]
+    r = [radius(s, truncate) for s in sigma3]
+    out = np.empty(d.shape, dtype=np.float64)
+    rc = fn(_p(d, ctypes.c_float), _p(w, ctypes.c_float), nx, ny, nz, _p(g[0], ctypes.c_double), r[0],
+            _p(g[1], ctypes.c_double), r[1], _p(g[2], ctypes.c_double), r[2], int(mode), _p(out, ctypes.c_double))
+    if rc not in (None, 0):
+        raise MemoryError(f"pgsf_oracle_wfilter failed ({rc})")
+    return out
+
+
+def wfilter_direct(d: np.ndarray, w: np.ndarray, sigma3, mode: int = 0, truncate: float = 3.0) -> np.ndarray:
+    """L0 of Eq. 1: direct loops.  d, w: [nz, ny, nx]; mode 0 = denominator as printed (sum w),
+    mode 1 = sum f w."""
+    return _wfilter(_load().pgsf_oracle_wfilter_direct, d, w, sigma3, mode, truncate)
+
+
+def wfilter_full(d: np.ndarray, w: np.ndarray, sigma3, mode: int = 0, truncate: float = 3.0) -> np.ndarray:
+    """L1 of Eq. 1: separable numerator (Eq. 2 of d*w) over box sum of w (mode 0) or Eq. 2 of w (mode 1)."""
+    return _wfilter(_load().pgsf_oracle_wfilter, d, w, sigma3, mode, truncate)
+
 
 def filter_region(sub: np.ndarray, sub_lo, cube, sigma3, lo, hi, truncate: float = 3.0) -> np.ndarray:
     """Separable fp64 filter on the region [lo,hi) (x,y,z order) of a cube with extents `cube`.

@@ -316,3 +316,102 @@ def test_S15_multiscale_or_halo_and_count(oracle):
     reg = oracle.find_region(d[a[2]:b[2], a[1]:b[1], a[0]:b[0]], a, (40, 40, 64), sig, h, k, lo, hi, halo)
     ref = oracle.find_full(d, sig, h, k, halo=halo)
     np.testing.assert_array_equal(reg.mask, ref.mask[lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]])
+
+
+# ---------------------------------------------------------------------------------- Eq. 1 (weighted), NEXT-1
+
+def _wcube(shape, seed):
+    rng = np.random.default_rng(seed)
+    d = rng.standard_normal(shape).astype(np.float32)
+    w = rng.uniform(0.25, 2.0, shape).astype(np.float32)
+    return d, w
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("sigma3", [(1.0, 1.0, 2.0), (0.0, 1.5, 1.0), (1.0, 2.0, 5.0)])
+def test_W1_weighted_separable_equals_direct(oracle, mode, sigma3):
+    """L1 (separable numerator / box or filtered denominator) == L0 (Eq. 1 as a six-deep loop),
+    including a radius larger than the cube (sigma_z = 5 -> r = 15 > 14)."""
+    d, w = _wcube((14, 10, 12), 7)
+    a = oracle.wfilter_full(d, w, sigma3, mode)
+    b = oracle.wfilter_direct(d, w, sigma3, mode)
+    assert np.max(np.abs(a - b)) <= 1e-13 * max(1.0, np.max(np.abs(b)))
+
+
+def test_W2_unit_weights(oracle):
+    """w == 1: the printed denominator counts the support voxels inside the cube, so c_w = c_u / n
+    (n = 7*7*13 in the interior: the property reading C-16 notes); mode 1 divides by the partial tap sums
+    instead, so c_w = c_u in the interior."""
+    rng = np.random.default_rng(11)
+    d = rng.standard_normal((30, 16, 18)).astype(np.float32)
+    w = np.ones_like(d)
+    sig = (1.0, 1.0, 2.0)
+    cu = oracle.filter_full(d, sig)
+    r = [oracle.radius(s) for s in sig]
+    nz, ny, nx = d.shape
+    cnt = [np.array([min(c + rr, n - 1) - max(c - rr, 0) + 1 for c in range(n)], dtype=np.float64)
+           for n, rr in zip((nx, ny, nz), r)]
+    n3 = cnt[2][:, None, None] * cnt[1][None, :, None] * cnt[0][None, None, :]
+    c0 = oracle.wfilter_full(d, w, sig, 0)
+    assert np.max(np.abs(c0 - cu / n3)) <= 1e-15
+    assert n3[15, 8, 9] == 7 * 7 * 13
+    c1 = oracle.wfilter_full(d, w, sig, 1)
+    inner = (slice(r[2], nz - r[2]), slice(r[1], ny - r[1]), slice(r[0], nx - r[0]))
+    assert np.max(np.abs(c1[inner] - cu[inner])) <= 1e-14
+    # at a face mode 1 renormalises by the partial tap sum (closed form, cf. S4)
+    g = [oracle.taps(s) for s in sig]
+    px = np.array([g[0][max(0, r[0] - x):min(2 * r[0] + 1, r[0] + nx - x)].sum() for x in range(nx)])
+    assert abs(c1[15, 8, 0] - cu[15, 8, 0] / px[0]) <= 1e-14
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_W3_weight_scale_invariance(oracle, mode):
+    """Eq. 1 is a ratio that is homogeneous of degree 0 in w: w -> 4 w changes nothing (power of two: exactly)."""
+    d, w = _wcube((12, 12, 12), 3)
+    a = oracle.wfilter_full(d, w, (1.0, 1.0, 2.0), mode)
+    b = oracle.wfilter_full(d, 4.0 * w, (1.0, 1.0, 2.0), mode)
+    assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_W4_zero_weight_removes_a_voxel(oracle, mode):
+    """A voxel with w = 0 contributes to neither sum: a huge spike there is invisible, and the result
+    equals the one with the spike removed from d."""
+    d, w = _wcube((16, 12, 12), 5)
+    w[8, 6, 5] = 0.0
+    d2 = d.copy()
+    d2[8, 6, 5] = 1e6
+    a = oracle.wfilter_full(d, w, (1.0, 1.0, 2.0), mode)
+    b = oracle.wfilter_full(d2, w, (1.0, 1.0, 2.0), mode)
+    assert np.array_equal(a, b)
+    # all-zero weights: 0 / 0 -> 0
+    z = oracle.wfilter_full(d, np.zeros_like(w), (1.0, 1.0, 2.0), mode)
+    assert not z.any()
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_W5_weighted_against_scipy(oracle, mode):
+    """Library special case: numerator = correlate1d chain on d*w (mode='constant'), denominator =
+    correlate1d chain on w with the taps (mode 1) or with ones (mode 0)."""
+    from scipy import ndimage
+    d, w = _wcube((20, 14, 16), 9)
+    sig = (1.0, 2.0, 3.0)
+    num = (d.astype(np.float64) * w.astype(np.float64))
+    den = w.astype(np.float64)
+    for ax, s in zip((2, 1, 0), sig):
+        g = oracle.taps(s)
+        num = ndimage.correlate1d(num, g, axis=ax, mode="constant", cval=0.0)
+        den = ndimage.correlate1d(den, g if mode else np.ones_like(g), axis=ax, mode="constant", cval=0.0)
+    ref = num / den
+    a = oracle.wfilter_full(d, w, sig, mode)
+    assert np.max(np.abs(a - ref)) <= 1e-13 * np.max(np.abs(ref))
+
+
+def test_W6_constant_data_any_weights(oracle):
+    """d == c: mode 1 returns c wherever any weight is positive (a weighted mean of a constant), for ANY
+    weights; mode 0 returns c * sum f w / sum w."""
+    rng = np.random.default_rng(2)
+    w = rng.uniform(0.1, 3.0, (12, 10, 14)).astype(np.float32)
+    d = np.full_like(w, 2.5)
+    c1 = oracle.wfilter_full(d, w, (1.0, 1.0, 2.0), 1)
+    assert np.max(np.abs(c1 - 2.5)) <= 1e-14
