@@ -121,6 +121,23 @@ PGSF_API pgsf_status pgsf_filter3d(pgsf_plan *plan, int scale, const float *d_in
                           void *d_workspace, void *cuda_stream);
 
 /*
+ * pgsf_filter3d_weighted -- Eq. 1, the weighted convolution, for the Gaussian of scale `scale`
+ * (reading C-16 of DESIGN.md).  With i = (x+ox, y+oy, z+oz) over the part of the
+ * filter support inside the cube:
+ *     mode PGSF_WEIGHTED_AS_PRINTED : d_out = sum_o d_in[i] f[o] d_w[i] / sum_o d_w[i]        (the paper's Eq. 1)
+ *     mode PGSF_WEIGHTED_NORMALISED : d_out = sum_o d_in[i] f[o] d_w[i] / sum_o f[o] d_w[i]   (w == 1 gives Eq. 2)
+ * f[o] = gx[ox] gy[oy] gz[oz]; a zero denominator gives 0.  Both sums are evaluated in their separable form
+ * (numerator = Eq. 2 of the product cube d_in * d_w), fp32 throughout.
+ * d_in, d_w, d_out: batch*nx*ny*nz floats, 16-byte aligned DEVICE pointers; d_out must overlap neither input.
+ * Enqueues on `cuda_stream`, does not synchronise; errors as for pgsf_filter3d.
+ */
+#define PGSF_WEIGHTED_AS_PRINTED 0
+#define PGSF_WEIGHTED_NORMALISED 1
+PGSF_API pgsf_status pgsf_filter3d_weighted(pgsf_plan *plan, int scale, const float *d_in, const float *d_w,
+                                            float *d_out, int mode, void *d_workspace, void *cuda_stream);
+
+
+/*
  * pgsf_local_threshold -- local statistics and voxel selection of one
  * filtered cube, with the plan's box_half, k and halo:
  *     S1 = sum of f, S2 = sum of f^2 over the box [v-h, v+h] clipped to the cube (C-7), n = its

@@ -18,13 +18,15 @@ LIB_PATH = os.path.join(_HERE, "libpgsf.so")
 PGSF_OK, PGSF_ERR_INVALID_ARG, PGSF_ERR_UNSUPPORTED, PGSF_ERR_OOM, PGSF_ERR_CUDA = range(5)
 PGSF_FLAG_FORCE_GENERIC = 0x1
 PGSF_FLAG_SMALL_GROUPS = 0x2
+PGSF_WEIGHTED_AS_PRINTED = 0
+PGSF_WEIGHTED_NORMALISED = 1
 PGSF_MAX_SCALES = 8
 PGSF_MAX_RADIUS = 96
 _STATUS = {0: "PGSF_OK", 1: "PGSF_ERR_INVALID_ARG", 2: "PGSF_ERR_UNSUPPORTED", 3: "PGSF_ERR_OOM",
            4: "PGSF_ERR_CUDA"}
 
 EXPORTS = ["pgsf_plan_create", "pgsf_plan_destroy", "pgsf_plan_workspace_bytes", "pgsf_last_error",
-           "pgsf_plan_get_taps", "pgsf_filter3d", "pgsf_local_threshold", "pgsf_find_multiscale",
+           "pgsf_plan_get_taps", "pgsf_filter3d", "pgsf_filter3d_weighted", "pgsf_local_threshold", "pgsf_find_multiscale",
            "pgsf_find_multiscale_host", "pgsf_plan_launch_count", "pgsf_plan_set_profiling",
            "pgsf_plan_profile_collect", "pgsf_plan_profile_entry"]
 
@@ -67,6 +69,8 @@ def load_library() -> ctypes.CDLL:
         lib.pgsf_plan_get_taps.restype = i
         lib.pgsf_filter3d.argtypes = [vp, i, vp, vp, vp, vp]
         lib.pgsf_filter3d.restype = i
+        lib.pgsf_filter3d_weighted.argtypes = [vp, i, vp, vp, vp, i, vp, vp]
+        lib.pgsf_filter3d_weighted.restype = i
         lib.pgsf_local_threshold.argtypes = [vp, vp, vp, i, vp, vp, vp, vp, vp]
         lib.pgsf_local_threshold.restype = i
         lib.pgsf_find_multiscale.argtypes = [vp, vp, ctypes.POINTER(vp), vp, vp, vp, vp]
@@ -203,6 +207,19 @@ class Plan:
         ws = self.workspace()
         self._check(self._lib.pgsf_filter3d(self._h, int(scale), _ptr(d_in), _ptr(d_out), _ptr(ws),
                                             _stream_ptr(stream)))
+        return d_out
+
+    def pgsf_filter3d_weighted(self, scale: int, d_in: torch.Tensor, d_w: torch.Tensor, mode: int = 0,
+                               d_out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+        """Eq. 1 of the paper (weighted convolution); mode: PGSF_WEIGHTED_AS_PRINTED / _NORMALISED."""
+        self._check_cube(d_in, torch.float32, "d_in")
+        self._check_cube(d_w, torch.float32, "d_w")
+        if d_out is None:
+            d_out = torch.empty_like(d_in)
+        self._check_cube(d_out, torch.float32, "d_out")
+        ws = self.workspace()
+        self._check(self._lib.pgsf_filter3d_weighted(self._h, int(scale), _ptr(d_in), _ptr(d_w), _ptr(d_out),
+                                                     int(mode), _ptr(ws), _stream_ptr(stream)))
         return d_out
 
     def pgsf_local_threshold(self, d_filtered: torch.Tensor, d_mask: Optional[torch.Tensor] = None,

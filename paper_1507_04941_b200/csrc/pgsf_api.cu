@@ -364,6 +364,47 @@ pgsf_status pgsf_filter3d(pgsf_plan *p, int scale, const float *d_in, float *d_o
     return PGSF_OK;
 }
 
+pgsf_status pgsf_filter3d_weighted(pgsf_plan *p, int scale, const float *d_in, const float *d_w, float *d_out,
+                                   int mode, void *d_ws, void *stream)
+{
+    if (!p) return PGSF_ERR_INVALID_ARG;
+    if (scale < 0 || scale >= p->desc.n_scales) return fail(p, PGSF_ERR_INVALID_ARG, "scale out of range");
+    if (mode != PGSF_WEIGHTED_AS_PRINTED && mode != PGSF_WEIGHTED_NORMALISED)
+        return fail(p, PGSF_ERR_INVALID_ARG, "mode must be PGSF_WEIGHTED_AS_PRINTED or PGSF_WEIGHTED_NORMALISED");
+    if (!d_in || !d_w || !d_out) return fail(p, PGSF_ERR_INVALID_ARG, "NULL cube pointer");
+    if (!aligned16(d_in) || !aligned16(d_w) || !aligned16(d_out))
+        return fail(p, PGSF_ERR_INVALID_ARG, "cube pointers must be 16-byte aligned");
+    const size_t bytes = (size_t)p->dims.cube * p->desc.batch * sizeof(float);
+    const char *o = reinterpret_cast<const char *>(d_out);
+    for (const float *src : {d_in, d_w}) {
+        const char *a = reinterpret_cast<const char *>(src);
+        if (a < o + bytes && o < a + bytes) return fail(p, PGSF_ERR_INVALID_ARG, "d_out overlaps an input");
+    }
+    pgsf_status s = check_ws(p, d_ws);
+    if (s != PGSF_OK) return s;
+    cudaError_t e = cudaSetDevice(p->device);
+    if (e != cudaSuccess) return cuda_fail(p, e, "cudaSetDevice");
+    const Workspace w = carve(p, d_ws);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    float *den = w.stmp, *tmp = w.stmp + p->dims.cube;      // (the statistics cubes are free here)
+    for (int bi = 0; bi < p->desc.batch; ++bi) {
+        const size_t off = (size_t)bi * p->dims.cube;
+        // numerator: Eq. 2 of the product cube
+        if ((e = pgsf::weighted_mul(p, d_in + off, d_w + off, w.scratch, st)) != cudaSuccess)
+            return cuda_fail(p, e, "weighted product launch");
+        if ((s = filter_one(p, scale, w.scratch, d_out + off, w, st)) != PGSF_OK) return s;
+        // denominator: box sum of w (as printed) or Eq. 2 of w
+        if (mode == PGSF_WEIGHTED_AS_PRINTED) {
+            if ((e = pgsf::weighted_boxsum(p, scale, d_w + off, den, tmp, st)) != cudaSuccess)
+                return cuda_fail(p, e, "weight box sum launch");
+        } else if ((s = filter_one(p, scale, d_w + off, den, w, st)) != PGSF_OK) {
+            return s;
+        }
+        if ((e = pgsf::weighted_div(p, d_out + off, den, st)) != cudaSuccess) return cuda_fail(p, e, "division launch");
+    }
+    return PGSF_OK;
+}
+
 pgsf_status pgsf_local_threshold(pgsf_plan *p, const float *d_f, uint8_t *d_mask, int or_into,
                                  float *d_mean, float *d_std, unsigned long long *d_count, void *d_ws,
                                  void *stream)

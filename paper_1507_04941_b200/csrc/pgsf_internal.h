@@ -128,4 +128,9 @@ cudaError_t fast_threshold_xy(pgsf_plan *p, const float *f, const float *Z1, con
 cudaError_t fast_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean,
                            float *sd, unsigned long long *count, float *tmp2, cudaStream_t st);
 
+// ---- Eq. 1, weighted convolution (pgsf_weighted.cu): one cube per call
+cudaError_t weighted_mul(pgsf_plan *p, const float *d, const float *w, float *prod, cudaStream_t st);
+cudaError_t weighted_boxsum(pgsf_plan *p, int scale, const float *w, float *a, float *b, cudaStream_t st);
+cudaError_t weighted_div(pgsf_plan *p, float *c, const float *den, cudaStream_t st);
+
 }  // namespace pgsf

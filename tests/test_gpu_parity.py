@@ -129,6 +129,53 @@ def test_batch_in_ragged_groups(pg, synth, oracle):
     assert torch.equal(mask1, mask2) and int(cnt1.item()) == int(cnt2.item()) == count
 
 
+# ------------------------------------------------------------------------------------ Eq. 1 (weighted, NEXT-1)
+
+WEIGHTED_TOL = 1e-5     # max |gpu - oracle| <= WEIGHTED_TOL * max |oracle| (fp32 sums of O(1) data and weights)
+
+
+@pytest.mark.parametrize("flags", IMPLS)
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("dims,sigmas", [
+    ((64, 64, 128), ((1.0, 1.0, 2.0),)),                       # config 1 shape
+    ((100, 52, 77), ((1.0, 1.0, 2.0), (2.0, 2.0, 4.0))),       # ragged (nx % 4 == 0 keeps the fast path), two scales
+    ((30, 17, 9), ((1.5, 1.0, 4.0),)),                         # nx % 4 != 0, radius larger than nz
+])
+def test_weighted_filter(pg, synth, oracle, flags, mode, dims, sigmas):
+    """pgsf_filter3d_weighted against the oracle's Eq. 1 (P:57), both denominators, element by element;
+    weights U(0.25, 2) with a block of exact zeros (dead channels) and one all-zero neighbourhood."""
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[1], dims, n_sources=4), sigmas=sigmas)
+    d = synth.make_workload(w, "cuda")
+    g = torch.Generator(device="cuda").manual_seed(1234)
+    wt = torch.empty_like(d).uniform_(0.25, 2.0, generator=g)
+    wt[:, dims[2] // 3, :, :] = 0.0                                # a dead channel
+    wt[:, :, : min(12, dims[1]), : min(12, dims[0])] = 0.0         # a dead corner column (0 / 0 -> 0 deep inside it)
+    with _plan(pg, w, flags) as plan:
+        for s in range(len(sigmas)):
+            out = plan.pgsf_filter3d_weighted(s, d, wt, mode)
+            torch.cuda.synchronize()
+            ref = oracle.wfilter_full(d[0].cpu().numpy(), wt[0].cpu().numpy(), sigmas[s], mode)
+            got = out[0].cpu().numpy().astype(np.float64)
+            assert np.isfinite(got).all()
+            diff = np.max(np.abs(got - ref))
+            assert diff <= WEIGHTED_TOL * np.max(np.abs(ref)), f"scale {s} mode {mode}: {diff:.3e} vs max {np.max(np.abs(ref)):.3e}"
+            assert np.array_equal(got == 0.0, ref == 0.0) or np.max(np.abs(ref[got == 0.0])) <= WEIGHTED_TOL * np.max(np.abs(ref))
+
+
+def test_weighted_unit_weights_reproduce_filter3d(pg, synth):
+    """w == 1, normalised mode: Eq. 1 reduces to Eq. 2 in the interior (both sides the same kernels)."""
+    w = synth.WORKLOADS[1]
+    d = synth.make_workload(w, "cuda")
+    with _plan(pg, w) as plan:
+        a = plan.pgsf_filter3d(0, d)
+        b = plan.pgsf_filter3d_weighted(0, d, torch.ones_like(d), pg.PGSF_WEIGHTED_NORMALISED)
+        torch.cuda.synchronize()
+    rx, ry, rz = 3, 3, 6
+    ai, bi = a[0, rz:-rz, ry:-ry, rx:-rx], b[0, rz:-rz, ry:-ry, rx:-rx]
+    assert float((ai - bi).abs().max()) <= 2e-6
+
+
 # ------------------------------------------------------------------------------------ degenerate cases
 
 @pytest.mark.parametrize("flags", IMPLS)
