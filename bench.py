@@ -232,6 +232,8 @@ def _kernel_work(name: str, w, taps, n_vox: int):
     the separable method must do, not what the implementation happens to move."""
     S = len(taps)
     kind, _, tail = name.partition("_")
+    if kind in ("bxy", "bz"):                     # the filter kernels with all-ones taps (Eq. 1 denominator)
+        kind = kind[1:]
     if kind == "xy" and tail.startswith("m"):  # x and y passes of the scales in the bit mask, one read of the input
         grp = [t for i, t in enumerate(taps) if (int(tail[1:]) >> i) & 1]
         return 2 * sum(t[0] + t[1] for t in grp) * n_vox, (4 + 4 * len(grp)) * n_vox
@@ -246,6 +248,9 @@ def _kernel_work(name: str, w, taps, n_vox: int):
         return (2 * t[2] + STATS_Z_FLOPS) * n_vox, 8 * n_vox
     if kind == "stats" and tail == "xybox":     # x/y window sums + selection after a fused zm launch
         return (STATS_FLOPS - STATS_Z_FLOPS) * n_vox, 5 * n_vox
+    if kind == "w":                              # Eq. 1 helpers: product, box sum of the weights, division
+        return {"mul": (1, 12), "box": (6, 8), "div": (1, 12)}.get(tail, (0, 0))[0] * n_vox, \
+               {"mul": (1, 12), "box": (6, 8), "div": (1, 12)}.get(tail, (0, 0))[1] * n_vox
     if kind == "stats" and tail == "all":    # statistics of every scale, one mask write
         return STATS_FLOPS * S * n_vox, (4 * S + 1) * n_vox
     if kind == "stats":
@@ -412,6 +417,129 @@ def run_cpu_baseline(w, sub, a, lo, hi):
             "sample": _sample_text(w, lo, hi)}
 
 
+# ------------------------------------------------------------------------------------ Eq. 1 (weighted), NEXT-1
+
+W_METRIC = "Gvoxel/s per Gaussian scale (weighted filter, Eq. 1)"
+W_SAMPLE = (128, 128, 256)
+
+
+def run_weighted(args, w):
+    """--path weighted: one step = pgsf_filter3d_weighted (denominator as printed) for every scale of the
+    config over its cube; single GPU.  Same JSON contract as the main path."""
+    import torch
+    from paper_1507_04941_b200 import binding, build, synth
+    from oracle import pgsf_oracle
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a B200: the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    build.build()
+    binding.load_library()
+    props = torch.cuda.get_device_properties(0)
+    peaks = _peaks()
+    d = synth.make_workload(w, "cuda:0")
+    g = torch.Generator(device="cuda:0").manual_seed(w.seed + 5000)
+    wt = torch.empty_like(d).uniform_(0.25, 2.0, generator=g)
+    S = len(w.sigmas)
+    taps = _taps(w)
+    cube = w.dims[0] * w.dims[1] * w.dims[2]
+    plan = binding.Plan(w.dims, w.sigmas, w.box_half, w.k, batch=w.batch, halo=w.halo, truncate=w.truncate)
+    out = torch.empty_like(d)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        for s in range(S):
+            plan.pgsf_filter3d_weighted(s, d, wt, binding.PGSF_WEIGHTED_AS_PRINTED, d_out=out, stream=stream)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    plan.pgsf_plan_set_profiling(True)
+    l0 = plan.pgsf_plan_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    ms_step = ev0.elapsed_time(ev1) / args.steps
+    launches = plan.pgsf_plan_launch_count() - l0
+    prof = plan.pgsf_plan_profile()
+    plan.pgsf_plan_set_profiling(False)
+    clocks = sampler.stop()
+    alu_peak = _alu_peak_tflops(props.multi_processor_count, peaks["sm_max_mhz"])
+    hbm_peak = peaks["hbm_gbs"]
+    kern = []
+    for name, (n, ms) in prof.items():
+        fl, by = _kernel_work(name, w, taps, cube)
+        kern.append({"name": name, "launches": n, "ms_per_launch": ms / max(n, 1),
+                     "share": ms / max(ms_step * args.steps, 1e-9), "flops": fl, "bytes": by})
+    kern.sort(key=lambda k: -k["share"])
+    k0 = kern[0]
+    t_alu, t_hbm = k0["flops"] / (alu_peak * 1e12), k0["bytes"] / (hbm_peak * 1e9)
+    sec = k0["ms_per_launch"] * 1e-3
+    if t_alu >= t_hbm:
+        ach = k0["flops"] / sec / 1e12
+        roofline = {"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak}
+    else:
+        ach = k0["bytes"] / sec / 1e9
+        roofline = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak}
+    roofline.update({"kernel": k0["name"], "ms_per_launch": k0["ms_per_launch"], "share_of_step": k0["share"],
+                     "traffic": None})
+    n_vox = w.voxels
+    path_flops = sum(2 * sum(t) + 8 for t in taps) * n_vox
+    path_bytes = 12 * S * n_vox
+    t_path = max(path_flops / (alu_peak * 1e12), path_bytes / (hbm_peak * 1e9))
+    # end to end: pinned host cubes in, every scale's result out
+    e2e = None
+    if not args.no_e2e:
+        h_d = torch.empty(d.shape, dtype=torch.float32, pin_memory=True).copy_(d)
+        h_w = torch.empty(d.shape, dtype=torch.float32, pin_memory=True).copy_(wt)
+        h_o = torch.empty(d.shape, dtype=torch.float32, pin_memory=True)
+        steps = max(1, min(args.steps, 3))
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            d.copy_(h_d, non_blocking=True)
+            wt.copy_(h_w, non_blocking=True)
+            for s in range(S):
+                plan.pgsf_filter3d_weighted(s, d, wt, binding.PGSF_WEIGHTED_AS_PRINTED, d_out=out, stream=stream)
+                h_o.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+        sec_e = (time.perf_counter() - t0) / steps
+        e2e = {"value": n_vox * S / sec_e / 1e9, "unit": UNIT, "ms_per_step": sec_e * 1e3, "steps": steps,
+               "h2d_bytes_per_step": 8 * n_vox, "d2h_bytes_per_step": 4 * n_vox * S,
+               "api": "binding.Plan.pgsf_filter3d_weighted on pinned host cubes (torch copies)"}
+    cpu = None
+    if not args.no_cpu_baseline:
+        lo = [max(0, (n - sz) // 2) for n, sz in zip(w.dims, W_SAMPLE)]
+        hi = [min(n, l + sz) for n, l, sz in zip(w.dims, lo, W_SAMPLE)]
+        sd = d[0, lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]].cpu().numpy()
+        sw = wt[0, lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]].cpu().numpy()
+        plan.close()
+        threads = pgsf_oracle.set_threads(0)
+        t0 = time.perf_counter()
+        for sg in w.sigmas:
+            pgsf_oracle.wfilter_full(sd, sw, sg, 0, w.truncate)
+        dt = time.perf_counter() - t0
+        cpu = {"value": sd.size * S / dt / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle", "seconds": dt,
+               "sample": f"centred brick {sd.shape[2]}x{sd.shape[1]}x{sd.shape[0]} of {w.name} taken as a "
+                         f"standalone cube, all {S} scales, oracle Eq. 1 (L1 separable, fp64)"}
+    line = {"metric": W_METRIC, "value": n_vox * S / (ms_step * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "path": "weighted (Eq. 1, denominator as printed)",
+                       "weights": "U(0.25, 2) fp32, seeded", "scales": S,
+                       "l2": "inputs larger than L2" if n_vox * 4 > 2**28 else "inputs fit L2 (small config)"},
+            "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline,
+            "path_roofline": {"flops_per_voxel": path_flops / n_vox, "bytes_per_voxel": path_bytes / n_vox,
+                              "roofline_ms": t_path * 1e3, "frac": t_path * 1e3 / ms_step},
+            "kernels": [{"name": k["name"], "launches": k["launches"], "ms_per_launch": round(k["ms_per_launch"], 4),
+                         "share": round(k["share"], 4)} for k in kern],
+            "e2e": e2e, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -420,6 +548,8 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5],
                     help="BASELINE.json config (1-based); default 3 = the 8 GiB cube the north star is quoted on")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--path", default="find", choices=["find", "weighted"],
+                    help="find = the hot path (default); weighted = Eq. 1 of the paper (NEXT-1), single GPU")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -428,6 +558,10 @@ def main():
     w = synth.WORKLOADS[args.config]
     if args.impl == "reference":
         run_reference(args, w)
+        return
+    if args.path == "weighted":
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_weighted(args, w)
         return
     line, ctx = run_b200(args, w)
     rank, world = ctx["rank"], ctx["world"]

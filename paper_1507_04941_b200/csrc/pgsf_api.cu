@@ -184,6 +184,10 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
         for (int o = -sp.r[1]; o <= sp.r[1]; ++o) sp.txy.gy[o + sp.rxy_c] = sp.taps[1].g[o + sp.r[1]];
         sp.tz.r = sp.rz_c;
         for (int o = -sp.r[2]; o <= sp.r[2]; ++o) sp.tz.g[o + sp.rz_c + pgsf::kTapPad] = sp.taps[2].g[o + sp.r[2]];
+        for (int o = -sp.r[0]; o <= sp.r[0]; ++o) sp.txy_box.gx[o + sp.rxy_c] = 1.f;
+        for (int o = -sp.r[1]; o <= sp.r[1]; ++o) sp.txy_box.gy[o + sp.rxy_c] = 1.f;
+        sp.tz_box.r = sp.rz_c;
+        for (int o = -sp.r[2]; o <= sp.r[2]; ++o) sp.tz_box.g[o + sp.rz_c + pgsf::kTapPad] = 1.f;
     }
     p->fast_filter = fast;
     p->fast_stats = !force_generic && (desc->nx % 4 == 0) && pgsf::fast_stats_supported(p);
@@ -395,8 +399,10 @@ pgsf_status pgsf_filter3d_weighted(pgsf_plan *p, int scale, const float *d_in, c
         if ((s = filter_one(p, scale, w.scratch, d_out + off, w, st)) != PGSF_OK) return s;
         // denominator: box sum of w (as printed) or Eq. 2 of w
         if (mode == PGSF_WEIGHTED_AS_PRINTED) {
-            if ((e = pgsf::weighted_boxsum(p, scale, d_w + off, den, tmp, st)) != cudaSuccess)
-                return cuda_fail(p, e, "weight box sum launch");
+            // fast path: the filter kernels with all-ones taps; else three generic directional sums
+            e = p->fast_filter ? pgsf::fast_filter3d(p, scale, d_w + off, den, w.ftmp, st, true)
+                               : pgsf::weighted_boxsum(p, scale, d_w + off, den, tmp, st);
+            if (e != cudaSuccess) return cuda_fail(p, e, "weight box sum launch");
         } else if ((s = filter_one(p, scale, d_w + off, den, w, st)) != PGSF_OK) {
             return s;
         }

@@ -333,7 +333,7 @@ static bool xym_dispatch(int n, const int *rc, const float *in, const XymParams 
 // scales are sorted by compiled radius and cut into the largest groups a k_xym instance exists for;
 // every group reads the input once.
 cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *in, float *const *out, int ncubes,
-                          cudaStream_t st)
+                          cudaStream_t st, bool box)
 {
     // the x and y passes do not couple planes: `ncubes` consecutive cubes are one stack of ncubes * nz planes
     Dims d = p->dims;
@@ -375,11 +375,11 @@ cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *i
             const int j = i < take ? i : 0;
             const int sidx = scales[order[pos + j]];
             P.out[i] = out[order[pos + j]];
-            P.t[i] = p->scales[sidx].txy;
+            P.t[i] = box ? p->scales[sidx].txy_box : p->scales[sidx].txy;
             if (i < take) mask |= 1u << sidx;
         }
         char name[32];
-        snprintf(name, sizeof name, "xy_m%u", mask);
+        snprintf(name, sizeof name, box ? "bxy_m%u" : "xy_m%u", mask);
         LaunchScope ls(p, name, st);
         cudaError_t e = cudaSuccess;
         xym_dispatch(take, rc, in, P, p->sm_count, st, false, &e);
@@ -390,21 +390,22 @@ cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *i
 }
 
 // frequency pass of one scale: in (x/y-filtered cube) -> out
-cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStream_t st)
+cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStream_t st, bool box)
 {
     const Dims &d = p->dims;
     const ScalePlan &sp = p->scales[scale];
     if (d.ny > 65535 || d.nz > 65535 * 64) return cudaErrorInvalidConfiguration;
     char name[32];
-    snprintf(name, sizeof name, "z_s%d", scale);
+    snprintf(name, sizeof name, box ? "bz_s%d" : "z_s%d", scale);
     LaunchScope ls(p, name, st);
+    const Taps &tz = box ? sp.tz_box : sp.tz;
     switch (sp.rz_c) {
-    case 6: return launch_z_r6(in, out, d, sp.tz, st);
-    case 12: return launch_z_r12(in, out, d, sp.tz, st);
-    case 24: return launch_z_r24(in, out, d, sp.tz, st);
-    case 48: return launch_z_r48(in, out, d, sp.tz, st);
-    case 72: return launch_z_r72(in, out, d, sp.tz, st);
-    case 96: return launch_z_r96(in, out, d, sp.tz, st);
+    case 6: return launch_z_r6(in, out, d, tz, st);
+    case 12: return launch_z_r12(in, out, d, tz, st);
+    case 24: return launch_z_r24(in, out, d, tz, st);
+    case 48: return launch_z_r48(in, out, d, tz, st);
+    case 72: return launch_z_r72(in, out, d, tz, st);
+    case 96: return launch_z_r96(in, out, d, tz, st);
     default: return cudaErrorNotSupported;
     }
 }
@@ -433,12 +434,12 @@ cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float 
 }
 
 cudaError_t fast_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp,
-                          cudaStream_t st)
+                          cudaStream_t st, bool box)
 {
     float *outs[1] = {tmp};
-    cudaError_t e = fast_xy_multi(p, &scale, 1, in, outs, 1, st);
+    cudaError_t e = fast_xy_multi(p, &scale, 1, in, outs, 1, st, box);
     if (e != cudaSuccess) return e;
-    return fast_z(p, scale, tmp, out, st);
+    return fast_z(p, scale, tmp, out, st, box);
 }
 
 }  // namespace pgsf

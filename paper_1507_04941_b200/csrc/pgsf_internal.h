@@ -39,6 +39,8 @@ struct ScalePlan {
     Taps taps[3];        // true taps (generic path; also what pgsf_plan_get_taps reports)
     TapsXY txy;          // taps centred in a 2*rxy_c+1 window, zero padded
     Taps tz;             // taps centred in a 2*rz_c+1 window, zero padded
+    TapsXY txy_box;      // all-ones taps over the true radii: the box of the filter support (Eq. 1 denominator)
+    Taps tz_box;
 };
 
 struct Dims {
@@ -111,12 +113,13 @@ cudaError_t generic_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int o
 // ---- fast kernels (pgsf_filter.cu, pgsf_stats.cu): nx % 4 == 0, 16-byte aligned, compiled radii --
 bool fast_xy_radius(int r, int *compiled);
 bool fast_z_radius(int r, int *compiled);
+// box = true: the same passes with all-ones taps (sum over the box of the filter support)
 cudaError_t fast_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp,
-                          cudaStream_t st);
+                          cudaStream_t st, bool box = false);
 // `ncubes` consecutive cubes (stride dims.cube) per call, for the entry points that take it
 cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *in, float *const *out, int ncubes,
-                          cudaStream_t st);
-cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStream_t st);
+                          cudaStream_t st, bool box = false);
+cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStream_t st, bool box = false);
 cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, int ncubes,
                     cudaStream_t st);
 bool fast_stats_supported(const pgsf_plan *p);

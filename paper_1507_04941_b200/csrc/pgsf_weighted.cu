@@ -29,12 +29,19 @@ __global__ void __launch_bounds__(kThreads) k_wmul(const float *__restrict__ d, 
 }
 
 // c = den != 0 ? c / den : 0
-__global__ void __launch_bounds__(kThreads) k_wdiv(float *__restrict__ c, const float *__restrict__ den, long long n)
+__device__ __forceinline__ float wdiv(float c, float q) { return q != 0.f ? c / q : 0.f; }
+
+__global__ void __launch_bounds__(kThreads) k_wdiv(float *__restrict__ c, const float *__restrict__ den, long long n4,
+                                                   long long n)
 {
     const long long i = (long long)blockIdx.x * kThreads + threadIdx.x;
-    if (i >= n) return;
-    const float q = den[i];
-    c[i] = q != 0.f ? c[i] / q : 0.f;
+    if (i < n4) {
+        const float4 a = reinterpret_cast<const float4 *>(c)[i];
+        const float4 q = __ldg(reinterpret_cast<const float4 *>(den) + i);
+        reinterpret_cast<float4 *>(c)[i] = make_float4(wdiv(a.x, q.x), wdiv(a.y, q.y), wdiv(a.z, q.z), wdiv(a.w, q.w));
+    }
+    const long long t = 4 * n4 + i;
+    if (i < n - 4 * n4) c[t] = wdiv(c[t], den[t]);
 }
 
 // out[v] = sum_{|o| <= r} in[v + o e_AXIS] over the part of the support inside the cube (C-5)
@@ -85,8 +92,12 @@ cudaError_t weighted_boxsum(pgsf_plan *p, int scale, const float *w, float *a, f
 
 cudaError_t weighted_div(pgsf_plan *p, float *c, const float *den, cudaStream_t st)
 {
+    const long long n = p->dims.cube;
+    const bool vec = ((reinterpret_cast<uintptr_t>(c) | reinterpret_cast<uintptr_t>(den)) & 15u) == 0;
+    const long long n4 = vec ? n / 4 : 0;
+    const long long work = n4 > n - 4 * n4 ? n4 : n - 4 * n4;
     LaunchScope ls(p, "w_div", st);
-    k_wdiv<<<blocks_for(p->dims.cube), kThreads, 0, st>>>(c, den, p->dims.cube);
+    k_wdiv<<<blocks_for(work > 0 ? work : 1), kThreads, 0, st>>>(c, den, n4, n);
     return cudaGetLastError();
 }
 
