@@ -37,8 +37,32 @@ __device__ __forceinline__ void kahan_add(float &s, float &e, float v)
     s = t;
 }
 
-__host__ __device__ constexpr int round4(int v) { return (v + 3) & ~3; }
 
+
+// Opt a kernel in to `bytes` of dynamic shared memory.  The attribute belongs to the (kernel, device) pair,
+// so what has been granted is remembered per pair (many kernels share one function-pointer type).
+template <class K>
+cudaError_t ensure_dynamic_smem(K kernel, int bytes)
+{
+    struct Grant { const void *fn; int dev; int bytes; };
+    static Grant table[256];
+    static int used = 0;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const void *fn = reinterpret_cast<const void *>(kernel);
+    Grant *g = nullptr;
+    for (int i = 0; i < used; ++i)
+        if (table[i].fn == fn && table[i].dev == dev) { g = &table[i]; break; }
+    if (g && g->bytes >= bytes) return cudaSuccess;
+    if (bytes > 48 * 1024) {
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        if (e != cudaSuccess) return e;
+    }
+    if (!g && used < 256) g = &table[used++];
+    if (g) { g->fn = fn; g->dev = dev; g->bytes = bytes; }
+    return cudaSuccess;
+}
 
 }  // namespace
 }  // namespace pgsf

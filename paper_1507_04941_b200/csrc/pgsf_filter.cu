@@ -1,11 +1,9 @@
 // Tiled sm_100a kernels for the separable form of Eq. 2 (index ranges Eq. 3-5).
 //
-//   k_xy<R>  : per z-plane, x and y passes staged through shared memory (input tile + halo, zero
-//              filled outside the cube = the zero padding of reading C-5), result t2 to HBM.
-//   k_z<RZ>  : the frequency axis (filters are largest along z).  A CTA stages a slab of
-//              ZB + 2 RZ planes of a 128-column strip in shared memory; every thread owns four
-//              x columns and PZ consecutive channels and walks along z with its accumulators in
-//              registers.
+//   k_xym<NS,R..> : per z-plane, the x and y passes of up to four scales from one read of the input
+//              (this file); result t2 to HBM.
+//   k_z<RZ>, k_zm<RZ> : the frequency axis (filters are largest along z), alone or fused with the
+//              z-direction window sums of the statistics (pgsf_zpass.cuh, one translation unit per radius).
 //
 // Both passes are plain FP32 FMAs: the inner loops are packed `fma.rn.f32x2` (SASS FFMA2) whose
 // tap operand is a kernel-parameter constant, i.e. a uniform register broadcast -- the sm_100a form
@@ -266,12 +264,8 @@ template <int NS, int RA, int RB, int RC, int RD>
 cudaError_t launch_xym(const float *in, const XymParams &P, int sm_count, cudaStream_t st)
 {
     constexpr int SMEM = (XM_NB * XM_SIN + XM_NB * NS * XM_U) * (int)sizeof(float2);
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_xym<NS, RA, RB, RC, RD>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    cudaError_t e = ensure_dynamic_smem(k_xym<NS, RA, RB, RC, RD>, SMEM);
+    if (e != cudaSuccess) return e;
     (void)sm_count;
     dim3 grid((P.d.nx + XM_NT - 1) / XM_NT, (P.d.ny + P.ychunk - 1) / P.ychunk, P.d.nz);
     k_xym<NS, RA, RB, RC, RD><<<grid, XM_NT, SMEM, st>>>(in, P);

@@ -1,6 +1,6 @@
 // Local statistics + voxel selection for sm_100a ("three directional sums" of the filtered
 // data and of its square, then the z-score; P:33 / P:282 threshold and voxel selection; readings
-// C-6..C-10).  Two kernels per filtered cube, no other pass over the data:
+// C-6..C-10).  Two kernels per filtered cube:
 //
 //   k_zbox    frequency direction first.  Every thread owns four adjacent (x, y) columns and marches
 //             along z with the window sums  Z1 = sum_{|o|<=hz} f(z+o),  Z2 = sum f(z+o)^2  in registers:
@@ -9,18 +9,18 @@
 //             > 10^3 x the filtered noise in f^2, and an uncompensated fp32 running sum would keep the
 //             rounding error made while the source was inside the window long after it has left.
 //             Writes Z1, Z2 (two workspace cubes).
-//   k_xybox   per z plane: 128 x 32 tile + (hx, hy) halo of Z1 and Z2 staged in shared memory (cp.async,
-//             zero fill outside the cube = the clipped window of C-7), x- then y-direction window sums,
-//             then m = S1/n, var = S2/n - m^2, selection f > m + k sd (division-free form of
-//             pgsf_generic.cu), mask write / OR, count.  The window sums use the van Herk / Gil-Werman
-//             decomposition (suffix sum of one block + prefix sum of the next): ~3 additions per output
-//             like a sliding sum, but every output is a plain sum of the elements of ITS window, so no
-//             cancellation and no error carried over from bright neighbours.
+//   k_ymarch  per z plane: y-direction window sums marched in registers, x-direction window from the
+//             prefix / suffix sums of thread-owned column groups, then m = S1/n, var = S2/n - m^2,
+//             selection f > m + k sd (division-free form of pgsf_generic.cu), halo, mask write / OR, count
+//             (details at the kernel).
+// Inside pgsf_find_multiscale the z direction comes out of the frequency pass itself (k_zm, pgsf_zpass.cuh)
+// and k_zbox is not launched.
 //
-// Preconditions (else the generic kernels run): nx % 4 == 0, hx in {0,4,8,12,16}, hy <= 16.
+// Preconditions (else the generic kernels run): fast_stats_supported() below.
 #include <stdio.h>
 
 #include "pgsf_internal.h"
+#include "pgsf_device.cuh"
 
 namespace pgsf {
 namespace {
@@ -35,15 +35,6 @@ struct ZboxParams {
     int zchunk, nchunks;
     long long cols4;     // nx*ny/4 float4 columns per cube
 };
-
-// Kahan-compensated s += v (e holds the running low-order error)
-__device__ __forceinline__ void kahan_add(float &s, float &e, float v)
-{
-    const float y = v - e;
-    const float t = s + y;
-    e = (t - s) - y;
-    s = t;
-}
 
 __global__ void __launch_bounds__(ZB_NT) k_zbox(const float4 *__restrict__ f, float4 *__restrict__ Z1,
                                                 float4 *__restrict__ Z2, ZboxParams p)
@@ -392,12 +383,8 @@ cudaError_t launch_ymarch(const pgsf_plan *pl, const float *f, const float *Z1, 
     p.ychunk = (d.ny + nch - 1) / nch;
     nch = (d.ny + p.ychunk - 1) / p.ychunk;
     const int smem = 8 * (G / VL) * (nt + 4) * VL * (int)sizeof(float);
-    static int configured = 0;
-    if (smem > 48 * 1024 && configured < smem) {
-        cudaError_t e = cudaFuncSetAttribute(k_ymarch<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        configured = smem;
-    }
+    cudaError_t ce = ensure_dynamic_smem(k_ymarch<G>, smem);
+    if (ce != cudaSuccess) return ce;
     if ((long long)d.nz * ncubes > 65535) return cudaErrorInvalidConfiguration;
     dim3 grid(p.ntiles, nch, d.nz * ncubes);
     k_ymarch<G><<<grid, nt, smem, st>>>(f, Z1, Z2, mask, mean, sd, count, p);

@@ -256,13 +256,8 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
 template <int RZ>
 cudaError_t launch_z(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st)
 {
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_z<RZ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             ZShape<RZ>::SMEM);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    cudaError_t e = ensure_dynamic_smem(k_z<RZ>, ZShape<RZ>::SMEM);
+    if (e != cudaSuccess) return e;
     dim3 grid((d.nz + Z_ZB - 1) / Z_ZB, (d.nx + Z_XT - 1) / Z_XT, d.ny);
     k_z<RZ><<<grid, Z_THREADS, ZShape<RZ>::SMEM, st>>>(in, out, d, t);
     return cudaGetLastError();
@@ -279,12 +274,8 @@ cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const D
 {
     constexpr int ZB = zm_step_channels<RZ>();
     using S = ZmShape<RZ, ZM_XT, ZB>;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_zm<RZ, ZM_XT, ZB>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    cudaError_t e = ensure_dynamic_smem(k_zm<RZ, ZM_XT, ZB>, S::SMEM);
+    if (e != cudaSuccess) return e;
     dim3 grid((d.nx + ZM_XT - 1) / ZM_XT, d.ny, ncubes);
     k_zm<RZ, ZM_XT, ZB><<<grid, S::THREADS, S::SMEM, st>>>(in, out, Z1, Z2, d, hz, t);
     return cudaGetLastError();
