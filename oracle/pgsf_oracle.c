@@ -18,9 +18,10 @@
  * Memory order (reading C-0): linear index = x + nx*(y + ny*z); x is unit stride.
  * All accumulation is double.  Input cubes are float (the paper stores fp32).
  *
- * Also here: Eq. 1, the weighted convolution (NEXT-1 of SURVEY.md 8(f)), at both levels.
+ * Also here: Eq. 1, the weighted convolution (NEXT-1 of SURVEY.md 8(f)), at both levels, and Eq. 2
+ * for an arbitrary non-separable filter array (NEXT-2).
  *
- * Pins: tests/test_oracle_pins.py (S1-S15 and W1-W6 of DESIGN.md).  Nothing here is "parity unpinned"
+ * Pins: tests/test_oracle_pins.py (S1-S15, W1-W6 and G1-G3 of DESIGN.md).  Nothing here is "parity unpinned"
  * except agreement with the authors' own PGSF output on their simulated cube, which is not
  * available (no code, no data).
  */
@@ -430,4 +431,40 @@ int pgsf_oracle_wfilter(const float *d, const float *w, int nx, int ny, int nz,
     for (i64 i = 0; i < n; ++i) c[i] = den[i] != 0.0 ? c[i] / den[i] : 0.0;
     free(a); free(b); free(den);
     return 0;
+}
+
+/* ---------------------------------------------------------------- Eq. 2 for an ARBITRARY filter (NEXT-2) */
+
+/*
+ * Eq. 2 with the index ranges of Eq. 3-5 for a general, non-separable filter array
+ * f[oz][oy][ox] (x fastest, (2rz+1) x (2ry+1) x (2rx+1) doubles) -- what the paper's own kernel evaluates
+ * ("for each X and Y position in the filter ... for each Z position").  As printed it is a
+ * correlation, d[x+ox] f[ox] (C-4): the orientation matters once f is not symmetric.  Input outside the
+ * cube = 0 (C-5).  fp64 accumulation.
+ */
+void pgsf_oracle_filter_general(const float *d, int nx, int ny, int nz, const double *f, int rx, int ry, int rz,
+                                double *c)
+{
+    const int fx = 2 * rx + 1, fy = 2 * ry + 1;
+#pragma omp parallel for schedule(static)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                double sum = 0.0;
+                for (int oz = -rz; oz <= rz; ++oz) {
+                    const int iz = z + oz;
+                    if (iz < 0 || iz >= nz) continue;
+                    for (int oy = -ry; oy <= ry; ++oy) {
+                        const int iy = y + oy;
+                        if (iy < 0 || iy >= ny) continue;
+                        for (int ox = -rx; ox <= rx; ++ox) {
+                            const int ix = x + ox;
+                            if (ix < 0 || ix >= nx) continue;
+                            sum += (double)d[(i64)ix + (i64)nx * ((i64)iy + (i64)ny * iz)] *
+                                   f[(ox + rx) + (i64)fx * ((oy + ry) + (i64)fy * (oz + rz))];
+                        }
+                    }
+                }
+                c[(i64)x + (i64)nx * ((i64)y + (i64)ny * z)] = sum;
+            }
 }

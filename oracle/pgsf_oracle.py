@@ -65,6 +65,10 @@ def _load():
         lib.pgsf_oracle_wfilter_direct.restype = None
         lib.pgsf_oracle_wfilter.argtypes = lib.pgsf_oracle_wfilter_direct.argtypes
         lib.pgsf_oracle_wfilter.restype = ctypes.c_int
+        lib.pgsf_oracle_filter_general.argtypes = [
+            c_flt_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, c_dbl_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+            c_dbl_p]
+        lib.pgsf_oracle_filter_general.restype = None
         lib.pgsf_oracle_filter_region.argtypes = [
             c_flt_p, c_int_p, c_int_p, c_int_p,
             c_dbl_p, ctypes.c_int, c_dbl_p, ctypes.c_int, c_dbl_p, ctypes.c_int,
@@ -142,6 +146,20 @@ def threshold_brute(c: np.ndarray, box_half: Sequence[int], k: float) -> Stats:
 
 
 # --------------------------------------------------------------------------- L1: separable, regions
+
+def filter_general(d: np.ndarray, f: np.ndarray) -> np.ndarray:
+    """Eq. 2 for an arbitrary filter array f[oz, oy, ox] with odd extents (NEXT-2): direct loops,
+    correlation orientation as printed, zero outside the cube, fp64.  d: [nz, ny, nx]."""
+    d = np.ascontiguousarray(d, dtype=np.float32)
+    f = np.ascontiguousarray(f, dtype=np.float64)
+    assert d.ndim == 3 and f.ndim == 3 and all(n % 2 == 1 for n in f.shape)
+    nz, ny, nx = d.shape
+    rz, ry, rx = [(n - 1) // 2 for n in f.shape]
+    out = np.empty(d.shape, dtype=np.float64)
+    _load().pgsf_oracle_filter_general(_p(d, ctypes.c_float), nx, ny, nz, _p(f, ctypes.c_double), rx, ry, rz,
+                                       _p(out, ctypes.c_double))
+    return out
+
 
 def _wfilter(fn, d, w, sigma3, mode, truncate):
     d = np.ascontiguousarray(d, dtype=np.float32)

@@ -415,3 +415,48 @@ def test_W6_constant_data_any_weights(oracle):
     d = np.full_like(w, 2.5)
     c1 = oracle.wfilter_full(d, w, (1.0, 1.0, 2.0), 1)
     assert np.max(np.abs(c1 - 2.5)) <= 1e-14
+
+
+# ---------------------------------------------------------------------------------- Eq. 2, arbitrary filter (NEXT-2)
+
+def test_G1_general_equals_outer_product_path(oracle):
+    """With f = gz (x) gy (x) gx the general routine is the L0 routine of S5 (and hence the separable one)."""
+    rng = np.random.default_rng(21)
+    d = rng.standard_normal((14, 12, 16)).astype(np.float32)
+    sig = (1.0, 1.5, 2.0)
+    g = [oracle.taps(s) for s in sig]
+    f = g[2][:, None, None] * g[1][None, :, None] * g[0][None, None, :]
+    a = oracle.filter_general(d, f)
+    b = oracle.filter_direct(d, sig)
+    assert np.max(np.abs(a - b)) <= 1e-14
+
+
+def test_G2_general_impulse_orientation(oracle):
+    """Eq. 2 is printed as a correlation, c[v] = sum_o d[v+o] f[o]: an impulse at p gives c[p - o] = f[o],
+    i.e. the FLIPPED filter around p.  An asymmetric random f tells correlation from convolution and
+    catches transposed axes (unequal radii)."""
+    rng = np.random.default_rng(22)
+    f = rng.standard_normal((5, 3, 7))            # rz = 2, ry = 1, rx = 3
+    d = np.zeros((11, 9, 13), np.float32)
+    p = (5, 4, 6)
+    d[p] = 1.0
+    c = oracle.filter_general(d, f)
+    for oz in range(-2, 3):
+        for oy in range(-1, 2):
+            for ox in range(-3, 4):
+                assert c[p[0] - oz, p[1] - oy, p[2] - ox] == f[oz + 2, oy + 1, ox + 3]
+    assert np.count_nonzero(c) == np.count_nonzero(f)
+
+
+def test_G3_general_against_scipy_correlate(oracle):
+    """Library special case: scipy.ndimage.correlate(mode='constant') is Eq. 2 with zero padding."""
+    rng = np.random.default_rng(23)
+    d = rng.standard_normal((12, 10, 15)).astype(np.float32)
+    f = rng.standard_normal((7, 5, 3))
+    ref = ndi.correlate(d.astype(np.float64), f, mode="constant", cval=0.0)
+    a = oracle.filter_general(d, f)
+    assert np.max(np.abs(a - ref)) <= 1e-13
+    # a radius larger than the cube along z
+    f2 = rng.standard_normal((29, 1, 3))
+    ref2 = ndi.correlate(d.astype(np.float64), f2, mode="constant", cval=0.0)
+    assert np.max(np.abs(oracle.filter_general(d, f2) - ref2)) <= 1e-13
