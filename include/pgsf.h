@@ -121,6 +121,20 @@ PGSF_API pgsf_status pgsf_filter3d(pgsf_plan *plan, int scale, const float *d_in
                           void *d_workspace, void *cuda_stream);
 
 /*
+ * pgsf_filter3d_direct -- Eq. 2 (Eq. 3-5) for an ARBITRARY filter by direct summation, the
+ * operation of the paper's own kernel:
+ *     d_out[x,y,z] = sum_ox sum_oy sum_oz d_in[x+ox, y+oy, z+oz] f[ox][oy][oz],   |ox| <= rx, |oy| <= ry, |oz| <= rz,
+ * a correlation as printed (C-4), input outside the cube = 0 (C-5).  d_filter: DEVICE array of
+ * (2rz+1)*(2ry+1)*(2rx+1) floats, index (ox+rx) + (2rx+1)*((oy+ry) + (2ry+1)*(oz+rz)) (x fastest, like the
+ * cubes).  flags: PGSF_DIRECT_FP64_ACCUM accumulates in double as the paper does; default fp32.
+ * Uses only the plan's extents, batch and device (not its scales); needs no workspace.  d_in, d_out as for
+ * pgsf_filter3d.  UNSUPPORTED when the staged slab of 64 + 2rz channels x 64 + 2rx columns exceeds shared memory.
+ */
+#define PGSF_DIRECT_FP64_ACCUM 0x1u
+PGSF_API pgsf_status pgsf_filter3d_direct(pgsf_plan *plan, const float *d_filter, int rx, int ry, int rz,
+                                          const float *d_in, float *d_out, unsigned flags, void *cuda_stream);
+
+/*
  * pgsf_filter3d_weighted -- Eq. 1, the weighted convolution, for the Gaussian of scale `scale`
  * (reading C-16 of DESIGN.md).  With i = (x+ox, y+oy, z+oz) over the part of the
  * filter support inside the cube:

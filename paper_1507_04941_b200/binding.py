@@ -20,13 +20,14 @@ PGSF_FLAG_FORCE_GENERIC = 0x1
 PGSF_FLAG_SMALL_GROUPS = 0x2
 PGSF_WEIGHTED_AS_PRINTED = 0
 PGSF_WEIGHTED_NORMALISED = 1
+PGSF_DIRECT_FP64_ACCUM = 0x1
 PGSF_MAX_SCALES = 8
 PGSF_MAX_RADIUS = 96
 _STATUS = {0: "PGSF_OK", 1: "PGSF_ERR_INVALID_ARG", 2: "PGSF_ERR_UNSUPPORTED", 3: "PGSF_ERR_OOM",
            4: "PGSF_ERR_CUDA"}
 
 EXPORTS = ["pgsf_plan_create", "pgsf_plan_destroy", "pgsf_plan_workspace_bytes", "pgsf_last_error",
-           "pgsf_plan_get_taps", "pgsf_filter3d", "pgsf_filter3d_weighted", "pgsf_local_threshold", "pgsf_find_multiscale",
+           "pgsf_plan_get_taps", "pgsf_filter3d", "pgsf_filter3d_weighted", "pgsf_filter3d_direct", "pgsf_local_threshold", "pgsf_find_multiscale",
            "pgsf_find_multiscale_host", "pgsf_plan_launch_count", "pgsf_plan_set_profiling",
            "pgsf_plan_profile_collect", "pgsf_plan_profile_entry"]
 
@@ -71,6 +72,8 @@ def load_library() -> ctypes.CDLL:
         lib.pgsf_filter3d.restype = i
         lib.pgsf_filter3d_weighted.argtypes = [vp, i, vp, vp, vp, i, vp, vp]
         lib.pgsf_filter3d_weighted.restype = i
+        lib.pgsf_filter3d_direct.argtypes = [vp, vp, i, i, i, vp, vp, ctypes.c_uint, vp]
+        lib.pgsf_filter3d_direct.restype = i
         lib.pgsf_local_threshold.argtypes = [vp, vp, vp, i, vp, vp, vp, vp, vp]
         lib.pgsf_local_threshold.restype = i
         lib.pgsf_find_multiscale.argtypes = [vp, vp, ctypes.POINTER(vp), vp, vp, vp, vp]
@@ -220,6 +223,21 @@ class Plan:
         ws = self.workspace()
         self._check(self._lib.pgsf_filter3d_weighted(self._h, int(scale), _ptr(d_in), _ptr(d_w), _ptr(d_out),
                                                      int(mode), _ptr(ws), _stream_ptr(stream)))
+        return d_out
+
+    def pgsf_filter3d_direct(self, d_filter: torch.Tensor, d_in: torch.Tensor, fp64_accum: bool = False,
+                             d_out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+        """Eq. 2 for an arbitrary filter array d_filter[fz, fy, fx] (odd extents, fp32, on the device)."""
+        self._check_cube(d_in, torch.float32, "d_in")
+        if d_filter.dtype != torch.float32 or d_filter.dim() != 3 or not d_filter.is_contiguous() or \
+                any(n % 2 == 0 for n in d_filter.shape) or d_filter.device != d_in.device:
+            raise ValueError("d_filter: contiguous fp32 [fz, fy, fx] with odd extents on the cube's device")
+        if d_out is None:
+            d_out = torch.empty_like(d_in)
+        self._check_cube(d_out, torch.float32, "d_out")
+        rz, ry, rx = [(n - 1) // 2 for n in d_filter.shape]
+        self._check(self._lib.pgsf_filter3d_direct(self._h, _ptr(d_filter), rx, ry, rz, _ptr(d_in), _ptr(d_out),
+                                                   PGSF_DIRECT_FP64_ACCUM if fp64_accum else 0, _stream_ptr(stream)))
         return d_out
 
     def pgsf_local_threshold(self, d_filtered: torch.Tensor, d_mask: Optional[torch.Tensor] = None,

@@ -411,6 +411,33 @@ pgsf_status pgsf_filter3d_weighted(pgsf_plan *p, int scale, const float *d_in, c
     return PGSF_OK;
 }
 
+pgsf_status pgsf_filter3d_direct(pgsf_plan *p, const float *d_filter, int rx, int ry, int rz, const float *d_in,
+                                 float *d_out, unsigned flags, void *stream)
+{
+    if (!p) return PGSF_ERR_INVALID_ARG;
+    if (!d_filter || !d_in || !d_out) return fail(p, PGSF_ERR_INVALID_ARG, "NULL pointer");
+    if (rx < 0 || ry < 0 || rz < 0) return fail(p, PGSF_ERR_INVALID_ARG, "radii must be >= 0");
+    if (flags & ~(unsigned)PGSF_DIRECT_FP64_ACCUM) return fail(p, PGSF_ERR_INVALID_ARG, "unknown flag");
+    if (!aligned16(d_in) || !aligned16(d_out) || (reinterpret_cast<uintptr_t>(d_filter) & 3u))
+        return fail(p, PGSF_ERR_INVALID_ARG, "cube pointers must be 16-byte, the filter 4-byte aligned");
+    const size_t bytes = (size_t)p->dims.cube * p->desc.batch * sizeof(float);
+    const char *a = reinterpret_cast<const char *>(d_in), *b = reinterpret_cast<const char *>(d_out);
+    if (a < b + bytes && b < a + bytes) return fail(p, PGSF_ERR_INVALID_ARG, "d_out overlaps d_in");
+    int smem = 0;
+    if (!pgsf::direct_supported(p, rx, ry, rz, &smem))
+        return fail(p, PGSF_ERR_UNSUPPORTED, "filter radii (%d, %d, %d) need %d bytes of shared memory or exceed %d",
+                    rx, ry, rz, smem, PGSF_MAX_RADIUS);
+    cudaError_t e = cudaSetDevice(p->device);
+    if (e != cudaSuccess) return cuda_fail(p, e, "cudaSetDevice");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    for (int bi = 0; bi < p->desc.batch; ++bi) {
+        const size_t off = (size_t)bi * p->dims.cube;
+        e = pgsf::direct_filter3d(p, d_filter, rx, ry, rz, d_in + off, d_out + off, (flags & PGSF_DIRECT_FP64_ACCUM) != 0, st);
+        if (e != cudaSuccess) return cuda_fail(p, e, "direct filter launch");
+    }
+    return PGSF_OK;
+}
+
 pgsf_status pgsf_local_threshold(pgsf_plan *p, const float *d_f, uint8_t *d_mask, int or_into,
                                  float *d_mean, float *d_std, unsigned long long *d_count, void *d_ws,
                                  void *stream)

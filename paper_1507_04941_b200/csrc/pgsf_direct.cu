@@ -1,0 +1,169 @@
+// Eq. 2 (index ranges Eq. 3-5) for an ARBITRARY, non-separable filter f[oz][oy][ox] by direct
+// summation -- the operation the paper's own kernel performs, with fp32 or,
+// as in the paper, fp64 accumulators.
+//
+// k_direct: one CTA = 64 columns x 64 channels of one row y.  For every filter row oy the CTA stages the slab
+// of 64 + 2 rz channels x (64 + 2 rx) columns of input row y + oy in shared memory (zero fill outside the
+// cube, C-5) together with that row's taps; then, for every ox, each thread walks along z with 4 columns x 8
+// channels of accumulators in registers (the register-march of k_z): per staged channel 4 shared-memory words
+// and 16 FFMA2, the 15 taps a block of 8 channels needs held in registers.  Where the paper re-reads a z line
+// per (ox, oy) and does one multiply-add per shared-memory read, this does 8.
+#include "pgsf_internal.h"
+#include "pgsf_device.cuh"
+
+namespace pgsf {
+namespace {
+
+constexpr int DR_XT = 64;                 // columns per CTA
+constexpr int DR_PZ = 8;                  // channels per thread
+constexpr int DR_GROUPS = 8;              // groups of 8 channels
+constexpr int DR_ZB = DR_PZ * DR_GROUPS;  // 64 channels per CTA
+constexpr int DR_LX = DR_XT / 4;          // 16 lanes per channel row
+constexpr int DR_THREADS = DR_LX * DR_GROUPS;
+
+struct DirectShape {
+    int rxp;     // rx rounded up to a multiple of 4 (16-byte aligned staging)
+    int sw;      // staged columns = 64 + 2 rxp
+    int nj;      // channels walked per thread = 8 + 2 rz rounded up to a multiple of 8
+    int planes;  // staged channels = 56 + nj (>= 64 + 2 rz; the surplus is zero filled)
+    int tlen;    // padded taps per ox = nj + 8
+    int smem_bytes(int rx) const { return (planes * sw + (2 * rx + 1) * tlen) * (int)sizeof(float); }
+};
+
+DirectShape direct_shape(int rx, int rz)
+{
+    DirectShape s;
+    s.rxp = (rx + 3) & ~3;
+    s.sw = DR_XT + 2 * s.rxp;
+    s.nj = (DR_PZ + 2 * rz + 7) & ~7;
+    s.planes = DR_ZB - DR_PZ + s.nj;
+    s.tlen = s.nj + 8;
+    return s;
+}
+
+template <bool F64>
+__global__ void __launch_bounds__(DR_THREADS) k_direct(const float *__restrict__ in, float *__restrict__ out,
+                                                        const float *__restrict__ filt, Dims d, int rx, int ry,
+                                                        int rz, DirectShape sh)
+{
+    extern __shared__ __align__(16) float dr_smem[];
+    float *slab = dr_smem;                              // [planes][sw]
+    float *taps = dr_smem + sh.planes * sh.sw;          // [2 rx + 1][tlen]: tap of channel offset o at [8 + o + rz]
+    const int tid = threadIdx.x, lx = tid % DR_LX, wz = tid / DR_LX;
+    const int z0 = blockIdx.x * DR_ZB, x0 = blockIdx.y * DR_XT, y = blockIdx.z;
+    const int fx = 2 * rx + 1, fy = 2 * ry + 1, fz = 2 * rz + 1;
+    const bool vec = (d.nx & 3) == 0;                   // rows are 16-byte aligned
+
+    using acc_t = typename std::conditional<F64, double, float>::type;
+    acc_t acc[DR_PZ][4];
+#pragma unroll
+    for (int p = 0; p < DR_PZ; ++p) acc[p][0] = acc[p][1] = acc[p][2] = acc[p][3] = (acc_t)0;
+
+    for (int oy = -ry; oy <= ry; ++oy) {
+        const int yy = y + oy;
+        if (yy < 0 || yy >= d.ny) continue;             // (uniform over the CTA)
+        __syncthreads();                                // the previous row's slab and taps are no longer read
+        // slab: channels z0 - rz .. , columns x0 - rxp .. of row yy; zero outside the cube and in the surplus
+        const float *row = in + (long long)yy * d.nx;
+        if (vec) {
+            const int cpr = sh.sw / 4;                  // 16-byte chunks per staged channel row
+            for (int q = tid; q < sh.planes * cpr; q += DR_THREADS) {
+                const int pz = q / cpr, ch = q - pz * cpr;
+                const int gz = z0 - rz + pz, gx = x0 - sh.rxp + 4 * ch;
+                const bool ok = pz < DR_ZB + 2 * rz && gz >= 0 && gz < d.nz && gx >= 0 && gx < d.nx;
+                cp_async16(slab + pz * sh.sw + 4 * ch, ok ? row + (long long)gz * d.plane + gx : in, ok);
+            }
+        } else {
+            for (int q = tid; q < sh.planes * sh.sw; q += DR_THREADS) {
+                const int pz = q / sh.sw, c = q - pz * sh.sw;
+                const int gz = z0 - rz + pz, gx = x0 - sh.rxp + c;
+                const bool ok = pz < DR_ZB + 2 * rz && gz >= 0 && gz < d.nz && gx >= 0 && gx < d.nx;
+                slab[q] = ok ? __ldg(row + (long long)gz * d.plane + gx) : 0.f;
+            }
+        }
+        // taps of filter row oy: taps[ox][8 + o] = f[o][oy][ox], o = oz + rz; zero padding on both sides
+        for (int q = tid; q < fx * sh.tlen; q += DR_THREADS) {
+            const int ix = q / sh.tlen, i = q - ix * sh.tlen;
+            const int o = i - 8;
+            taps[q] = (o >= 0 && o < fz) ? __ldg(filt + ((long long)o * fy + (oy + ry)) * fx + ix) : 0.f;
+        }
+        cp_async_wait_all();
+        __syncthreads();
+
+        for (int ix = 0; ix < fx; ++ix) {
+            // data of output column c and channel offset o sits at slab[(channel - z0 + rz + o)][c + rxp + ox]
+            const float *base = slab + (wz * DR_PZ) * sh.sw + sh.rxp + 4 * lx + (ix - rx);
+            const float *tv = taps + ix * sh.tlen;
+#pragma unroll 1
+            for (int jc = 0; jc < sh.nj; jc += 8) {
+                float tw[16];                           // taps jc .. jc + 15 of the padded vector
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const float4 t4 = *reinterpret_cast<const float4 *>(tv + jc + 4 * i);
+                    tw[4 * i] = t4.x; tw[4 * i + 1] = t4.y; tw[4 * i + 2] = t4.z; tw[4 * i + 3] = t4.w;
+                }
+#pragma unroll
+                for (int jj = 0; jj < 8; ++jj) {
+                    const float *pv = base + (jc + jj) * sh.sw;
+                    const float v0 = pv[0], v1 = pv[1], v2 = pv[2], v3 = pv[3];
+#pragma unroll
+                    for (int p = 0; p < DR_PZ; ++p) {
+                        const float g = tw[jj - p + 8];  // tap of channel offset (jc + jj) - p - rz
+                        if constexpr (F64) {
+                            acc[p][0] += (double)v0 * (double)g; acc[p][1] += (double)v1 * (double)g;
+                            acc[p][2] += (double)v2 * (double)g; acc[p][3] += (double)v3 * (double)g;
+                        } else {
+                            acc[p][0] = fmaf(v0, g, acc[p][0]); acc[p][1] = fmaf(v1, g, acc[p][1]);
+                            acc[p][2] = fmaf(v2, g, acc[p][2]); acc[p][3] = fmaf(v3, g, acc[p][3]);
+                        }
+                    }
+                }
+            }
+        }
+    }
+
+    const int gx = x0 + 4 * lx;
+    if (gx >= d.nx) return;
+    float *col = out + (long long)y * d.nx + gx;
+#pragma unroll
+    for (int p = 0; p < DR_PZ; ++p) {
+        const int gz = z0 + wz * DR_PZ + p;
+        if (gz >= d.nz) break;
+        float *o = col + (long long)gz * d.plane;
+        if (vec) {
+            *reinterpret_cast<float4 *>(o) = make_float4((float)acc[p][0], (float)acc[p][1], (float)acc[p][2], (float)acc[p][3]);
+        } else {
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+                if (gx + c < d.nx) o[c] = (float)acc[p][c];
+        }
+    }
+}
+
+}  // namespace
+
+bool direct_supported(const pgsf_plan *p, int rx, int ry, int rz, int *smem)
+{
+    if (rx < 0 || ry < 0 || rz < 0 || rx > PGSF_MAX_RADIUS || ry > PGSF_MAX_RADIUS || rz > PGSF_MAX_RADIUS) return false;
+    const DirectShape sh = direct_shape(rx, rz);
+    *smem = sh.smem_bytes(rx);
+    return *smem <= 200 * 1024 && p->dims.ny <= 65535 && (p->dims.nx + DR_XT - 1) / DR_XT <= 65535;
+}
+
+// one cube per call
+cudaError_t direct_filter3d(pgsf_plan *p, const float *filt, int rx, int ry, int rz, const float *in, float *out,
+                            bool fp64, cudaStream_t st)
+{
+    const Dims &d = p->dims;
+    const DirectShape sh = direct_shape(rx, rz);
+    const int smem = sh.smem_bytes(rx);
+    cudaError_t e = fp64 ? ensure_dynamic_smem(k_direct<true>, smem) : ensure_dynamic_smem(k_direct<false>, smem);
+    if (e != cudaSuccess) return e;
+    dim3 grid((d.nz + DR_ZB - 1) / DR_ZB, (d.nx + DR_XT - 1) / DR_XT, d.ny);
+    LaunchScope ls(p, fp64 ? "direct_f64" : "direct_f32", st);
+    if (fp64) k_direct<true><<<grid, DR_THREADS, smem, st>>>(in, out, filt, d, rx, ry, rz, sh);
+    else k_direct<false><<<grid, DR_THREADS, smem, st>>>(in, out, filt, d, rx, ry, rz, sh);
+    return cudaGetLastError();
+}
+
+}  // namespace pgsf

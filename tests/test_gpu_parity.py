@@ -176,6 +176,47 @@ def test_weighted_unit_weights_reproduce_filter3d(pg, synth):
     assert float((ai - bi).abs().max()) <= 2e-6
 
 
+# ------------------------------------------------------------------------------------ Eq. 2, arbitrary filter (NEXT-2)
+
+@pytest.mark.parametrize("fp64", [False, True])
+@pytest.mark.parametrize("dims,fshape", [
+    ((64, 64, 128), (13, 7, 7)),        # config 1 cube, the extents of its sigma (1,1,2) filter, random taps
+    ((100, 52, 77), (5, 3, 9)),         # ragged cube, unequal radii (rz=2, ry=1, rx=4)
+    ((30, 17, 9), (21, 1, 3)),          # nx % 4 != 0 (scalar staging), rz = 10 larger than nz
+    ((72, 20, 150), (1, 5, 1)),         # a filter along y only
+])
+def test_direct_general_filter(pg, synth, oracle, dims, fshape, fp64):
+    """pgsf_filter3d_direct against the oracle's Eq. 2 for an asymmetric random filter (correlation
+    orientation, zero padding), element by element; fp32 and fp64 accumulation."""
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[1], dims, n_sources=4))
+    d = synth.make_workload(w, "cuda")
+    rng = np.random.default_rng(77)
+    f = rng.standard_normal(fshape).astype(np.float32)
+    f /= np.abs(f).sum()                                         # |f|_1 = 1: outputs O(1) like the Gaussian path
+    with _plan(pg, w) as plan:
+        out = plan.pgsf_filter3d_direct(torch.from_numpy(f).cuda(), d, fp64_accum=fp64)
+        torch.cuda.synchronize()
+    ref = oracle.filter_general(d[0].cpu().numpy(), f.astype(np.float64))
+    diff = parity.assert_filter_close(out[0].cpu().numpy(), ref, f"direct filter fp64={fp64}")
+    if fp64:
+        assert diff <= 2e-7          # only the final rounding to fp32 remains
+
+
+def test_direct_equals_separable_for_gaussian(pg, synth, oracle):
+    """The paper's direct kernel and the separable path agree for the outer-product Gaussian (config 1)."""
+    w = synth.WORKLOADS[1]
+    d = synth.make_workload(w, "cuda")
+    g = [oracle.taps(s) for s in w.sigmas[0]]
+    f = (g[2][:, None, None] * g[1][None, :, None] * g[0][None, None, :]).astype(np.float32)
+    with _plan(pg, w) as plan:
+        a = plan.pgsf_filter3d(0, d)
+        b = plan.pgsf_filter3d_direct(torch.from_numpy(f).cuda(), d)
+        torch.cuda.synchronize()
+    # both are within FILTER_TOL of Eq. 2; the fp32 rounding of the 637 products gz gy gx adds ~3e-6 here
+    assert float((a - b).abs().max()) <= parity.FILTER_TOL
+
+
 # ------------------------------------------------------------------------------------ degenerate cases
 
 @pytest.mark.parametrize("flags", IMPLS)
