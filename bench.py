@@ -540,6 +540,101 @@ def run_weighted(args, w):
     print(json.dumps(line), flush=True)
 
 
+# ------------------------------------------------------------------------------------ Eq. 2 direct (NEXT-2)
+
+D_METRIC = "Gvoxel/s (direct 3-D filter, Eq. 2, arbitrary taps)"
+D_SAMPLE = (96, 96, 96)
+
+
+def run_direct(args, w):
+    """--path direct: one step = pgsf_filter3d_direct over the config's cube with the (2rz+1)(2ry+1)(2rx+1)
+    taps of its FIRST scale as a general filter array (fp32 accumulation; --fp64 for the paper's fp64).
+    Single GPU.  Same JSON contract as the main path."""
+    import numpy as np
+    import torch
+    from paper_1507_04941_b200 import binding, build, synth
+    from oracle import pgsf_oracle
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a B200: the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    build.build()
+    binding.load_library()
+    props = torch.cuda.get_device_properties(0)
+    peaks = _peaks()
+    d = synth.make_workload(w, "cuda:0")
+    g = [pgsf_oracle.taps(sg, w.truncate) for sg in w.sigmas[0]]
+    f = (g[2][:, None, None] * g[1][None, :, None] * g[0][None, None, :]).astype(np.float32)
+    d_f = torch.from_numpy(f).cuda()
+    ntaps = f.size
+    plan = binding.Plan(w.dims, w.sigmas, w.box_half, w.k, batch=w.batch, halo=w.halo, truncate=w.truncate)
+    out = torch.empty_like(d)
+    stream = torch.cuda.current_stream()
+    step = lambda: plan.pgsf_filter3d_direct(d_f, d, fp64_accum=args.fp64, d_out=out, stream=stream)
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    l0 = plan.pgsf_plan_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    ms_step = ev0.elapsed_time(ev1) / args.steps
+    launches = plan.pgsf_plan_launch_count() - l0
+    clocks = sampler.stop()
+    n_vox = w.voxels
+    alu_peak = _alu_peak_tflops(props.multi_processor_count, peaks["sm_max_mhz"]) * (0.5 if args.fp64 else 1.0)
+    flops = 2.0 * ntaps * n_vox
+    ach = flops / (ms_step * 1e-3) / 1e12
+    roofline = {"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak,
+                "kernel": "direct_f64" if args.fp64 else "direct_f32", "ms_per_launch": ms_step / max(w.batch, 1),
+                "share_of_step": 1.0, "traffic": None,
+                "peak_source": "148 SM x 128 lanes x 2 x sm_max_mhz" + (" / 2 (fp64)" if args.fp64 else "")}
+    e2e = None
+    if not args.no_e2e:
+        h_d = torch.empty(d.shape, dtype=torch.float32, pin_memory=True).copy_(d)
+        h_o = torch.empty(d.shape, dtype=torch.float32, pin_memory=True)
+        steps = max(1, min(args.steps, 3))
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            d.copy_(h_d, non_blocking=True)
+            step()
+            h_o.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+        sec_e = (time.perf_counter() - t0) / steps
+        e2e = {"value": n_vox / sec_e / 1e9, "unit": "Gvoxel/s", "ms_per_step": sec_e * 1e3, "steps": steps,
+               "h2d_bytes_per_step": 4 * n_vox, "d2h_bytes_per_step": 4 * n_vox,
+               "api": "binding.Plan.pgsf_filter3d_direct on a pinned host cube (torch copies)"}
+    cpu = None
+    if not args.no_cpu_baseline:
+        lo = [max(0, (n - sz) // 2) for n, sz in zip(w.dims, D_SAMPLE)]
+        hi = [min(n, l + sz) for n, l, sz in zip(w.dims, lo, D_SAMPLE)]
+        sd = d[0, lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]].cpu().numpy()
+        plan.close()
+        threads = pgsf_oracle.set_threads(0)
+        t0 = time.perf_counter()
+        pgsf_oracle.filter_general(sd, f.astype(np.float64))
+        dt = time.perf_counter() - t0
+        cpu = {"value": sd.size / dt / 1e9, "unit": "Gvoxel/s", "cores": threads, "kind": "oracle", "seconds": dt,
+               "sample": f"centred brick {sd.shape[2]}x{sd.shape[1]}x{sd.shape[0]} of {w.name} taken as a standalone "
+                         f"cube, the same {ntaps} taps, oracle Eq. 2 by direct loops (fp64)"}
+    line = {"metric": D_METRIC, "value": n_vox / (ms_step * 1e-3) / 1e9, "unit": "Gvoxel/s", "n_gpus": 1,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.fp64 else "f32", "data": "synthetic",
+            "config": {"workload": w.name, "path": "direct (Eq. 2, arbitrary filter array)",
+                       "filter_extent_xyz": [f.shape[2], f.shape[1], f.shape[0]], "taps": int(ntaps),
+                       "l2": "inputs larger than L2" if n_vox * 4 > 2**28 else "inputs fit L2 (small config)"},
+            "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline,
+            "path_roofline": {"flops_per_voxel": 2.0 * ntaps, "bytes_per_voxel": 8.0,
+                              "roofline_ms": flops / (alu_peak * 1e12) * 1e3,
+                              "frac": flops / (alu_peak * 1e12) * 1e3 / ms_step},
+            "e2e": e2e, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -548,8 +643,10 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5],
                     help="BASELINE.json config (1-based); default 3 = the 8 GiB cube the north star is quoted on")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--path", default="find", choices=["find", "weighted"],
-                    help="find = the hot path (default); weighted = Eq. 1 of the paper (NEXT-1), single GPU")
+    ap.add_argument("--path", default="find", choices=["find", "weighted", "direct"],
+                    help="find = the hot path (default); weighted = Eq. 1 of the paper (NEXT-1); direct = Eq. 2 for "
+                         "an arbitrary filter array (NEXT-2); the last two single GPU")
+    ap.add_argument("--fp64", action="store_true", help="--path direct: accumulate in fp64 as the paper does")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -559,9 +656,9 @@ def main():
     if args.impl == "reference":
         run_reference(args, w)
         return
-    if args.path == "weighted":
+    if args.path in ("weighted", "direct"):
         if int(os.environ.get("RANK", "0")) == 0:
-            run_weighted(args, w)
+            (run_weighted if args.path == "weighted" else run_direct)(args, w)
         return
     line, ctx = run_b200(args, w)
     rank, world = ctx["rank"], ctx["world"]

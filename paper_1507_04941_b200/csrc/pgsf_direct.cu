@@ -2,11 +2,12 @@
 // summation -- the operation the paper's own kernel performs, with fp32 or,
 // as in the paper, fp64 accumulators.
 //
-// k_direct: one CTA = 64 columns x 64 channels of one row y.  For every filter row oy the CTA stages the slab
-// of 64 + 2 rz channels x (64 + 2 rx) columns of input row y + oy in shared memory (zero fill outside the
+// k_direct: one CTA = 128 columns x 64 channels of one row y.  For every filter row oy the CTA stages the slab
+// of 64 + 2 rz channels x (128 + 2 rx) columns of input row y + oy in shared memory (zero fill outside the
 // cube, C-5) together with that row's taps; then, for every ox, each thread walks along z with 4 columns x 8
 // channels of accumulators in registers (the register-march of k_z): per staged channel 4 shared-memory words
-// and 16 FFMA2, the 15 taps a block of 8 channels needs held in registers.  Where the paper re-reads a z line
+// (a lane's columns are 32 apart, so every load is one conflict-free wavefront) and 16 FFMA2, the 15 taps a
+// block of 8 channels needs held in registers.  Where the paper re-reads a z line
 // per (ox, oy) and does one multiply-add per shared-memory read, this does 8.
 #include "pgsf_internal.h"
 #include "pgsf_device.cuh"
@@ -14,16 +15,16 @@
 namespace pgsf {
 namespace {
 
-constexpr int DR_XT = 64;                 // columns per CTA
+constexpr int DR_XT = 128;                // columns per CTA: lane l owns columns l, l + 32, l + 64, l + 96
 constexpr int DR_PZ = 8;                  // channels per thread
-constexpr int DR_GROUPS = 8;              // groups of 8 channels
+constexpr int DR_GROUPS = 8;              // groups of 8 channels = warps
 constexpr int DR_ZB = DR_PZ * DR_GROUPS;  // 64 channels per CTA
-constexpr int DR_LX = DR_XT / 4;          // 16 lanes per channel row
+constexpr int DR_LX = 32;                 // one warp per channel group
 constexpr int DR_THREADS = DR_LX * DR_GROUPS;
 
 struct DirectShape {
     int rxp;     // rx rounded up to a multiple of 4 (16-byte aligned staging)
-    int sw;      // staged columns = 64 + 2 rxp
+    int sw;      // staged columns = 128 + 2 rxp
     int nj;      // channels walked per thread = 8 + 2 rz rounded up to a multiple of 8
     int planes;  // staged channels = 56 + nj (>= 64 + 2 rz; the surplus is zero filled)
     int tlen;    // padded taps per ox = nj + 8
@@ -55,9 +56,13 @@ __global__ void __launch_bounds__(DR_THREADS) k_direct(const float *__restrict__
     const bool vec = (d.nx & 3) == 0;                   // rows are 16-byte aligned
 
     using acc_t = typename std::conditional<F64, double, float>::type;
-    acc_t acc[DR_PZ][4];
+    acc_t acc[DR_PZ][4];                                // fp64 path
+    float2 a2[DR_PZ][2];                                // fp32 path: (columns 0, 1) and (2, 3) of the lane as FFMA2 pairs
 #pragma unroll
-    for (int p = 0; p < DR_PZ; ++p) acc[p][0] = acc[p][1] = acc[p][2] = acc[p][3] = (acc_t)0;
+    for (int p = 0; p < DR_PZ; ++p) {
+        acc[p][0] = acc[p][1] = acc[p][2] = acc[p][3] = (acc_t)0;
+        a2[p][0] = a2[p][1] = make_float2(0.f, 0.f);
+    }
 
     for (int oy = -ry; oy <= ry; ++oy) {
         const int yy = y + oy;
@@ -92,7 +97,7 @@ __global__ void __launch_bounds__(DR_THREADS) k_direct(const float *__restrict__
 
         for (int ix = 0; ix < fx; ++ix) {
             // data of output column c and channel offset o sits at slab[(channel - z0 + rz + o)][c + rxp + ox]
-            const float *base = slab + (wz * DR_PZ) * sh.sw + sh.rxp + 4 * lx + (ix - rx);
+            const float *base = slab + (wz * DR_PZ) * sh.sw + sh.rxp + lx + (ix - rx);
             const float *tv = taps + ix * sh.tlen;
 #pragma unroll 1
             for (int jc = 0; jc < sh.nj; jc += 8) {
@@ -105,7 +110,7 @@ __global__ void __launch_bounds__(DR_THREADS) k_direct(const float *__restrict__
 #pragma unroll
                 for (int jj = 0; jj < 8; ++jj) {
                     const float *pv = base + (jc + jj) * sh.sw;
-                    const float v0 = pv[0], v1 = pv[1], v2 = pv[2], v3 = pv[3];
+                    const float v0 = pv[0], v1 = pv[32], v2 = pv[64], v3 = pv[96];
 #pragma unroll
                     for (int p = 0; p < DR_PZ; ++p) {
                         const float g = tw[jj - p + 8];  // tap of channel offset (jc + jj) - p - rz
@@ -113,8 +118,8 @@ __global__ void __launch_bounds__(DR_THREADS) k_direct(const float *__restrict__
                             acc[p][0] += (double)v0 * (double)g; acc[p][1] += (double)v1 * (double)g;
                             acc[p][2] += (double)v2 * (double)g; acc[p][3] += (double)v3 * (double)g;
                         } else {
-                            acc[p][0] = fmaf(v0, g, acc[p][0]); acc[p][1] = fmaf(v1, g, acc[p][1]);
-                            acc[p][2] = fmaf(v2, g, acc[p][2]); acc[p][3] = fmaf(v3, g, acc[p][3]);
+                            a2[p][0] = ffma2(make_float2(v0, v1), g, a2[p][0]);
+                            a2[p][1] = ffma2(make_float2(v2, v3), g, a2[p][1]);
                         }
                     }
                 }
@@ -122,20 +127,23 @@ __global__ void __launch_bounds__(DR_THREADS) k_direct(const float *__restrict__
         }
     }
 
-    const int gx = x0 + 4 * lx;
-    if (gx >= d.nx) return;
-    float *col = out + (long long)y * d.nx + gx;
+    float *rowo = out + (long long)y * d.nx;
 #pragma unroll
     for (int p = 0; p < DR_PZ; ++p) {
         const int gz = z0 + wz * DR_PZ + p;
         if (gz >= d.nz) break;
-        float *o = col + (long long)gz * d.plane;
-        if (vec) {
-            *reinterpret_cast<float4 *>(o) = make_float4((float)acc[p][0], (float)acc[p][1], (float)acc[p][2], (float)acc[p][3]);
-        } else {
+        float *o = rowo + (long long)gz * d.plane;
+        float v[4];
+        if constexpr (F64) {
 #pragma unroll
-            for (int c = 0; c < 4; ++c)
-                if (gx + c < d.nx) o[c] = (float)acc[p][c];
+            for (int c = 0; c < 4; ++c) v[c] = (float)acc[p][c];
+        } else {
+            v[0] = a2[p][0].x; v[1] = a2[p][0].y; v[2] = a2[p][1].x; v[3] = a2[p][1].y;
+        }
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int gx = x0 + lx + 32 * c;
+            if (gx < d.nx) o[gx] = v[c];
         }
     }
 }
