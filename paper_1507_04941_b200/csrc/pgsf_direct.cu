@@ -70,28 +70,31 @@ __global__ void __launch_bounds__(DR_THREADS) k_direct(const float *__restrict__
         __syncthreads();                                // the previous row's slab and taps are no longer read
         // slab: channels z0 - rz .. , columns x0 - rxp .. of row yy; zero outside the cube and in the surplus
         const float *row = in + (long long)yy * d.nx;
-        if (vec) {
-            const int cpr = sh.sw / 4;                  // 16-byte chunks per staged channel row
-            for (int q = tid; q < sh.planes * cpr; q += DR_THREADS) {
-                const int pz = q / cpr, ch = q - pz * cpr;
-                const int gz = z0 - rz + pz, gx = x0 - sh.rxp + 4 * ch;
-                const bool ok = pz < DR_ZB + 2 * rz && gz >= 0 && gz < d.nz && gx >= 0 && gx < d.nx;
-                cp_async16(slab + pz * sh.sw + 4 * ch, ok ? row + (long long)gz * d.plane + gx : in, ok);
-            }
-        } else {
-            for (int q = tid; q < sh.planes * sh.sw; q += DR_THREADS) {
-                const int pz = q / sh.sw, c = q - pz * sh.sw;
-                const int gz = z0 - rz + pz, gx = x0 - sh.rxp + c;
-                const bool ok = pz < DR_ZB + 2 * rz && gz >= 0 && gz < d.nz && gx >= 0 && gx < d.nx;
-                slab[q] = ok ? __ldg(row + (long long)gz * d.plane + gx) : 0.f;
+        // (warp wz takes every 8th staged channel, its lanes stride along the row: no integer divisions)
+        for (int pz = wz; pz < sh.planes; pz += DR_GROUPS) {
+            const int gz = z0 - rz + pz;
+            const bool pok = pz < DR_ZB + 2 * rz && gz >= 0 && gz < d.nz;
+            const float *src = row + (long long)(pok ? gz : 0) * d.plane;
+            float *dst = slab + pz * sh.sw;
+            if (vec) {
+                for (int ch = lx; 4 * ch < sh.sw; ch += DR_LX) {
+                    const int gx = x0 - sh.rxp + 4 * ch;
+                    const bool ok = pok && gx >= 0 && gx < d.nx;
+                    cp_async16(dst + 4 * ch, ok ? src + gx : in, ok);
+                }
+            } else {
+                for (int c = lx; c < sh.sw; c += DR_LX) {
+                    const int gx = x0 - sh.rxp + c;
+                    dst[c] = (pok && gx >= 0 && gx < d.nx) ? __ldg(src + gx) : 0.f;
+                }
             }
         }
         // taps of filter row oy: taps[ox][8 + o] = f[o][oy][ox], o = oz + rz; zero padding on both sides
-        for (int q = tid; q < fx * sh.tlen; q += DR_THREADS) {
-            const int ix = q / sh.tlen, i = q - ix * sh.tlen;
-            const int o = i - 8;
-            taps[q] = (o >= 0 && o < fz) ? __ldg(filt + ((long long)o * fy + (oy + ry)) * fx + ix) : 0.f;
-        }
+        for (int ix = wz; ix < fx; ix += DR_GROUPS)
+            for (int i = lx; i < sh.tlen; i += DR_LX) {
+                const int o = i - 8;
+                taps[ix * sh.tlen + i] = (o >= 0 && o < fz) ? __ldg(filt + ((long long)o * fy + (oy + ry)) * fx + ix) : 0.f;
+            }
         cp_async_wait_all();
         __syncthreads();
 
