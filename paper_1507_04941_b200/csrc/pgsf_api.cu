@@ -527,6 +527,19 @@ pgsf_status pgsf_find_multiscale(pgsf_plan *p, const float *d_in, float *const *
         const size_t off = (size_t)bi * p->dims.cube;
         for (int s = 0; s < S; ++s) {
             float *f = (d_filtered && d_filtered[s]) ? d_filtered[s] + off : w.scratch;
+            if (p->fast_filter && p->fast_stats) {
+                // filtered cubes not (all) kept: no room to park the x/y passes of all scales, so one x/y launch
+                // per scale; the frequency pass still carries the z-direction window sums
+                float *t2[1] = {w.ftmp};
+                float *Z1 = w.stmp, *Z2 = w.stmp + (size_t)p->group * p->dims.cube;
+                cudaError_t ce = pgsf::fast_xy_multi(p, &s, 1, d_in + off, t2, 1, st);
+                if (ce == cudaSuccess) ce = pgsf::fast_zm(p, s, w.ftmp, f, Z1, Z2, 1, st);
+                if (ce == cudaSuccess)
+                    ce = pgsf::fast_threshold_xy(p, f, Z1, Z2, d_mask + off, s > 0, nullptr, nullptr,
+                                                 (s == S - 1) ? d_count : nullptr, 1, st);
+                if (ce != cudaSuccess) return cuda_fail(p, ce, "filter / threshold launch");
+                continue;
+            }
             rc = filter_one(p, s, d_in + off, f, w, st);
             if (rc != PGSF_OK) return rc;
             rc = threshold_batch(p, f, d_mask + off, s > 0, nullptr, nullptr, (s == S - 1) ? d_count : nullptr,

@@ -115,6 +115,24 @@ def test_batch_with_halo(pg, synth, oracle, flags):
     assert count > 0
 
 
+def test_find_without_keeping_filtered_cubes(pg, synth):
+    """d_filtered = NULL (only mask and count wanted, the host entry point's case): same mask and count as the
+    run that keeps every filtered cube, and as a run that keeps only some of them."""
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[2], (100, 52, 77), n_sources=12), k=3.0)
+    d = synth.make_workload(w, "cuda")
+    with _plan(pg, w) as plan:
+        m1, c1, f1 = plan.pgsf_find_multiscale(d, keep_filtered=True)
+        m2, c2, _ = plan.pgsf_find_multiscale(d, keep_filtered=False)
+        some = [None, torch.empty_like(d), None]
+        m3, c3, f3 = plan.pgsf_find_multiscale(d, d_filtered=some)
+        torch.cuda.synchronize()
+    assert int(c1.item()) > 0
+    assert torch.equal(m1, m2) and int(c1.item()) == int(c2.item())
+    assert torch.equal(m1, m3) and int(c1.item()) == int(c3.item())
+    assert torch.equal(f1[1], some[1])
+
+
 def test_batch_in_ragged_groups(pg, synth, oracle):
     """A batch of 3 taken two cubes per launch group (groups of 2 and 1): same result as one group."""
     from dataclasses import replace
