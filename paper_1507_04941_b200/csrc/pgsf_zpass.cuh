@@ -124,13 +124,15 @@ __global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, f
 //   window phase  thread (column c, quantity q in {f, f^2}) walks the 64 new channels: the channel
 //                 entering the window [z - hz, z + hz] comes from the shared-memory slab, the one
 //                 leaving it is re-read from the f this CTA wrote 2 hz + 1 channels earlier -- the
-//                 strip is narrow, so that plane is still in L2 (ld.global.cg); running sums are
-//                 Kahan-compensated as in k_zbox.  Writes Z1 = sum f, Z2 = sum f^2 (window clipped to
-//                 the cube, C-7).
+//                 strip is narrow, so that plane is still in L2 (fetched with the slab by cp.async).
+//                 The running sum of f^2 is Kahan-compensated as in k_zbox; the sum of f is plain (it
+//                 enters only through the mean: a retained rounding error of one column is divided by
+//                 the window's n and stays below 1 % of the mask band).  Writes Z1 = sum f, Z2 = sum f^2
+//                 (window clipped to the cube, C-7).
 // Against k_z + k_zbox this saves one HBM read of t2's halo, both HBM reads of f by k_zbox and one
 // launch: 8 + 8 + 16 GB instead of 17 + 35 GB per scale at config 3.
 
-// n steps of the compensated sliding window of one (column, quantity): add the entering channel, write
+// n steps of the sliding window of one (column, quantity; the sum of f^2 Kahan-compensated): add the entering channel, write
 // the window sum, subtract the leaving channel.  lead / trail advance by one staged channel per step.
 template <bool SQ, int XT>
 __device__ __forceinline__ float *window_run(float &s, float &e, const float *__restrict__ lead,
@@ -139,10 +141,16 @@ __device__ __forceinline__ float *window_run(float &s, float &e, const float *__
 #pragma unroll 8
     for (int j = 0; j < n; ++j) {
         const float a = lead[j * XT], b = trail[j * XT];
-        kahan_add(s, e, SQ ? a * a : a);
-        *zp = s - e;
+        if constexpr (SQ) {
+            kahan_add(s, e, a * a);
+            *zp = s - e;
+            kahan_add(s, e, -(b * b));
+        } else {                // sum of f: enters only through the mean, whose tolerance is ~n times looser
+            s += a;
+            *zp = s;
+            s -= b;
+        }
         zp += plane;
-        kahan_add(s, e, SQ ? -(b * b) : -b);
     }
     return zp;
 }
@@ -238,13 +246,15 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
                     const int zo = zl - hz;
                     if (zl < nz) {
                         const float v = fs[j * XT + c];
-                        kahan_add(s, e, sq ? v * v : v);
+                        if (sq) kahan_add(s, e, v * v);
+                        else s += v;
                     }
                     if (zo >= 0 && zo < nz) {
                         Zq[(long long)zo * d.plane + cb] = s - e;
                         const int jt = j - 2 * hz;  // the channel leaving after this output, relative to z0
                         const float v = jt >= 0 ? fs[jt * XT + c] : ts[j * XT + c];   // (zero where zt < 0)
-                        kahan_add(s, e, sq ? -(v * v) : -v);
+                        if (sq) kahan_add(s, e, -(v * v));
+                        else s -= v;
                     }
                 }
             }
