@@ -23,6 +23,12 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem, bool va
     const int bytes = valid ? 16 : 0;  // src-size 0 -> 16 bytes of zeros
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(gmem), "r"(bytes));
 }
+// same with the shared-memory address already converted (staging loops that step it by a constant)
+__device__ __forceinline__ void cp_async16_s(unsigned smem_addr, const void *gmem, bool valid)
+{
+    const int bytes = valid ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_addr), "l"(gmem), "r"(bytes));
+}
 __device__ __forceinline__ void cp_async_wait_all()
 {
     asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");

@@ -91,10 +91,14 @@ __global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, f
     const float *col_in = in + (long long)y * d.nx + (col_ok ? gx : 0);
 
     // stage channels z0-RZ .. z0+ZB+RZ-1 of this 128-column strip; outside the cube -> 0 (C-5)
-    for (int pz = wz; pz < S::PLANES; pz += Z_WARPS) {
-        const int gz = z0 - RZ + pz;
-        const bool ok = col_ok && gz >= 0 && gz < d.nz;
-        cp_async16(smem + pz * Z_XT + 4 * lane, ok ? col_in + (long long)gz * d.plane : in, ok);
+    {   // (running source pointer and shared-memory address: a handful of instructions per row)
+        const float *src = col_in + (long long)(z0 - RZ + wz) * d.plane;   // dereferenced only where gz is inside the cube
+        const long long step = (long long)Z_WARPS * d.plane;
+        unsigned dst = (unsigned)__cvta_generic_to_shared(smem + wz * Z_XT + 4 * lane);
+        int gz = z0 - RZ + wz;
+#pragma unroll 4
+        for (int pz = wz; pz < S::PLANES; pz += Z_WARPS, gz += Z_WARPS, src += step, dst += Z_WARPS * Z_XT * 4)
+            cp_async16_s(dst, src, col_ok && (unsigned)gz < (unsigned)d.nz);
     }
     cp_async_wait_all();
     __syncthreads();
@@ -194,24 +198,30 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
     float s = 0.f, e = 0.f;
     const int nz = d.nz;
     const int nsteps = (nz + hz + ZB - 1) / ZB;   // entering channels 0 .. nz + hz - 1 (the tail drains the window)
+    const long long gstep = (long long)S::GROUPS * d.plane;   // staging: a warp group takes every GROUPS-th channel
 
     for (int k = 0; k < nsteps; ++k) {
         const int z0 = k * ZB;
         // channels leaving the window in this step: z0 - 2 hz + j, j = 0..63.  Those written in EARLIER steps
         // (by this CTA: still in L2) are fetched now, together with the t2 slab; those of this step's own
         // f block (2 hz < 64) are read from the f slab instead.
-        for (int pz = wz; pz < ZB; pz += S::GROUPS) {
-            const int zt = z0 - 2 * hz + pz;
-            const bool ok = col_ok && zt >= 0 && zt < z0;
-            cp_async16(ts + pz * XT + 4 * lx, ok ? col_out + (long long)zt * d.plane : in, ok);
+        // (running source pointers and shared-memory addresses: a handful of instructions per staged row)
+        {
+            const float *src = col_out + (long long)(z0 - 2 * hz + wz) * d.plane;
+            unsigned dst = (unsigned)__cvta_generic_to_shared(ts + wz * XT + 4 * lx);
+            int zt = z0 - 2 * hz + wz;
+#pragma unroll 4
+            for (int pz = wz; pz < ZB; pz += S::GROUPS, zt += S::GROUPS, src += gstep, dst += S::GROUPS * XT * 4)
+                cp_async16_s(dst, src, col_ok && zt >= 0 && zt < z0);
         }
         if (z0 < nz) {
             // stage channels z0-RZ .. z0+ZB+RZ-1 of t2; outside the cube -> 0 (C-5)
-            for (int pz = wz; pz < S::PLANES; pz += S::GROUPS) {
-                const int gz = z0 - RZ + pz;
-                const bool ok = col_ok && gz >= 0 && gz < nz;
-                cp_async16(smem + pz * XT + 4 * lx, ok ? col_in + (long long)gz * d.plane : in, ok);
-            }
+            const float *src = col_in + (long long)(z0 - RZ + wz) * d.plane;
+            unsigned dst = (unsigned)__cvta_generic_to_shared(smem + wz * XT + 4 * lx);
+            int gz = z0 - RZ + wz;
+#pragma unroll 4
+            for (int pz = wz; pz < S::PLANES; pz += S::GROUPS, gz += S::GROUPS, src += gstep, dst += S::GROUPS * XT * 4)
+                cp_async16_s(dst, src, col_ok && (unsigned)gz < (unsigned)nz);
         }
         cp_async_wait_all();
         __syncthreads();
