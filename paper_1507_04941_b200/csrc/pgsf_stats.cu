@@ -364,14 +364,17 @@ cudaError_t launch_ymarch(const pgsf_plan *pl, const float *f, const float *Z1, 
     constexpr int VL = VecT<G>::L;
     const Dims &d = p.d;
     // threads: cover the whole row when it fits in one CTA, else tiles overlapping by 2 hx columns
+    // (CTAs of at most 128 threads: at 152 registers four of them share an SM, one of 256 threads would be alone)
+    constexpr int kPreferredNT = 128;
     int nt = ((d.nx + G - 1) / G + 31) / 32 * 32;
-    if (nt <= YM_MAX_NT) {
+    if (nt <= kPreferredNT) {
         p.ntiles = 1;
         p.wo = d.nx;
     } else {
-        nt = YM_MAX_NT;
-        p.wo = nt * G - 4 * G;
-        p.ntiles = (d.nx + p.wo - 1) / p.wo;
+        const int wo_max = kPreferredNT * G - 4 * G;
+        p.ntiles = (d.nx + wo_max - 1) / wo_max;
+        p.wo = ((d.nx + p.ntiles - 1) / p.ntiles + G - 1) / G * G;      // balanced tiles, whole column groups
+        nt = ((p.wo + 4 * G) / G + 31) / 32 * 32;
     }
     // y chunks: enough CTAs for a few waves; a chunk start re-reads 2 hy rows
     const long long resident = (long long)pl->sm_count * (nt <= 128 ? 4 : 2);
