@@ -1,5 +1,7 @@
 // Device helpers shared by the filter kernels (internal; not part of the ABI).
 #pragma once
+#include <mutex>
+
 #include "pgsf_internal.h"
 
 namespace pgsf {
@@ -53,6 +55,8 @@ cudaError_t ensure_dynamic_smem(K kernel, int bytes)
     struct Grant { const void *fn; int dev; int bytes; };
     static Grant table[256];
     static int used = 0;
+    static std::mutex mtx;                    // plans of different host threads share this table
+    std::lock_guard<std::mutex> lock(mtx);
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
