@@ -98,7 +98,10 @@ __global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, f
         int gz = z0 - RZ + wz;
 #pragma unroll 4
         for (int pz = wz; pz < S::PLANES; pz += Z_WARPS, gz += Z_WARPS, src += step, dst += Z_WARPS * Z_XT * 4)
-            cp_async16_s(dst, src, col_ok && (unsigned)gz < (unsigned)d.nz);
+        {
+            const bool ok = col_ok && (unsigned)gz < (unsigned)d.nz;
+            cp_async16_s(dst, ok ? src : in, ok);   // (a valid address even when nothing is read)
+        }
     }
     cp_async_wait_all();
     __syncthreads();
@@ -212,7 +215,10 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
             int zt = z0 - 2 * hz + wz;
 #pragma unroll 4
             for (int pz = wz; pz < ZB; pz += S::GROUPS, zt += S::GROUPS, src += gstep, dst += S::GROUPS * XT * 4)
-                cp_async16_s(dst, src, col_ok && zt >= 0 && zt < z0);
+            {
+                const bool ok = col_ok && zt >= 0 && zt < z0;
+                cp_async16_s(dst, ok ? src : in, ok);   // (a valid address even when nothing is read)
+            }
         }
         if (z0 < nz) {
             // stage channels z0-RZ .. z0+ZB+RZ-1 of t2; outside the cube -> 0 (C-5)
@@ -221,7 +227,10 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
             int gz = z0 - RZ + wz;
 #pragma unroll 4
             for (int pz = wz; pz < S::PLANES; pz += S::GROUPS, gz += S::GROUPS, src += gstep, dst += S::GROUPS * XT * 4)
-                cp_async16_s(dst, src, col_ok && (unsigned)gz < (unsigned)nz);
+            {
+                const bool ok = col_ok && (unsigned)gz < (unsigned)nz;
+                cp_async16_s(dst, ok ? src : in, ok);
+            }
         }
         cp_async_wait_all();
         __syncthreads();
