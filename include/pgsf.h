@@ -26,7 +26,8 @@
  * void*; NULL = the legacy default stream) and return WITHOUT synchronising; results (including
  * *d_count) are valid once the caller has synchronised the stream.  pgsf_find_multiscale_host is
  * the exception: it synchronises before returning.  One plan must not be used from two threads
- * at once.
+ * at once (different plans may).  Every compute call makes the plan's device the calling thread's
+ * current CUDA device (cudaSetDevice) and leaves it so.
  *
  * Errors: every call returns a pgsf_status; nothing throws or aborts across the ABI.  The text of
  * the last error of a plan is available from pgsf_last_error().  There is no CPU fallback: on a
