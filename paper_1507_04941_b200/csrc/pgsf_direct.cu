@@ -15,38 +15,39 @@
 namespace pgsf {
 namespace {
 
-constexpr int DR_XT = 128;                // columns per CTA: lane l owns columns l, l + 32, l + 64, l + 96
-constexpr int DR_PZ = 8;                  // channels per thread
-constexpr int DR_GROUPS = 8;              // groups of 8 channels = warps
-constexpr int DR_ZB = DR_PZ * DR_GROUPS;  // 64 channels per CTA
+// A thread owns PZ consecutive channels x NC columns (lane l: columns l, l + 32, ...); a warp is one channel
+// group, a CTA eight of them: tile = 32 NC columns x 8 PZ channels.  <PZ, NC> = <8, 4> in general; <4, 8> for
+// rz <= 8, where a walk in blocks of 8 channels x PZ outputs wastes fewer taps outside the band of 2 rz + 1.
+constexpr int DR_GROUPS = 8;              // channel groups = warps
 constexpr int DR_LX = 32;                 // one warp per channel group
 constexpr int DR_THREADS = DR_LX * DR_GROUPS;
 
 struct DirectShape {
     int rxp;     // rx rounded up to a multiple of 4 (16-byte aligned staging)
-    int sw;      // staged columns = 128 + 2 rxp
-    int nj;      // channels walked per thread = 8 + 2 rz rounded up to a multiple of 8
-    int planes;  // staged channels = 56 + nj (>= 64 + 2 rz; the surplus is zero filled)
+    int sw;      // staged columns = 32 NC + 2 rxp
+    int nj;      // channels walked per thread = PZ + 2 rz rounded up to a multiple of 8
+    int planes;  // staged channels = 7 PZ + nj (>= 8 PZ + 2 rz; the surplus is zero filled)
     int tlen;    // padded taps per ox = nj + 8
     int smem_bytes(int rx) const { return (planes * sw + (2 * rx + 1) * tlen) * (int)sizeof(float); }
 };
 
-DirectShape direct_shape(int rx, int rz)
+DirectShape direct_shape(int rx, int rz, int pz, int nc)
 {
     DirectShape s;
     s.rxp = (rx + 3) & ~3;
-    s.sw = DR_XT + 2 * s.rxp;
-    s.nj = (DR_PZ + 2 * rz + 7) & ~7;
-    s.planes = DR_ZB - DR_PZ + s.nj;
+    s.sw = 32 * nc + 2 * s.rxp;
+    s.nj = (pz + 2 * rz + 7) & ~7;
+    s.planes = (DR_GROUPS - 1) * pz + s.nj;
     s.tlen = s.nj + 8;
     return s;
 }
 
-template <bool F64>
+template <bool F64, int DR_PZ, int NC>
 __global__ void __launch_bounds__(DR_THREADS) k_direct(const float *__restrict__ in, float *__restrict__ out,
                                                         const float *__restrict__ filt, Dims d, int rx, int ry,
                                                         int rz, DirectShape sh)
 {
+    constexpr int DR_XT = 32 * NC, DR_ZB = DR_PZ * DR_GROUPS;
     extern __shared__ __align__(16) float dr_smem[];
     float *slab = dr_smem;                              // [planes][sw]
     float *taps = dr_smem + sh.planes * sh.sw;          // [2 rx + 1][tlen]: tap of channel offset o at [8 + o + rz]
@@ -56,12 +57,14 @@ __global__ void __launch_bounds__(DR_THREADS) k_direct(const float *__restrict__
     const bool vec = (d.nx & 3) == 0;                   // rows are 16-byte aligned
 
     using acc_t = typename std::conditional<F64, double, float>::type;
-    acc_t acc[DR_PZ][4];                                // fp64 path
-    float2 a2[DR_PZ][2];                                // fp32 path: (columns 0, 1) and (2, 3) of the lane as FFMA2 pairs
+    acc_t acc[DR_PZ][NC];                               // fp64 path
+    float2 a2[DR_PZ][NC / 2];                           // fp32 path: pairs of the lane's columns as FFMA2 operands
 #pragma unroll
     for (int p = 0; p < DR_PZ; ++p) {
-        acc[p][0] = acc[p][1] = acc[p][2] = acc[p][3] = (acc_t)0;
-        a2[p][0] = a2[p][1] = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) acc[p][c] = (acc_t)0;
+#pragma unroll
+        for (int c = 0; c < NC / 2; ++c) a2[p][c] = make_float2(0.f, 0.f);
     }
 
     for (int oy = -ry; oy <= ry; ++oy) {
@@ -113,16 +116,18 @@ __global__ void __launch_bounds__(DR_THREADS) k_direct(const float *__restrict__
 #pragma unroll
                 for (int jj = 0; jj < 8; ++jj) {
                     const float *pv = base + (jc + jj) * sh.sw;
-                    const float v0 = pv[0], v1 = pv[32], v2 = pv[64], v3 = pv[96];
+                    float v[NC];
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) v[c] = pv[32 * c];
 #pragma unroll
                     for (int p = 0; p < DR_PZ; ++p) {
                         const float g = tw[jj - p + 8];  // tap of channel offset (jc + jj) - p - rz
                         if constexpr (F64) {
-                            acc[p][0] += (double)v0 * (double)g; acc[p][1] += (double)v1 * (double)g;
-                            acc[p][2] += (double)v2 * (double)g; acc[p][3] += (double)v3 * (double)g;
+#pragma unroll
+                            for (int c = 0; c < NC; ++c) acc[p][c] += (double)v[c] * (double)g;
                         } else {
-                            a2[p][0] = ffma2(make_float2(v0, v1), g, a2[p][0]);
-                            a2[p][1] = ffma2(make_float2(v2, v3), g, a2[p][1]);
+#pragma unroll
+                            for (int c = 0; c < NC / 2; ++c) a2[p][c] = ffma2(make_float2(v[2 * c], v[2 * c + 1]), g, a2[p][c]);
                         }
                     }
                 }
@@ -136,15 +141,16 @@ __global__ void __launch_bounds__(DR_THREADS) k_direct(const float *__restrict__
         const int gz = z0 + wz * DR_PZ + p;
         if (gz >= d.nz) break;
         float *o = rowo + (long long)gz * d.plane;
-        float v[4];
+        float v[NC];
         if constexpr (F64) {
 #pragma unroll
-            for (int c = 0; c < 4; ++c) v[c] = (float)acc[p][c];
+            for (int c = 0; c < NC; ++c) v[c] = (float)acc[p][c];
         } else {
-            v[0] = a2[p][0].x; v[1] = a2[p][0].y; v[2] = a2[p][1].x; v[3] = a2[p][1].y;
+#pragma unroll
+            for (int c = 0; c < NC / 2; ++c) { v[2 * c] = a2[p][c].x; v[2 * c + 1] = a2[p][c].y; }
         }
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
+        for (int c = 0; c < NC; ++c) {
             const int gx = x0 + lx + 32 * c;
             if (gx < d.nx) o[gx] = v[c];
         }
@@ -153,12 +159,30 @@ __global__ void __launch_bounds__(DR_THREADS) k_direct(const float *__restrict__
 
 }  // namespace
 
+// <PZ, NC> of the launch: narrow bands walk 4 outputs per thread
+inline bool direct_narrow(int rz) { return rz <= 8; }
+
 bool direct_supported(const pgsf_plan *p, int rx, int ry, int rz, int *smem)
 {
     if (rx < 0 || ry < 0 || rz < 0 || rx > PGSF_MAX_RADIUS || ry > PGSF_MAX_RADIUS || rz > PGSF_MAX_RADIUS) return false;
-    const DirectShape sh = direct_shape(rx, rz);
+    const bool nb = direct_narrow(rz);
+    const DirectShape sh = direct_shape(rx, rz, nb ? 4 : 8, nb ? 8 : 4);
     *smem = sh.smem_bytes(rx);
-    return *smem <= 200 * 1024 && p->dims.ny <= 65535 && (p->dims.nx + DR_XT - 1) / DR_XT <= 65535;
+    const int xt = nb ? 256 : 128;
+    return *smem <= 200 * 1024 && p->dims.ny <= 65535 && (p->dims.nx + xt - 1) / xt <= 65535;
+}
+
+template <bool F64, int PZ, int NC>
+cudaError_t launch_direct(const float *filt, int rx, int ry, int rz, const float *in, float *out, const Dims &d,
+                          cudaStream_t st)
+{
+    const DirectShape sh = direct_shape(rx, rz, PZ, NC);
+    const int smem = sh.smem_bytes(rx);
+    cudaError_t e = ensure_dynamic_smem(k_direct<F64, PZ, NC>, smem);
+    if (e != cudaSuccess) return e;
+    dim3 grid((d.nz + PZ * DR_GROUPS - 1) / (PZ * DR_GROUPS), (d.nx + 32 * NC - 1) / (32 * NC), d.ny);
+    k_direct<F64, PZ, NC><<<grid, DR_THREADS, smem, st>>>(in, out, filt, d, rx, ry, rz, sh);
+    return cudaGetLastError();
 }
 
 // one cube per call
@@ -166,15 +190,12 @@ cudaError_t direct_filter3d(pgsf_plan *p, const float *filt, int rx, int ry, int
                             bool fp64, cudaStream_t st)
 {
     const Dims &d = p->dims;
-    const DirectShape sh = direct_shape(rx, rz);
-    const int smem = sh.smem_bytes(rx);
-    cudaError_t e = fp64 ? ensure_dynamic_smem(k_direct<true>, smem) : ensure_dynamic_smem(k_direct<false>, smem);
-    if (e != cudaSuccess) return e;
-    dim3 grid((d.nz + DR_ZB - 1) / DR_ZB, (d.nx + DR_XT - 1) / DR_XT, d.ny);
     LaunchScope ls(p, fp64 ? "direct_f64" : "direct_f32", st);
-    if (fp64) k_direct<true><<<grid, DR_THREADS, smem, st>>>(in, out, filt, d, rx, ry, rz, sh);
-    else k_direct<false><<<grid, DR_THREADS, smem, st>>>(in, out, filt, d, rx, ry, rz, sh);
-    return cudaGetLastError();
+    if (direct_narrow(rz))
+        return fp64 ? launch_direct<true, 4, 8>(filt, rx, ry, rz, in, out, d, st)
+                    : launch_direct<false, 4, 8>(filt, rx, ry, rz, in, out, d, st);
+    return fp64 ? launch_direct<true, 8, 4>(filt, rx, ry, rz, in, out, d, st)
+                : launch_direct<false, 8, 4>(filt, rx, ry, rz, in, out, d, st);
 }
 
 }  // namespace pgsf
