@@ -393,16 +393,26 @@ pgsf_status pgsf_filter3d_weighted(pgsf_plan *p, int scale, const float *d_in, c
     float *den = w.stmp, *tmp = w.stmp + p->dims.cube;      // (the statistics cubes are free here)
     for (int bi = 0; bi < p->desc.batch; ++bi) {
         const size_t off = (size_t)bi * p->dims.cube;
-        // numerator: Eq. 2 of the product cube
-        if ((e = pgsf::weighted_mul(p, d_in + off, d_w + off, w.scratch, st)) != cudaSuccess)
-            return cuda_fail(p, e, "weighted product launch");
-        if ((s = filter_one(p, scale, w.scratch, d_out + off, w, st)) != PGSF_OK) return s;
+        // numerator: Eq. 2 of the product cube (fast path: the product is formed while the x/y pass stages its input)
+        if (p->fast_filter) {
+            if ((e = pgsf::fast_filter3d(p, scale, d_in + off, d_out + off, w.ftmp, st, false, d_w + off)) != cudaSuccess)
+                return cuda_fail(p, e, "weighted filter launch");
+        } else {
+            if ((e = pgsf::weighted_mul(p, d_in + off, d_w + off, w.scratch, st)) != cudaSuccess)
+                return cuda_fail(p, e, "weighted product launch");
+            if ((s = filter_one(p, scale, w.scratch, d_out + off, w, st)) != PGSF_OK) return s;
+        }
         // denominator: box sum of w (as printed) or Eq. 2 of w
+        if (p->fast_filter) {
+            // the filter kernels with all-ones (or the Gaussian) taps; their frequency pass divides d_out in place
+            e = pgsf::fast_filter3d(p, scale, d_w + off, den, w.ftmp, st, mode == PGSF_WEIGHTED_AS_PRINTED, nullptr,
+                                    d_out + off);
+            if (e != cudaSuccess) return cuda_fail(p, e, "weight sum launch");
+            continue;
+        }
         if (mode == PGSF_WEIGHTED_AS_PRINTED) {
-            // fast path: the filter kernels with all-ones taps; else three generic directional sums
-            e = p->fast_filter ? pgsf::fast_filter3d(p, scale, d_w + off, den, w.ftmp, st, true)
-                               : pgsf::weighted_boxsum(p, scale, d_w + off, den, tmp, st);
-            if (e != cudaSuccess) return cuda_fail(p, e, "weight box sum launch");
+            if ((e = pgsf::weighted_boxsum(p, scale, d_w + off, den, tmp, st)) != cudaSuccess)
+                return cuda_fail(p, e, "weight box sum launch");
         } else if ((s = filter_one(p, scale, d_w + off, den, w, st)) != PGSF_OK) {
             return s;
         }

@@ -19,17 +19,17 @@
 
 namespace pgsf {
 // per-radius entry points of the frequency-axis kernels (pgsf_z_r*.cu)
-cudaError_t launch_z_r6(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
+cudaError_t launch_z_r6(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
 cudaError_t launch_zm_r6(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
-cudaError_t launch_z_r12(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
+cudaError_t launch_z_r12(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
 cudaError_t launch_zm_r12(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
-cudaError_t launch_z_r24(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
+cudaError_t launch_z_r24(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
 cudaError_t launch_zm_r24(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
-cudaError_t launch_z_r48(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
+cudaError_t launch_z_r48(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
 cudaError_t launch_zm_r48(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
-cudaError_t launch_z_r72(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
+cudaError_t launch_z_r72(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
 cudaError_t launch_zm_r72(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
-cudaError_t launch_z_r96(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st);
+cudaError_t launch_z_r96(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
 cudaError_t launch_zm_r96(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
 
 namespace {
@@ -64,6 +64,7 @@ struct XymParams {
     Dims d;
     int ychunk;                       // output rows per CTA (multiple of 16)
     float *out[XM_MAXS];              // x/y-filtered cube of each scale
+    const float *wgt;                 // Eq. 1: the input is multiplied by this cube while it is staged (NULL: Eq. 2)
     TapsXY t[XM_MAXS];
 };
 
@@ -146,7 +147,7 @@ struct XmY {
     }
 };
 
-template <int NS, int RA, int RB, int RC, int RD>
+template <int NS, int RA, int RB, int RC, int RD, bool WGT = false>
 __global__ void __launch_bounds__(XM_NT, 2) k_xym(const float *__restrict__ in, const __grid_constant__ XymParams P)
 {
     extern __shared__ __align__(16) float2 xm_smem[];
@@ -187,8 +188,12 @@ __global__ void __launch_bounds__(XM_NT, 2) k_xym(const float *__restrict__ in, 
                 const int idx = lane + 32 * q;
                 const int xx = x0 - XM_HALO + 4 * idx;
                 const bool ok = rok && idx < XM_SW / 4 && xx >= 0 && xx < d.nx;
-                pf[rr][q] = ok ? __ldg(reinterpret_cast<const float4 *>(in + plane_off + (long long)r * d.nx + xx))
-                               : make_float4(0.f, 0.f, 0.f, 0.f);
+                const long long o = plane_off + (long long)r * d.nx + xx;
+                pf[rr][q] = ok ? __ldg(reinterpret_cast<const float4 *>(in + o)) : make_float4(0.f, 0.f, 0.f, 0.f);
+                if (WGT && ok) {
+                    const float4 w4 = __ldg(reinterpret_cast<const float4 *>(P.wgt + o));
+                    pf[rr][q].x *= w4.x; pf[rr][q].y *= w4.y; pf[rr][q].z *= w4.z; pf[rr][q].w *= w4.w;
+                }
             }
         }
     };
@@ -260,15 +265,15 @@ __global__ void __launch_bounds__(XM_NT, 2) k_xym(const float *__restrict__ in, 
     }
 }
 
-template <int NS, int RA, int RB, int RC, int RD>
+template <int NS, int RA, int RB, int RC, int RD, bool WGT = false>
 cudaError_t launch_xym(const float *in, const XymParams &P, int sm_count, cudaStream_t st)
 {
     constexpr int SMEM = (XM_NB * XM_SIN + XM_NB * NS * XM_U) * (int)sizeof(float2);
-    cudaError_t e = ensure_dynamic_smem(k_xym<NS, RA, RB, RC, RD>, SMEM);
+    cudaError_t e = ensure_dynamic_smem(k_xym<NS, RA, RB, RC, RD, WGT>, SMEM);
     if (e != cudaSuccess) return e;
     (void)sm_count;
     dim3 grid((P.d.nx + XM_NT - 1) / XM_NT, (P.d.ny + P.ychunk - 1) / P.ychunk, P.d.nz);
-    k_xym<NS, RA, RB, RC, RD><<<grid, XM_NT, SMEM, st>>>(in, P);
+    k_xym<NS, RA, RB, RC, RD, WGT><<<grid, XM_NT, SMEM, st>>>(in, P);
     return cudaGetLastError();
 }
 
@@ -298,7 +303,11 @@ static bool xym_dispatch(int n, const int *rc, const float *in, const XymParams 
 {
 #define XYM_CASE(NS, A, B, C, D)                                                              \
     if (n == NS && rc[0] == A && (NS < 2 || rc[1] == B) && (NS < 3 || rc[2] == C) && (NS < 4 || rc[3] == D)) { \
-        if (!probe) *err = launch_xym<NS, A, (NS > 1 ? B : 3), (NS > 2 ? C : 3), (NS > 3 ? D : 3)>(in, P, sm_count, st); \
+        if (!probe) {                                                                         \
+            if (NS == 1 && P.wgt != nullptr) *err = launch_xym<1, A, 3, 3, 3, true>(in, P, sm_count, st); \
+            else if (P.wgt != nullptr) *err = cudaErrorNotSupported;  /* weighted staging: single-scale launches only */ \
+            else *err = launch_xym<NS, A, (NS > 1 ? B : 3), (NS > 2 ? C : 3), (NS > 3 ? D : 3)>(in, P, sm_count, st); \
+        }                                                                                     \
         return true;                                                                          \
     }
     XYM_CASE(4, 3, 6, 9, 12)
@@ -327,7 +336,7 @@ static bool xym_dispatch(int n, const int *rc, const float *in, const XymParams 
 // scales are sorted by compiled radius and cut into the largest groups a k_xym instance exists for;
 // every group reads the input once.
 cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *in, float *const *out, int ncubes,
-                          cudaStream_t st, bool box)
+                          cudaStream_t st, bool box, const float *wgt)
 {
     // the x and y passes do not couple planes: `ncubes` consecutive cubes are one stack of ncubes * nz planes
     Dims d = p->dims;
@@ -364,6 +373,7 @@ cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *i
         if (take < 1) return cudaErrorNotSupported;
         P.d = d;
         P.ychunk = ychunk;
+        P.wgt = wgt;
         unsigned mask = 0;
         for (int i = 0; i < XM_MAXS; ++i) {
             const int j = i < take ? i : 0;
@@ -384,7 +394,7 @@ cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *i
 }
 
 // frequency pass of one scale: in (x/y-filtered cube) -> out
-cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStream_t st, bool box)
+cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStream_t st, bool box, float *ratio)
 {
     const Dims &d = p->dims;
     const ScalePlan &sp = p->scales[scale];
@@ -394,12 +404,12 @@ cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStr
     LaunchScope ls(p, name, st);
     const Taps &tz = box ? sp.tz_box : sp.tz;
     switch (sp.rz_c) {
-    case 6: return launch_z_r6(in, out, d, tz, st);
-    case 12: return launch_z_r12(in, out, d, tz, st);
-    case 24: return launch_z_r24(in, out, d, tz, st);
-    case 48: return launch_z_r48(in, out, d, tz, st);
-    case 72: return launch_z_r72(in, out, d, tz, st);
-    case 96: return launch_z_r96(in, out, d, tz, st);
+    case 6: return launch_z_r6(in, out, ratio, d, tz, st);
+    case 12: return launch_z_r12(in, out, ratio, d, tz, st);
+    case 24: return launch_z_r24(in, out, ratio, d, tz, st);
+    case 48: return launch_z_r48(in, out, ratio, d, tz, st);
+    case 72: return launch_z_r72(in, out, ratio, d, tz, st);
+    case 96: return launch_z_r96(in, out, ratio, d, tz, st);
     default: return cudaErrorNotSupported;
     }
 }
@@ -428,12 +438,12 @@ cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float 
 }
 
 cudaError_t fast_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp,
-                          cudaStream_t st, bool box)
+                          cudaStream_t st, bool box, const float *wgt, float *ratio)
 {
     float *outs[1] = {tmp};
-    cudaError_t e = fast_xy_multi(p, &scale, 1, in, outs, 1, st, box);
+    cudaError_t e = fast_xy_multi(p, &scale, 1, in, outs, 1, st, box, wgt);
     if (e != cudaSuccess) return e;
-    return fast_z(p, scale, tmp, out, st, box);
+    return fast_z(p, scale, tmp, out, st, box, ratio);
 }
 
 }  // namespace pgsf

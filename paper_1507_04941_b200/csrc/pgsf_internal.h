@@ -113,13 +113,16 @@ cudaError_t generic_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int o
 // ---- fast kernels (pgsf_filter.cu, pgsf_stats.cu): nx % 4 == 0, 16-byte aligned, compiled radii --
 bool fast_xy_radius(int r, int *compiled);
 bool fast_z_radius(int r, int *compiled);
-// box = true: the same passes with all-ones taps (sum over the box of the filter support)
+// box = true: the same passes with all-ones taps (sum over the box of the filter support);
+// wgt != NULL: the input is multiplied by this cube while it is staged (numerator of Eq. 1);
+// ratio != NULL: the result is not written to `out` but divides the cube `ratio` in place (denominator of Eq. 1)
 cudaError_t fast_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp,
-                          cudaStream_t st, bool box = false);
+                          cudaStream_t st, bool box = false, const float *wgt = nullptr, float *ratio = nullptr);
 // `ncubes` consecutive cubes (stride dims.cube) per call, for the entry points that take it
 cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *in, float *const *out, int ncubes,
-                          cudaStream_t st, bool box = false);
-cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStream_t st, bool box = false);
+                          cudaStream_t st, bool box = false, const float *wgt = nullptr);
+cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStream_t st, bool box = false,
+                   float *ratio = nullptr);
 cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, int ncubes,
                     cudaStream_t st);
 bool fast_stats_supported(const pgsf_plan *p);

@@ -80,7 +80,7 @@ __device__ __forceinline__ void z_accumulate(const float *__restrict__ base, con
 
 template <int RZ>
 __global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, float *__restrict__ out,
-                                                 Dims d, Taps t)
+                                                 float *__restrict__ ratio, Dims d, Taps t)
 {
     using S = ZShape<RZ>;
     extern __shared__ __align__(16) float smem[];  // [PLANES][Z_XT]
@@ -110,6 +110,21 @@ __global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, f
     float2 acc[Z_PZ][2];
     z_accumulate<RZ>(smem + (wz * Z_PZ) * Z_XT + 4 * lane, t, acc);
     if (!col_ok) return;
+    if (ratio != nullptr) {
+        // Eq. 1: this pass produced the denominator; `ratio` holds the numerator and receives the quotient (0 / 0 -> 0)
+        float *col = ratio + (long long)y * d.nx + gx;
+#pragma unroll
+        for (int p = 0; p < Z_PZ; ++p) {
+            const int gz = z0 + wz * Z_PZ + p;
+            if (gz >= d.nz) break;
+            float4 *q = reinterpret_cast<float4 *>(col + (long long)gz * d.plane);
+            const float4 n = *q;
+            const float4 dn = make_float4(acc[p][0].x, acc[p][0].y, acc[p][1].x, acc[p][1].y);
+            *q = make_float4(dn.x != 0.f ? n.x / dn.x : 0.f, dn.y != 0.f ? n.y / dn.y : 0.f,
+                             dn.z != 0.f ? n.z / dn.z : 0.f, dn.w != 0.f ? n.w / dn.w : 0.f);
+        }
+        return;
+    }
     float *col_out = out + (long long)y * d.nx + gx;
 #pragma unroll
     for (int p = 0; p < Z_PZ; ++p) {
@@ -283,12 +298,12 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
 }
 
 template <int RZ>
-cudaError_t launch_z(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st)
+cudaError_t launch_z(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st)
 {
     cudaError_t e = ensure_dynamic_smem(k_z<RZ>, ZShape<RZ>::SMEM);
     if (e != cudaSuccess) return e;
     dim3 grid((d.nz + Z_ZB - 1) / Z_ZB, (d.nx + Z_XT - 1) / Z_XT, d.ny);
-    k_z<RZ><<<grid, Z_THREADS, ZShape<RZ>::SMEM, st>>>(in, out, d, t);
+    k_z<RZ><<<grid, Z_THREADS, ZShape<RZ>::SMEM, st>>>(in, out, ratio, d, t);
     return cudaGetLastError();
 }
 
@@ -316,9 +331,10 @@ cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const D
 // one pair of plain entry points per radius
 #define PGSF_INSTANTIATE_Z(RZ)                                                                              \
     namespace pgsf {                                                                                        \
-    cudaError_t launch_z_r##RZ(const float *in, float *out, const Dims &d, const Taps &t, cudaStream_t st)  \
+    cudaError_t launch_z_r##RZ(const float *in, float *out, float *ratio, const Dims &d, const Taps &t,     \
+                               cudaStream_t st)                                                             \
     {                                                                                                       \
-        return launch_z<RZ>(in, out, d, t, st);                                                             \
+        return launch_z<RZ>(in, out, ratio, d, t, st);                                                      \
     }                                                                                                       \
     cudaError_t launch_zm_r##RZ(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz,   \
                                 const Taps &t, int ncubes, cudaStream_t st)                                 \
