@@ -41,9 +41,9 @@ def _peaks():
 
 
 def _dram_traffic(workload: str, kernel: str):
-    """DRAM bytes per launch of `kernel` from the committed ncu capture (profiles/r01_dram_traffic.csv),
-    or None when no capture exists for this workload / kernel."""
-    path = os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")
+    """DRAM bytes per launch of `kernel` from the committed ncu capture of the current kernels
+    (profiles/r02_dram_traffic.csv), or None when no capture exists for this workload / kernel."""
+    path = os.path.join(ROOT, "profiles", "r02_dram_traffic.csv")
     if not os.path.exists(path):
         return None
     import csv
@@ -229,39 +229,179 @@ def aggregate_value(n_vox: int, n_scales: int, world: int, ms_step: float) -> fl
 
 def _kernel_work(name: str, w, taps, n_vox: int):
     """Algorithmic (flops, bytes) of ONE launch of the kernel `name`: the work
-    the separable method must do, not what the implementation happens to move."""
+    the separable method must do, not what the implementation happens to move.  Bytes follow SURVEY.md 8(d)
+    strictly: the input is read once (charged to the x/y kernel), every filtered cube is written once (charged
+    to its z kernel), the mask is written once (charged to the statistics kernel); every intermediate (t2, the
+    window sums, the re-read of f) is implementation traffic and counts for nothing here."""
     S = len(taps)
     kind, _, tail = name.partition("_")
     if kind in ("bxy", "bz"):                     # the filter kernels with all-ones taps (Eq. 1 denominator)
         kind = kind[1:]
     if kind == "xy" and tail.startswith("m"):  # x and y passes of the scales in the bit mask, one read of the input
         grp = [t for i, t in enumerate(taps) if (int(tail[1:]) >> i) & 1]
-        return 2 * sum(t[0] + t[1] for t in grp) * n_vox, (4 + 4 * len(grp)) * n_vox
+        return 2 * sum(t[0] + t[1] for t in grp) * n_vox, 4 * n_vox
     if kind == "xy" and tail.startswith("s"):
         t = taps[int(tail[1:])]
-        return 2 * (t[0] + t[1]) * n_vox, 8 * n_vox
+        return 2 * (t[0] + t[1]) * n_vox, 4 * n_vox
     if kind == "z" and tail.startswith("s"):
         t = taps[int(tail[1:])]
-        return 2 * t[2] * n_vox, 8 * n_vox
+        return 2 * t[2] * n_vox, 4 * n_vox
     if kind == "zm" and tail.startswith("s"):   # z pass + z-direction window sums (5 of the 21 statistics flops)
         t = taps[int(tail[1:])]
-        return (2 * t[2] + STATS_Z_FLOPS) * n_vox, 8 * n_vox
+        return (2 * t[2] + STATS_Z_FLOPS) * n_vox, 4 * n_vox
     if kind == "stats" and tail == "xybox":     # x/y window sums + selection after a fused zm launch
-        return (STATS_FLOPS - STATS_Z_FLOPS) * n_vox, 5 * n_vox
+        return (STATS_FLOPS - STATS_Z_FLOPS) * n_vox, 1 * n_vox
     if kind == "w":                              # Eq. 1 helpers: product, box sum of the weights, division
         return {"mul": (1, 12), "box": (6, 8), "div": (1, 12)}.get(tail, (0, 0))[0] * n_vox, \
                {"mul": (1, 12), "box": (6, 8), "div": (1, 12)}.get(tail, (0, 0))[1] * n_vox
     if kind == "stats" and tail == "all":    # statistics of every scale, one mask write
         return STATS_FLOPS * S * n_vox, (4 * S + 1) * n_vox
     if kind == "stats":
-        return STATS_FLOPS * n_vox, 5 * n_vox
+        return STATS_FLOPS * n_vox, 1 * n_vox
     return 0, 0
+
+
+def _path_roofline(w, taps, n_vox, ms_step, alu_peak, hbm_peak):
+    S = len(taps)
+    path_flops = sum(2 * sum(t) + STATS_FLOPS for t in taps) * n_vox
+    path_bytes = (4 + 4 * S + 1) * n_vox
+    t_alu, t_hbm = path_flops / (alu_peak * 1e12), path_bytes / (hbm_peak * 1e9)
+    t_path = max(t_alu, t_hbm)
+    return {"flops_per_voxel": path_flops / n_vox, "bytes_per_voxel": path_bytes / n_vox,
+            "roofline_ms": t_path * 1e3, "frac": t_path * 1e3 / ms_step, "bound": "alu" if t_alu >= t_hbm else "hbm"}
+
+
+def measure_workload(w, dev, device_index, rank, world, steps, warmup, peaks, sm_count, detail=True):
+    """One workload on this rank's GPU: W warm-up steps, K timed steps (CUDA events on the launching stream,
+    per-launch profiling events OFF), then -- with detail -- a second, profiled pass for the per-kernel table and
+    the per-scale calls of SURVEY.md 8(d) metric (i).  Returns (dict of results, ctx with the live buffers)."""
+    import torch
+    import torch.distributed as dist
+    from paper_1507_04941_b200 import binding, synth
+
+    d = synth.make_workload(replica_workload(w, rank), dev)
+    n_vox = w.voxels
+    S = len(w.sigmas)
+    taps = _taps(w)
+    plan = binding.Plan(w.dims, w.sigmas, w.box_half, w.k, batch=w.batch, halo=w.halo, truncate=w.truncate,
+                        device=device_index)
+    filt = [torch.empty_like(d) for _ in range(S)]
+    mask = torch.empty(d.shape, dtype=torch.uint8, device=dev)
+    cnt = torch.zeros(1, dtype=torch.int64, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        plan.pgsf_find_multiscale(d, d_filtered=filt, d_mask=mask, d_count=cnt, stream=stream)
+
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(device_index)
+    sampler.start()
+    l0 = plan.pgsf_plan_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record(stream)
+    for _ in range(steps):
+        step()
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    launches = plan.pgsf_plan_launch_count() - l0
+    clocks = sampler.stop()
+    count = int(cnt.item())
+    ms_step = max_over_ranks(ms_total, world, dev) / steps
+    alu_peak = _alu_peak_tflops(sm_count, peaks["sm_max_mhz"])
+    hbm_peak = peaks["hbm_gbs"]
+    out = {"ms_per_step": ms_step, "value": aggregate_value(n_vox, S, world, ms_step), "count": count,
+           "launches": int(launches), "clocks": clocks,
+           "path_roofline": _path_roofline(w, taps, n_vox, ms_step, alu_peak, hbm_peak)}
+    ctx = dict(plan=plan, d=d, filt=filt, mask=mask, cnt=cnt, rank=rank, world=world, dev=dev)
+    if not detail:
+        return out, ctx
+
+    # ---- second pass, per-launch CUDA events on: which kernel dominates, and its roofline (DESIGN.md 'Rooflines')
+    psteps = max(1, min(steps, 5))
+    plan.pgsf_plan_set_profiling(True)
+    pe0, pe1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    pe0.record(stream)
+    for _ in range(psteps):
+        step()
+    pe1.record(stream)
+    torch.cuda.synchronize()
+    prof = plan.pgsf_plan_profile()
+    plan.pgsf_plan_set_profiling(False)
+    ms_prof_total = pe0.elapsed_time(pe1)
+    kern = []
+    cube = w.dims[0] * w.dims[1] * w.dims[2]
+    for name, (n, ms) in prof.items():
+        # voxels per launch: a batch goes through in groups of cubes; a name shared by all scales
+        # (stats_*) is launched once per scale and group
+        per_step = S if name.startswith("stats_") else 1
+        vox_launch = cube * w.batch * per_step * psteps / max(n, 1)
+        if name == "pivot":
+            vox_launch = 0
+        fl, by = _kernel_work(name, w, taps, vox_launch)
+        kern.append({"name": name, "launches": n, "ms_per_launch": ms / max(n, 1), "share": ms / max(ms_prof_total, 1e-9),
+                     "flops": fl, "bytes": by})
+    kern.sort(key=lambda k: -k["share"])
+    roofline = None
+    if kern:
+        k0 = kern[0]
+        t_alu = k0["flops"] / (alu_peak * 1e12)
+        t_hbm = k0["bytes"] / (hbm_peak * 1e9)
+        sec = k0["ms_per_launch"] * 1e-3
+        if t_alu >= t_hbm:
+            ach = k0["flops"] / sec / 1e12
+            roofline = {"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak}
+        else:
+            ach = k0["bytes"] / sec / 1e9
+            roofline = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak}
+        roofline.update({"kernel": k0["name"], "ms_per_launch": k0["ms_per_launch"], "share_of_step": k0["share"],
+                         "algorithmic_flops": k0["flops"], "algorithmic_bytes": k0["bytes"],
+                         "traffic": _dram_traffic(w.name, k0["name"]),
+                         "peak_source": ("148 SM x 128 lanes x 2 x sm_max_mhz" if t_alu >= t_hbm else peaks["source"]),
+                         "timed": "per-launch CUDA events in a separate pass of %d steps (%.3f ms per step with the "
+                                  "events on; the headline loop runs with them off)" % (psteps, ms_prof_total / psteps)})
+    out["roofline"] = roofline
+    out["kernels"] = [{"name": k["name"], "launches": k["launches"], "ms_per_launch": round(k["ms_per_launch"], 4),
+                       "share": round(k["share"], 4)} for k in kern]
+
+    # ---- SURVEY.md 8(d) metric (i): per scale, N / (t_filter3d + t_local_threshold) through the per-scale calls
+    per_scale = []
+    for s_i in range(S):
+        times = []
+        for which in ("filter3d", "local_threshold"):
+            best = None
+            for rep in range(3):                     # first repetition = warm-up
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                if which == "filter3d":
+                    plan.pgsf_filter3d(s_i, d, d_out=filt[s_i], stream=stream)
+                else:
+                    plan.pgsf_local_threshold(filt[s_i], d_mask=mask, want_count=False, stream=stream)
+                b.record(stream)
+                torch.cuda.synchronize()
+                if rep:
+                    t = a.elapsed_time(b)
+                    best = t if best is None else min(best, t)
+            times.append(best)
+        t_sum = max_over_ranks(times[0] + times[1], world, dev)
+        per_scale.append({"sigma": list(w.sigmas[s_i]), "ms_filter3d": round(times[0], 4),
+                          "ms_local_threshold": round(times[1], 4),
+                          "gvoxel_per_s": n_vox * world / (t_sum * 1e-3) / 1e9})
+    out["per_scale"] = per_scale
+    return out, ctx
 
 
 def run_b200(args, w):
     import torch
     import torch.distributed as dist
-    from paper_1507_04941_b200 import binding, build, synth
+    from paper_1507_04941_b200 import binding, build
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -279,101 +419,53 @@ def run_b200(args, w):
     binding.load_library()
     props = torch.cuda.get_device_properties(local_rank)
     peaks = _peaks()
-
-    # every rank runs its own replica of the workload (seed offset by rank)
-    d = synth.make_workload(replica_workload(w, rank), dev)
-    n_vox = w.voxels
-    S = len(w.sigmas)
-    taps = _taps(w)
-    plan = binding.Plan(w.dims, w.sigmas, w.box_half, w.k, batch=w.batch, halo=w.halo, truncate=w.truncate,
-                        device=local_rank)
-    filt = [torch.empty_like(d) for _ in range(S)]
-    mask = torch.empty(d.shape, dtype=torch.uint8, device=dev)
-    cnt = torch.zeros(1, dtype=torch.int64, device=dev)
-    stream = torch.cuda.current_stream()
-
-    def step():
-        plan.pgsf_find_multiscale(d, d_filtered=filt, d_mask=mask, d_count=cnt, stream=stream)
-
-    for _ in range(args.warmup):
-        step()
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    plan.pgsf_plan_set_profiling(True)
-    l0 = plan.pgsf_plan_launch_count()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    ev0.record(stream)
-    for _ in range(args.steps):
-        step()
-    ev1.record(stream)
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    ms_total = ev0.elapsed_time(ev1)
-    launches = plan.pgsf_plan_launch_count() - l0
-    prof = plan.pgsf_plan_profile()
-    plan.pgsf_plan_set_profiling(False)
-    clocks = sampler.stop()
-    count = int(cnt.item())
-    ms_total = max_over_ranks(ms_total, world, dev)
-    ms_step = ms_total / args.steps
-    value = aggregate_value(n_vox, S, world, ms_step)
-
-    # ---- roofline of the dominant kernel + of the whole path
-    alu_peak = _alu_peak_tflops(props.multi_processor_count, peaks["sm_max_mhz"])
-    hbm_peak = peaks["hbm_gbs"]
-    kern = []
-    cube = w.dims[0] * w.dims[1] * w.dims[2]
-    for name, (n, ms) in prof.items():
-        # voxels per launch: a batch goes through in groups of cubes; a name shared by all scales
-        # (stats_*) is launched once per scale and group
-        per_step = S if name.startswith("stats_") else 1
-        vox_launch = cube * w.batch * per_step * args.steps / max(n, 1)
-        fl, by = _kernel_work(name, w, taps, vox_launch)
-        kern.append({"name": name, "launches": n, "ms_per_launch": ms / max(n, 1), "share": ms / max(ms_total, 1e-9),
-                     "flops": fl, "bytes": by})
-    kern.sort(key=lambda k: -k["share"])
-    roofline = None
-    if kern:
-        k0 = kern[0]
-        t_alu = k0["flops"] / (alu_peak * 1e12)
-        t_hbm = k0["bytes"] / (hbm_peak * 1e9)
-        sec = k0["ms_per_launch"] * 1e-3
-        if t_alu >= t_hbm:
-            ach = k0["flops"] / sec / 1e12
-            roofline = {"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak}
-        else:
-            ach = k0["bytes"] / sec / 1e9
-            roofline = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak}
-        roofline.update({"kernel": k0["name"], "ms_per_launch": k0["ms_per_launch"], "share_of_step": k0["share"],
-                         "traffic": _dram_traffic(w.name, k0["name"]), "peak_source": ("148 SM x 128 lanes x 2 x sm_max_mhz" if t_alu >= t_hbm
-                                                          else peaks["source"])})
-    path_flops = sum(2 * sum(t) + STATS_FLOPS for t in taps) * n_vox
-    path_bytes = (4 + 4 * S + 1) * n_vox
-    t_path = max(path_flops / (alu_peak * 1e12), path_bytes / (hbm_peak * 1e9))
-    path = {"flops_per_voxel": path_flops / n_vox, "bytes_per_voxel": path_bytes / n_vox,
-            "roofline_ms": t_path * 1e3, "frac": t_path * 1e3 / ms_step,
-            "bound": "alu" if path_flops / (alu_peak * 1e12) >= path_bytes / (hbm_peak * 1e9) else "hbm"}
-
+    res, ctx = measure_workload(w, dev, local_rank, rank, world, args.steps, args.warmup, peaks,
+                                props.multi_processor_count)
+    n_vox, S = w.voxels, len(w.sigmas)
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": {"workload": w.name, "dims_xyz": list(w.dims), "batch": w.batch, "halo": list(w.halo),
                    "sigmas": [list(s) for s in w.sigmas], "box_half": list(w.box_half), "k": w.k,
-                   "voxels": n_vox, "scales": S, "filtered_cubes_kept": True, "count": count,
+                   "voxels": n_vox, "scales": S, "filtered_cubes_kept": True, "count": res["count"],
                    "l2": "inputs larger than L2 (input %.1f GiB, outputs %.1f GiB per step)" % (
                        n_vox * 4 / 2**30, n_vox * (4 * S + 1) / 2**30),
+                   "timing": "CUDA events on the launching stream around the K steps; per-launch profiling events off",
+                   "kernel_path": ctx["plan"].pgsf_plan_path()[1],
                    "parallelism": "replicas only (no collective)"},
-        "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline, "path_roofline": path,
-        "kernels": [{"name": k["name"], "launches": k["launches"], "ms_per_launch": round(k["ms_per_launch"], 4),
-                     "share": round(k["share"], 4)} for k in kern],
+        "clocks": res["clocks"], "gpu_launches": res["launches"], "roofline": res["roofline"],
+        "path_roofline": res["path_roofline"], "kernels": res["kernels"], "per_scale": res["per_scale"],
     }
-    return line, dict(plan=plan, d=d, filt=filt, mask=mask, cnt=cnt, rank=rank, world=world, dev=dev)
+    ctx["peaks"], ctx["sm_count"], ctx["local_rank"] = peaks, props.multi_processor_count, local_rank
+    return line, ctx
+
+
+def run_other_configs(args, main_w, ctx):
+    """ms per step and path-roofline fraction of the other BASELINE.json configs, measured in this same invocation
+    after the headline (buffers allocated and freed per config; K <= 5 steps, no kernel table)."""
+    import gc
+    import torch
+    from paper_1507_04941_b200 import synth
+    out = []
+    for c in sorted(synth.WORKLOADS):
+        w = synth.WORKLOADS[c]
+        if w.name == main_w.name:
+            continue
+        gc.collect()
+        torch.cuda.empty_cache()
+        res, c2 = measure_workload(w, ctx["dev"], ctx["local_rank"], 0, 1, max(1, min(args.steps, 5)), 3, ctx["peaks"],
+                                   ctx["sm_count"], detail=False)
+        c2["plan"].close()
+        pr = res["path_roofline"]
+        out.append({"workload": w.name, "ms_per_step": res["ms_per_step"], "value": res["value"], "unit": UNIT,
+                    "count": res["count"], "gpu_launches": res["launches"], "roofline_ms": pr["roofline_ms"],
+                    "path_frac": pr["frac"], "bound": pr["bound"], "sm_mhz": res["clocks"].get("sm_mhz"),
+                    "reasons": res["clocks"].get("reasons")})
+        del c2, res
+    gc.collect()
+    torch.cuda.empty_cache()
+    return out
 
 
 def run_e2e(args, w, ctx):
@@ -411,10 +503,29 @@ def run_e2e(args, w, ctx):
             "api": "pgsf_find_multiscale_host (pinned host cube in; mask + count out)"}
 
 
-def run_cpu_baseline(w, sub, a, lo, hi):
+CPU_SAMPLE_1T = (128, 128, 128)    # the 1-thread leg: a smaller brick of the same cube (~10 s)
+
+
+def run_cpu_baseline(w, sub, a, lo, hi, d_full=None):
+    """The oracle as it stands on the box's host cores: all cores (OpenMP) on the sample brick and, per
+    SURVEY.md 8(d), one thread on a smaller brick of the same cube."""
+    from oracle import pgsf_oracle
     sec, vs, threads = time_oracle(w, sub, a, lo, hi)
-    return {"value": vs / sec / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle", "seconds": sec,
-            "sample": _sample_text(w, lo, hi)}
+    out = {"value": vs / sec / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle", "seconds": sec,
+           "sample": _sample_text(w, lo, hi)}
+    if d_full is not None:
+        lo1, hi1 = _oracle_sample_region(w, CPU_SAMPLE_1T)
+        a1, e1 = pgsf_oracle.required_input_box(w.dims, w.sigmas, w.box_half, lo1, hi1, w.truncate)
+        sub1 = d_full[a1[2] - a[2]:e1[2] - a[2], a1[1] - a[1]:e1[1] - a[1], a1[0] - a[0]:e1[0] - a[0]]
+        pgsf_oracle.set_threads(1)
+        t0 = time.perf_counter()
+        pgsf_oracle.find_region(sub1, a1, w.dims, w.sigmas, w.box_half, w.k, lo1, hi1, w.halo, w.truncate)
+        dt = time.perf_counter() - t0
+        pgsf_oracle.set_threads(0)
+        vs1 = (hi1[0] - lo1[0]) * (hi1[1] - lo1[1]) * (hi1[2] - lo1[2]) * len(w.sigmas)
+        out["single_thread"] = {"value": vs1 / dt / 1e9, "unit": UNIT, "cores": 1, "seconds": dt,
+                                "sample": _sample_text(w, lo1, hi1)}
+    return out
 
 
 # ------------------------------------------------------------------------------------ Eq. 1 (weighted), NEXT-1
@@ -649,6 +760,8 @@ def main():
     ap.add_argument("--fp64", action="store_true", help="--path direct: accumulate in fp64 as the paper does")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="skip the ms-per-step sweep over the other BASELINE.json configs after the headline")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
     from paper_1507_04941_b200 import synth
@@ -672,8 +785,13 @@ def main():
         line["e2e"] = run_e2e(args, w, ctx)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         ctx["plan"].close()
-        cpu = run_cpu_baseline(w, sub, a, lo, hi)
+        cpu = run_cpu_baseline(w, sub, a, lo, hi, d_full=sub)
     line["cpu_baseline"] = cpu
+    if rank == 0 and world == 1 and not args.no_other_configs:
+        ctx["plan"].close()
+        for k in ("d", "filt", "mask", "cnt"):
+            ctx[k] = None
+        line["other_configs"] = run_other_configs(args, w, ctx)
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:

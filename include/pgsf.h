@@ -61,8 +61,11 @@ typedef enum {
 
 /* plan flags */
 #define PGSF_FLAG_FORCE_GENERIC 0x1u /* use only the generic (any shape / any radius) kernels */
-#define PGSF_FLAG_SMALL_GROUPS  0x2u /* test aid: pgsf_find_multiscale takes a batch two cubes per launch group
-                                        (by default as many as fit 2^32 voxels), so that ragged last groups run */
+/* (bit 0x2 is reserved: it was a test aid in an earlier revision, now PGSF_OPT_GROUP_CUBES below) */
+#define PGSF_FLAG_DRY_RUN 0x4u       /* plan for inspection only: pgsf_plan_create touches no device (148 SMs are
+                                        assumed), so pgsf_plan_path / pgsf_plan_workspace_bytes / the argument
+                                        validation of every call can be exercised on a machine without a GPU;
+                                        a compute call that passes validation returns PGSF_ERR_CUDA */
 
 #define PGSF_MAX_SCALES 8
 #define PGSF_MAX_RADIUS 96 /* largest supported ceil(truncate*sigma) on any axis */
@@ -95,6 +98,30 @@ PGSF_API pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *des
 
 /* Releases the plan and everything it owns.  NULL is allowed. */
 PGSF_API pgsf_status pgsf_plan_destroy(pgsf_plan *plan);
+
+/*
+ * pgsf_plan_set_option -- run-time knobs of a plan (host only; none of them changes a result).
+ *   PGSF_OPT_GROUP_CUBES          cubes of a batch that pgsf_find_multiscale takes per launch group; 1 .. the plan's
+ *                                 default (as many as fit 2^32 voxels).  A test aid: ragged last groups.
+ *   PGSF_OPT_HOST_SECTION_PLANES  pgsf_find_multiscale_host: core planes (channels) per section of the streamed
+ *                                 cube ("section = core + halo"); 0 = chosen from the device budget.
+ *   PGSF_OPT_HOST_DEVICE_BUDGET   pgsf_find_multiscale_host: bytes of device memory its staging may use;
+ *                                 0 = 80 % of the memory free at the first call.
+ * INVALID_ARG for an unknown option or a value outside its range.
+ */
+#define PGSF_OPT_GROUP_CUBES 1
+#define PGSF_OPT_HOST_SECTION_PLANES 2
+#define PGSF_OPT_HOST_DEVICE_BUDGET 3
+PGSF_API pgsf_status pgsf_plan_set_option(pgsf_plan *plan, int option, long long value);
+
+/*
+ * pgsf_plan_path -- which kernels this plan runs, as text ("filter: tiled ...; stats: generic (hx = 5 ...)"),
+ * so that a caller can see a shape / radius / box that falls off the tiled sm_100a kernels onto the
+ * one-thread-per-voxel generic ones (several times slower, same results).  Writes at most cap bytes (NUL
+ * terminated) to HOST `text`; returns 1 if every stage of pgsf_find_multiscale runs tiled kernels, 0 if some
+ * stage is generic, -1 for bad arguments.
+ */
+PGSF_API int pgsf_plan_path(const pgsf_plan *plan, char *text, int cap);
 
 /* Bytes of DEVICE scratch the caller must pass as d_workspace to the calls below (256-byte
  * aligned; may be 0, in which case d_workspace may be NULL).  0 for a NULL plan. */
@@ -171,7 +198,10 @@ PGSF_API pgsf_status pgsf_local_threshold(pgsf_plan *plan, const float *d_filter
  * pgsf_find_multiscale -- the whole hot path: for every scale of the plan, filter
  * d_in, threshold, OR into d_mask; *d_count = set voxels of the final mask.
  * d_filtered: HOST array of n_scales DEVICE pointers receiving the filtered cubes, or NULL /
- * NULL entries = do not keep (the workspace then holds one scratch cube).
+ * NULL entries = do not keep (the workspace then holds one scratch cube).  The cubes of d_filtered are used
+ * as scratch before they hold their final content (the x/y-filtered data of scale s+1 is parked in
+ * d_filtered[s+1] while scale s runs), so d_in, d_mask, d_count, the workspace and every d_filtered[s] must
+ * be mutually disjoint: INVALID_ARG otherwise.
  */
 PGSF_API pgsf_status pgsf_find_multiscale(pgsf_plan *plan, const float *d_in, float *const *d_filtered,
                                  uint8_t *d_mask, unsigned long long *d_count, void *d_workspace,

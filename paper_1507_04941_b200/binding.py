@@ -17,7 +17,8 @@ LIB_PATH = os.path.join(_HERE, "libpgsf.so")
 
 PGSF_OK, PGSF_ERR_INVALID_ARG, PGSF_ERR_UNSUPPORTED, PGSF_ERR_OOM, PGSF_ERR_CUDA = range(5)
 PGSF_FLAG_FORCE_GENERIC = 0x1
-PGSF_FLAG_SMALL_GROUPS = 0x2
+PGSF_FLAG_DRY_RUN = 0x4
+PGSF_OPT_GROUP_CUBES, PGSF_OPT_HOST_SECTION_PLANES, PGSF_OPT_HOST_DEVICE_BUDGET = 1, 2, 3
 PGSF_WEIGHTED_AS_PRINTED = 0
 PGSF_WEIGHTED_NORMALISED = 1
 PGSF_DIRECT_FP64_ACCUM = 0x1
@@ -26,7 +27,8 @@ PGSF_MAX_RADIUS = 96
 _STATUS = {0: "PGSF_OK", 1: "PGSF_ERR_INVALID_ARG", 2: "PGSF_ERR_UNSUPPORTED", 3: "PGSF_ERR_OOM",
            4: "PGSF_ERR_CUDA"}
 
-EXPORTS = ["pgsf_plan_create", "pgsf_plan_destroy", "pgsf_plan_workspace_bytes", "pgsf_last_error",
+EXPORTS = ["pgsf_plan_create", "pgsf_plan_destroy", "pgsf_plan_set_option", "pgsf_plan_path",
+           "pgsf_plan_workspace_bytes", "pgsf_last_error",
            "pgsf_plan_get_taps", "pgsf_filter3d", "pgsf_filter3d_weighted", "pgsf_filter3d_direct", "pgsf_local_threshold", "pgsf_find_multiscale",
            "pgsf_find_multiscale_host", "pgsf_plan_launch_count", "pgsf_plan_set_profiling",
            "pgsf_plan_profile_collect", "pgsf_plan_profile_entry"]
@@ -62,6 +64,10 @@ def load_library() -> ctypes.CDLL:
         lib.pgsf_plan_create.restype = i
         lib.pgsf_plan_destroy.argtypes = [vp]
         lib.pgsf_plan_destroy.restype = i
+        lib.pgsf_plan_set_option.argtypes = [vp, i, ctypes.c_longlong]
+        lib.pgsf_plan_set_option.restype = i
+        lib.pgsf_plan_path.argtypes = [vp, ctypes.c_char_p, i]
+        lib.pgsf_plan_path.restype = i
         lib.pgsf_plan_workspace_bytes.argtypes = [vp]
         lib.pgsf_plan_workspace_bytes.restype = ctypes.c_size_t
         lib.pgsf_last_error.argtypes = [vp]
@@ -157,6 +163,17 @@ class Plan:
 
     def pgsf_plan_workspace_bytes(self) -> int:
         return int(self._lib.pgsf_plan_workspace_bytes(self._h))
+
+    def pgsf_plan_set_option(self, option: int, value: int) -> None:
+        self._check(self._lib.pgsf_plan_set_option(self._h, int(option), int(value)))
+
+    def pgsf_plan_path(self):
+        """(all_tiled: bool, text) -- which kernels the plan runs and why."""
+        buf = ctypes.create_string_buffer(512)
+        rc = self._lib.pgsf_plan_path(self._h, buf, 512)
+        if rc < 0:
+            raise PgsfError(PGSF_ERR_INVALID_ARG, "pgsf_plan_path")
+        return bool(rc), buf.value.decode()
 
     def pgsf_plan_launch_count(self) -> int:
         return int(self._lib.pgsf_plan_launch_count(self._h))

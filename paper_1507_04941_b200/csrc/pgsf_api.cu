@@ -65,11 +65,41 @@ cudaEvent_t take_event(pgsf_plan *p)
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+struct Range { const char *name; const void *ptr; size_t bytes; };
+
+// first pair of overlapping byte ranges (NULL / empty ranges are skipped), or false
+bool find_overlap(const Range *r, int n, int *a, int *b)
+{
+    for (int i = 0; i < n; ++i)
+        for (int j = i + 1; j < n; ++j) {
+            if (!r[i].ptr || !r[j].ptr || !r[i].bytes || !r[j].bytes) continue;
+            const char *pi = static_cast<const char *>(r[i].ptr), *pj = static_cast<const char *>(r[j].ptr);
+            if (pi < pj + r[j].bytes && pj < pi + r[i].bytes) { *a = i; *b = j; return true; }
+        }
+    return false;
+}
+
 size_t round256(size_t v) { return (v + 255u) & ~(size_t)255u; }
 
 }  // namespace
 
 namespace pgsf {
+
+void host_release(pgsf_plan *p)
+{
+    cudaFree(p->h_d_in);
+    cudaFree(p->h_d_mask);
+    cudaFree(p->h_d_count);
+    cudaFree(p->h_d_ws);
+    p->h_d_in = nullptr;
+    p->h_d_mask = nullptr;
+    p->h_d_count = nullptr;
+    p->h_d_ws = nullptr;
+    for (int s = 0; s < PGSF_MAX_SCALES; ++s) { cudaFree(p->h_d_f[s]); p->h_d_f[s] = nullptr; }
+    if (p->h_stream) cudaStreamDestroy(p->h_stream);
+    p->h_stream = nullptr;
+    cudaGetLastError();
+}
 
 LaunchScope::LaunchScope(pgsf_plan *plan, const char *name, cudaStream_t stream) : p(plan), st(stream), b(nullptr)
 {
@@ -129,17 +159,21 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
             return fail(nullptr, PGSF_ERR_UNSUPPORTED, "radius ceil(truncate*sigma) above %d",
                         PGSF_MAX_RADIUS);
     }
-    int ndev = 0;
-    cudaError_t e = cudaGetDeviceCount(&ndev);
-    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDeviceCount (no CPU fallback exists)");
-    if (device < 0 || device >= ndev)
-        return fail(nullptr, PGSF_ERR_CUDA, "device %d not present (%d devices)", device, ndev);
+    const bool dry = (desc->flags & PGSF_FLAG_DRY_RUN) != 0;
     cudaDeviceProp prop;
-    e = cudaGetDeviceProperties(&prop, device);
-    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDeviceProperties");
-    if (prop.major != 10)
-        return fail(nullptr, PGSF_ERR_UNSUPPORTED, "device is sm_%d%d; this library is built for sm_100a",
-                    prop.major, prop.minor);
+    prop.multiProcessorCount = 148;
+    if (!dry) {
+        int ndev = 0;
+        cudaError_t e = cudaGetDeviceCount(&ndev);
+        if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDeviceCount (no CPU fallback exists)");
+        if (device < 0 || device >= ndev)
+            return fail(nullptr, PGSF_ERR_CUDA, "device %d not present (%d devices)", device, ndev);
+        e = cudaGetDeviceProperties(&prop, device);
+        if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDeviceProperties");
+        if (prop.major != 10)
+            return fail(nullptr, PGSF_ERR_UNSUPPORTED, "device is sm_%d%d; this library is built for sm_100a",
+                        prop.major, prop.minor);
+    }
 
     pgsf_plan *p = new (std::nothrow) pgsf_plan();
     if (!p) return fail(nullptr, PGSF_ERR_OOM, "plan allocation failed");
@@ -147,6 +181,7 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
     memcpy(p->sigmas, desc->sigmas, sizeof(double) * 3 * desc->n_scales);
     p->desc.sigmas = p->sigmas;
     p->device = device;
+    p->dry = dry;
     p->sm_count = prop.multiProcessorCount;
     p->dims.nx = desc->nx;
     p->dims.ny = desc->ny;
@@ -155,6 +190,7 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
     p->dims.cube = p->dims.plane * desc->nz;
     p->launches = 0;
     p->prof_on = false;
+    p->d_pivot = nullptr;
     p->h_d_in = nullptr;
     p->h_d_mask = nullptr;
     p->h_d_count = nullptr;
@@ -163,7 +199,14 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
     for (int s = 0; s < PGSF_MAX_SCALES; ++s) p->h_d_f[s] = nullptr;
 
     const bool force_generic = (desc->flags & PGSF_FLAG_FORCE_GENERIC) != 0;
-    bool fast = !force_generic && (desc->nx % 4 == 0);
+    // The tiled kernels put ny, nz (x batch group) on grid.y / grid.z: shapes beyond those limits run the generic
+    // kernels (decided here, so that no launch can fail with an invalid configuration later).
+    const bool grid_ok = desc->ny <= 65535 && desc->nz <= 65535;
+    bool fast = !force_generic && (desc->nx % 4 == 0) && grid_ok;
+    char why[160];
+    if (force_generic) p->why_filter = "PGSF_FLAG_FORCE_GENERIC";
+    else if (desc->nx % 4 != 0) p->why_filter = "nx % 4 != 0";
+    else if (!grid_ok) p->why_filter = "ny or nz above 65535";
     for (int s = 0; s < desc->n_scales; ++s) {
         pgsf::ScalePlan &sp = p->scales[s];
         memset(&sp, 0, sizeof sp);
@@ -175,6 +218,11 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
         }
         const int rxy = sp.r[0] > sp.r[1] ? sp.r[0] : sp.r[1];
         if (!pgsf::fast_xy_radius(rxy, &sp.rxy_c) || !pgsf::fast_z_radius(sp.r[2], &sp.rz_c)) {
+            if (fast) {
+                snprintf(why, sizeof why, "scale %d: radii (%d, %d, %d) outside the compiled x/y <= 12, z <= 96", s,
+                         sp.r[0], sp.r[1], sp.r[2]);
+                p->why_filter = why;
+            }
             fast = false;
             continue;
         }
@@ -190,7 +238,11 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
         for (int o = -sp.r[2]; o <= sp.r[2]; ++o) sp.tz_box.g[o + sp.rz_c + pgsf::kTapPad] = 1.f;
     }
     p->fast_filter = fast;
-    p->fast_stats = !force_generic && (desc->nx % 4 == 0) && pgsf::fast_stats_supported(p);
+    p->fast_stats = !force_generic && grid_ok && pgsf::fast_stats_supported(p, &p->why_stats);
+    if (force_generic) p->why_stats = "PGSF_FLAG_FORCE_GENERIC";
+    else if (!grid_ok) p->why_stats = "ny or nz above 65535";
+    p->host_section_planes = 0;
+    p->host_budget = 0;
 
     // workspace: [scratch filtered cube][filter temporaries][statistics temporaries]
     p->ws_cube_bytes = round256((size_t)p->dims.cube * sizeof(float));
@@ -200,9 +252,19 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
     if (p->fast_filter && p->fast_stats && desc->batch > 1) {
         long long g = (1LL << 32) / p->dims.cube;
         if (g > 65535 / desc->nz) g = 65535 / desc->nz;
-        if ((desc->flags & PGSF_FLAG_SMALL_GROUPS) && g > 2) g = 2;
         if (g > desc->batch) g = desc->batch;
         p->group = g < 1 ? 1 : (int)g;
+    }
+    p->group_max = p->group;
+    if (!dry) {
+        cudaError_t e = cudaSetDevice(device);
+        if (e == cudaSuccess) e = cudaMalloc(&p->d_pivot, 256);
+        if (e == cudaSuccess) e = cudaMemset(p->d_pivot, 0, 256);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            delete p;
+            return fail(nullptr, PGSF_ERR_OOM, "plan constants: %s", cudaGetErrorString(e));
+        }
     }
     const size_t cubes = 1 + (p->fast_filter ? (size_t)p->group : 2) + (p->fast_stats ? 2 * (size_t)p->group : 4);
     p->ws_bytes = cubes * p->ws_cube_bytes;
@@ -213,19 +275,52 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
 pgsf_status pgsf_plan_destroy(pgsf_plan *p)
 {
     if (!p) return PGSF_OK;
-    if (p->h_d_in || p->h_d_mask || p->h_d_ws || p->h_d_count) {
-        cudaSetDevice(p->device);
-        cudaFree(p->h_d_in);
-        cudaFree(p->h_d_mask);
-        cudaFree(p->h_d_count);
-        cudaFree(p->h_d_ws);
-        for (int s = 0; s < PGSF_MAX_SCALES; ++s) cudaFree(p->h_d_f[s]);
-        if (p->h_stream) cudaStreamDestroy(p->h_stream);
+    if (!p->dry) {
+        cudaSetDevice(p->device);      // (events, streams and staging buffers belong to the plan's device)
+        pgsf::host_release(p);
+        cudaFree(p->d_pivot);
+        for (auto &r : p->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+        for (auto e : p->prof_free) cudaEventDestroy(e);
+        cudaGetLastError();
     }
-    for (auto &r : p->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
-    for (auto e : p->prof_free) cudaEventDestroy(e);
     delete p;
     return PGSF_OK;
+}
+
+pgsf_status pgsf_plan_set_option(pgsf_plan *p, int option, long long value)
+{
+    if (!p) return PGSF_ERR_INVALID_ARG;
+    switch (option) {
+    case PGSF_OPT_GROUP_CUBES:
+        if (value < 1 || value > p->group_max)
+            return fail(p, PGSF_ERR_INVALID_ARG, "PGSF_OPT_GROUP_CUBES must be in 1..%d", p->group_max);
+        p->group = (int)value;
+        return PGSF_OK;
+    case PGSF_OPT_HOST_SECTION_PLANES:
+        if (value < 0 || value > p->desc.nz)
+            return fail(p, PGSF_ERR_INVALID_ARG, "PGSF_OPT_HOST_SECTION_PLANES must be in 0..nz");
+        if (value != p->host_section_planes && !p->dry) { cudaSetDevice(p->device); pgsf::host_release(p); }
+        p->host_section_planes = value;
+        return PGSF_OK;
+    case PGSF_OPT_HOST_DEVICE_BUDGET:
+        if (value < 0) return fail(p, PGSF_ERR_INVALID_ARG, "PGSF_OPT_HOST_DEVICE_BUDGET must be >= 0");
+        if (value != p->host_budget && !p->dry) { cudaSetDevice(p->device); pgsf::host_release(p); }
+        p->host_budget = value;
+        return PGSF_OK;
+    default:
+        return fail(p, PGSF_ERR_INVALID_ARG, "unknown option %d", option);
+    }
+}
+
+int pgsf_plan_path(const pgsf_plan *p, char *text, int cap)
+{
+    if (!p || !text || cap < 1) return -1;
+    const bool tiled = p->fast_filter && p->fast_stats;
+    snprintf(text, (size_t)cap, "filter: %s%s%s; stats: %s%s%s",
+             p->fast_filter ? "tiled (k_xym + k_z / k_zm)" : "generic (k_conv1d) because ", p->fast_filter ? "" : p->why_filter.c_str(), "",
+             p->fast_stats ? "tiled (k_zm / k_zbox + k_ymarch)" : "generic (k_boxsum + k_threshold) because ",
+             p->fast_stats ? "" : p->why_stats.c_str(), "");
+    return tiled ? 1 : 0;
 }
 
 pgsf_status pgsf_plan_set_profiling(pgsf_plan *p, int enable)
@@ -302,7 +397,7 @@ Workspace carve(const pgsf_plan *p, void *ws)
     char *b = static_cast<char *>(ws);
     w.scratch = reinterpret_cast<float *>(b);
     w.ftmp = reinterpret_cast<float *>(b + p->ws_cube_bytes);
-    w.stmp = reinterpret_cast<float *>(b + p->ws_cube_bytes * (1 + (p->fast_filter ? (size_t)p->group : 2)));
+    w.stmp = reinterpret_cast<float *>(b + p->ws_cube_bytes * (1 + (p->fast_filter ? (size_t)p->group_max : 2)));
     return w;
 }
 
@@ -333,6 +428,8 @@ pgsf_status threshold_batch(pgsf_plan *p, const float *f, uint8_t *mask, int or_
     for (int bi = 0; bi < batch && e == cudaSuccess; ++bi) {
         const size_t off = (size_t)bi * p->dims.cube;
         float *m = mean ? mean + off : nullptr, *s = sd ? sd + off : nullptr;
+        e = pgsf::compute_pivot(p, f + off, st);
+        if (e != cudaSuccess) break;
         if (p->fast_stats) e = pgsf::fast_threshold(p, f + off, mask + off, or_into, m, s, count, w.stmp, st);
         else e = pgsf::generic_threshold(p, f + off, mask + off, or_into, m, s, count, w.stmp, st);
     }
@@ -357,6 +454,7 @@ pgsf_status pgsf_filter3d(pgsf_plan *p, int scale, const float *d_in, float *d_o
     if (a < b + bytes && b < a + bytes) return fail(p, PGSF_ERR_INVALID_ARG, "d_out overlaps d_in");
     pgsf_status s = check_ws(p, d_ws);
     if (s != PGSF_OK) return s;
+    if (p->dry) return fail(p, PGSF_ERR_CUDA, "PGSF_FLAG_DRY_RUN plan: arguments are valid, but no device is attached");
     cudaError_t e = cudaSetDevice(p->device);
     if (e != cudaSuccess) return cuda_fail(p, e, "cudaSetDevice");
     const Workspace w = carve(p, d_ws);
@@ -386,6 +484,7 @@ pgsf_status pgsf_filter3d_weighted(pgsf_plan *p, int scale, const float *d_in, c
     }
     pgsf_status s = check_ws(p, d_ws);
     if (s != PGSF_OK) return s;
+    if (p->dry) return fail(p, PGSF_ERR_CUDA, "PGSF_FLAG_DRY_RUN plan: arguments are valid, but no device is attached");
     cudaError_t e = cudaSetDevice(p->device);
     if (e != cudaSuccess) return cuda_fail(p, e, "cudaSetDevice");
     const Workspace w = carve(p, d_ws);
@@ -437,6 +536,7 @@ pgsf_status pgsf_filter3d_direct(pgsf_plan *p, const float *d_filter, int rx, in
     if (!pgsf::direct_supported(p, rx, ry, rz, &smem))
         return fail(p, PGSF_ERR_UNSUPPORTED, "filter radii (%d, %d, %d) need %d bytes of shared memory or exceed %d",
                     rx, ry, rz, smem, PGSF_MAX_RADIUS);
+    if (p->dry) return fail(p, PGSF_ERR_CUDA, "PGSF_FLAG_DRY_RUN plan: arguments are valid, but no device is attached");
     cudaError_t e = cudaSetDevice(p->device);
     if (e != cudaSuccess) return cuda_fail(p, e, "cudaSetDevice");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -460,6 +560,7 @@ pgsf_status pgsf_local_threshold(pgsf_plan *p, const float *d_f, uint8_t *d_mask
         return fail(p, PGSF_ERR_INVALID_ARG, "d_count must be 8-byte aligned");
     pgsf_status s = check_ws(p, d_ws);
     if (s != PGSF_OK) return s;
+    if (p->dry) return fail(p, PGSF_ERR_CUDA, "PGSF_FLAG_DRY_RUN plan: arguments are valid, but no device is attached");
     cudaError_t e = cudaSetDevice(p->device);
     if (e != cudaSuccess) return cuda_fail(p, e, "cudaSetDevice");
     const Workspace w = carve(p, d_ws);
@@ -487,6 +588,24 @@ pgsf_status pgsf_find_multiscale(pgsf_plan *p, const float *d_in, float *const *
                 return fail(p, PGSF_ERR_INVALID_ARG, "d_filtered[%d] must be 16-byte aligned", s);
     pgsf_status rc = check_ws(p, d_ws);
     if (rc != PGSF_OK) return rc;
+    {
+        // the filtered cubes double as scratch (pgsf.h), so every buffer of the call must be disjoint
+        static const char *fname[PGSF_MAX_SCALES] = {"d_filtered[0]", "d_filtered[1]", "d_filtered[2]", "d_filtered[3]",
+                                                     "d_filtered[4]", "d_filtered[5]", "d_filtered[6]", "d_filtered[7]"};
+        const size_t nvox = (size_t)p->dims.cube * p->desc.batch;
+        Range r[4 + PGSF_MAX_SCALES];
+        int n = 0;
+        r[n++] = Range{"d_in", d_in, nvox * sizeof(float)};
+        r[n++] = Range{"d_mask", d_mask, nvox};
+        r[n++] = Range{"d_count", d_count, sizeof(unsigned long long)};
+        r[n++] = Range{"d_workspace", d_ws, p->ws_bytes};
+        if (d_filtered)
+            for (int s = 0; s < S; ++s) r[n++] = Range{fname[s], d_filtered[s], nvox * sizeof(float)};
+        int a = 0, b = 0;
+        if (find_overlap(r, n, &a, &b))
+            return fail(p, PGSF_ERR_INVALID_ARG, "%s overlaps %s", r[a].name, r[b].name);
+    }
+    if (p->dry) return fail(p, PGSF_ERR_CUDA, "PGSF_FLAG_DRY_RUN plan: arguments are valid, but no device is attached");
     cudaError_t e = cudaSetDevice(p->device);
     if (e != cudaSuccess) return cuda_fail(p, e, "cudaSetDevice");
     const Workspace w = carve(p, d_ws);
@@ -513,10 +632,13 @@ pgsf_status pgsf_find_multiscale(pgsf_plan *p, const float *d_in, float *const *
             for (int s = 0; s < S; ++s) park[s] = (s + 1 < S) ? d_filtered[s + 1] + off : w.ftmp;
             cudaError_t ce = pgsf::fast_xy_multi(p, idx, S, d_in + off, park, nb, st);
             if (ce != cudaSuccess) return cuda_fail(p, ce, "xy filter launch");
+            // pivot of the statistics of every scale of this group: the level of the input (the taps sum to 1)
+            if (p->fast_stats && (ce = pgsf::compute_pivot(p, d_in + off, st)) != cudaSuccess)
+                return cuda_fail(p, ce, "pivot launch");
             for (int s = 0; s < S; ++s) {
                 if (p->fast_stats) {
                     // frequency pass and z-direction window sums in one march; then the x/y window sums
-                    float *Z1 = w.stmp, *Z2 = w.stmp + (size_t)p->group * p->dims.cube;
+                    float *Z1 = w.stmp, *Z2 = w.stmp + (size_t)p->group_max * p->dims.cube;
                     ce = pgsf::fast_zm(p, s, park[s], d_filtered[s] + off, Z1, Z2, nb, st);
                     if (ce != cudaSuccess) return cuda_fail(p, ce, "z filter + window launch");
                     ce = pgsf::fast_threshold_xy(p, d_filtered[s] + off, Z1, Z2, d_mask + off, s > 0, nullptr,
@@ -541,8 +663,9 @@ pgsf_status pgsf_find_multiscale(pgsf_plan *p, const float *d_in, float *const *
                 // filtered cubes not (all) kept: no room to park the x/y passes of all scales, so one x/y launch
                 // per scale; the frequency pass still carries the z-direction window sums
                 float *t2[1] = {w.ftmp};
-                float *Z1 = w.stmp, *Z2 = w.stmp + (size_t)p->group * p->dims.cube;
-                cudaError_t ce = pgsf::fast_xy_multi(p, &s, 1, d_in + off, t2, 1, st);
+                float *Z1 = w.stmp, *Z2 = w.stmp + (size_t)p->group_max * p->dims.cube;
+                cudaError_t ce = s == 0 ? pgsf::compute_pivot(p, d_in + off, st) : cudaSuccess;
+                if (ce == cudaSuccess) ce = pgsf::fast_xy_multi(p, &s, 1, d_in + off, t2, 1, st);
                 if (ce == cudaSuccess) ce = pgsf::fast_zm(p, s, w.ftmp, f, Z1, Z2, 1, st);
                 if (ce == cudaSuccess)
                     ce = pgsf::fast_threshold_xy(p, f, Z1, Z2, d_mask + off, s > 0, nullptr, nullptr,
@@ -565,18 +688,21 @@ pgsf_status pgsf_find_multiscale_host(pgsf_plan *p, const float *h_in, float *co
 {
     if (!p) return PGSF_ERR_INVALID_ARG;
     if (!h_in || !h_mask) return fail(p, PGSF_ERR_INVALID_ARG, "NULL host pointer");
+    if (p->dry) return fail(p, PGSF_ERR_CUDA, "PGSF_FLAG_DRY_RUN plan: arguments are valid, but no device is attached");
     cudaError_t e = cudaSetDevice(p->device);
     if (e != cudaSuccess) return cuda_fail(p, e, "cudaSetDevice");
     const size_t nvox = (size_t)p->dims.cube * p->desc.batch;
     const int S = p->desc.n_scales;
     if (!p->h_d_in) {
-        if ((e = cudaStreamCreateWithFlags(&p->h_stream, cudaStreamNonBlocking)) != cudaSuccess)
+        if ((e = cudaStreamCreateWithFlags(&p->h_stream, cudaStreamNonBlocking)) != cudaSuccess) {
+            p->h_stream = nullptr;
             return cuda_fail(p, e, "cudaStreamCreate");
+        }
         if ((e = cudaMalloc(&p->h_d_in, nvox * sizeof(float))) != cudaSuccess ||
             (e = cudaMalloc(&p->h_d_mask, nvox)) != cudaSuccess ||
             (e = cudaMalloc(&p->h_d_count, sizeof(unsigned long long))) != cudaSuccess ||
             (e = cudaMalloc(&p->h_d_ws, p->ws_bytes ? p->ws_bytes : 256)) != cudaSuccess) {
-            cudaGetLastError();
+            pgsf::host_release(p);     // all or nothing: the next call starts from scratch
             return fail(p, PGSF_ERR_OOM, "device staging allocation failed: %s", cudaGetErrorString(e));
         }
     }
@@ -585,6 +711,7 @@ pgsf_status pgsf_find_multiscale_host(pgsf_plan *p, const float *h_in, float *co
         for (int s = 0; s < S; ++s) {
             if (!h_filtered[s]) continue;
             if (!p->h_d_f[s] && (e = cudaMalloc(&p->h_d_f[s], nvox * sizeof(float))) != cudaSuccess) {
+                p->h_d_f[s] = nullptr;
                 cudaGetLastError();
                 return fail(p, PGSF_ERR_OOM, "device staging allocation failed: %s", cudaGetErrorString(e));
             }

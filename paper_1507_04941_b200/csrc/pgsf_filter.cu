@@ -20,17 +20,17 @@
 namespace pgsf {
 // per-radius entry points of the frequency-axis kernels (pgsf_z_r*.cu)
 cudaError_t launch_z_r6(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r6(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
+cudaError_t launch_zm_r6(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st);
 cudaError_t launch_z_r12(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r12(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
+cudaError_t launch_zm_r12(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st);
 cudaError_t launch_z_r24(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r24(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
+cudaError_t launch_zm_r24(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st);
 cudaError_t launch_z_r48(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r48(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
+cudaError_t launch_zm_r48(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st);
 cudaError_t launch_z_r72(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r72(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
+cudaError_t launch_zm_r72(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st);
 cudaError_t launch_z_r96(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r96(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t, int ncubes, cudaStream_t st);
+cudaError_t launch_zm_r96(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st);
 
 namespace {
 
@@ -427,12 +427,12 @@ cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float 
     snprintf(name, sizeof name, "zm_s%d", scale);
     LaunchScope ls(p, name, st);
     switch (sp.rz_c) {
-    case 6: return launch_zm_r6(in, out, Z1, Z2, d, hz, sp.tz, ncubes, st);
-    case 12: return launch_zm_r12(in, out, Z1, Z2, d, hz, sp.tz, ncubes, st);
-    case 24: return launch_zm_r24(in, out, Z1, Z2, d, hz, sp.tz, ncubes, st);
-    case 48: return launch_zm_r48(in, out, Z1, Z2, d, hz, sp.tz, ncubes, st);
-    case 72: return launch_zm_r72(in, out, Z1, Z2, d, hz, sp.tz, ncubes, st);
-    case 96: return launch_zm_r96(in, out, Z1, Z2, d, hz, sp.tz, ncubes, st);
+    case 6: return launch_zm_r6(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st);
+    case 12: return launch_zm_r12(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st);
+    case 24: return launch_zm_r24(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st);
+    case 48: return launch_zm_r48(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st);
+    case 72: return launch_zm_r72(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st);
+    case 96: return launch_zm_r96(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st);
     default: return cudaErrorNotSupported;
     }
 }

@@ -36,14 +36,57 @@ __global__ void __launch_bounds__(kThreads) k_conv1d(const float *__restrict__ i
     out[i] = acc;
 }
 
+// Pivot of the statistics: mean of a lattice of at most kPivotAxis^3 samples of the CENTRAL half of the cube
+// along every axis (next to a face the zero padding of the filter pulls f towards 0, which is not the level of
+// the data), fp64, fixed summation order.  The pivot is applied only where it is free of cost: when the samples
+// sit within a quarter of their mean (|mean| >= 4 sd), f - c is an exact fp32 subtraction for nearly every voxel
+// (Sterbenz: c/2 <= f <= 2c); for data scattered around zero the pivot is 0 and nothing changes.
+constexpr int kPivotThreads = 1024;
+constexpr int kPivotAxis = 100;
+
+__global__ void __launch_bounds__(kPivotThreads) k_pivot(const float *__restrict__ data, Dims d, float *__restrict__ pivot)
+{
+    __shared__ double part[kPivotThreads];
+    const int lo[3] = {d.nx / 4, d.ny / 4, d.nz / 4};
+    const int len[3] = {max(d.nx / 2, 1), max(d.ny / 2, 1), max(d.nz / 2, 1)};
+    int st[3], cnt[3];
+    for (int a = 0; a < 3; ++a) {
+        st[a] = (len[a] + kPivotAxis - 1) / kPivotAxis;
+        cnt[a] = (len[a] + st[a] - 1) / st[a];
+    }
+    const int nsamp = cnt[0] * cnt[1] * cnt[2];
+    __shared__ double part2[kPivotThreads];
+    double acc = 0.0, acc2 = 0.0;
+    for (int i = threadIdx.x; i < nsamp; i += kPivotThreads) {
+        const int ix = i % cnt[0], iy = (i / cnt[0]) % cnt[1], iz = i / (cnt[0] * cnt[1]);
+        const long long o = (long long)(lo[0] + ix * st[0]) + (long long)d.nx * ((lo[1] + iy * st[1]) + (long long)d.ny * (lo[2] + iz * st[2]));
+        const double v = (double)__ldg(data + o);
+        acc += v;
+        acc2 += v * v;
+    }
+    part[threadIdx.x] = acc;
+    part2[threadIdx.x] = acc2;
+    __syncthreads();
+    for (int w = kPivotThreads / 2; w > 0; w >>= 1) {
+        if ((int)threadIdx.x < w) { part[threadIdx.x] += part[threadIdx.x + w]; part2[threadIdx.x] += part2[threadIdx.x + w]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const double m = part[0] / (double)nsamp;
+        const double var = fmax(part2[0] / (double)nsamp - m * m, 0.0);
+        *pivot = (m * m >= 16.0 * var && m != 0.0) ? (float)m : 0.f;
+    }
+}
+
 // One directional sum of P:152 over the window clipped to the cube (C-7).
-// FIRST: q1 = a, q2 = a*a; otherwise q1 = a, q2 = b.
+// FIRST: q1 = a - c, q2 = (a - c)^2 with the pivot c; otherwise q1 = a, q2 = b.
 template <int AXIS, bool FIRST>
 __global__ void __launch_bounds__(kThreads) k_boxsum(const float *__restrict__ a,
                                                       const float *__restrict__ b,
                                                       float *__restrict__ oa, float *__restrict__ ob,
-                                                      Dims d, int h)
+                                                      Dims d, int h, const float *__restrict__ pivot)
 {
+    const float c0 = FIRST ? __ldg(pivot) : 0.f;
     long long i = (long long)blockIdx.x * kThreads + threadIdx.x;
     if (i >= d.cube) return;
     int x, y, z;
@@ -54,7 +97,7 @@ __global__ void __launch_bounds__(kThreads) k_boxsum(const float *__restrict__ a
     const int lo = max(-h, -c), hi = min(h, n - 1 - c);
     float s1 = 0.f, s2 = 0.f;
     for (int o = lo; o <= hi; ++o) {
-        float v = a[i + o * stride];
+        float v = a[i + o * stride] - c0;
         s1 += v;
         if (FIRST) s2 = fmaf(v, v, s2);
         else s2 += b[i + o * stride];
@@ -74,16 +117,17 @@ __global__ void __launch_bounds__(kThreads) k_threshold(
     const float *__restrict__ f, const float *__restrict__ S1, const float *__restrict__ S2,
     uint8_t *__restrict__ mask, int or_into, float *__restrict__ mean, float *__restrict__ sd,
     unsigned long long *__restrict__ count, Dims d, int hx, int hy, int hz, int gx, int gy, int gz,
-    float k, float k2)
+    float k, float k2, const float *__restrict__ pivot)
 {
     long long i = (long long)blockIdx.x * kThreads + threadIdx.x;
+    const float c0 = __ldg(pivot);
     int set = 0;
     if (i < d.cube) {
         int x, y, z;
         decode(i, d, x, y, z);
         const float n = (float)clipped_len(x, hx, d.nx) * (float)clipped_len(y, hy, d.ny) *
                         (float)clipped_len(z, hz, d.nz);
-        const float v = f[i], s1 = S1[i], s2 = S2[i];
+        const float v = f[i] - c0, s1 = S1[i], s2 = S2[i];     // (S1, S2 are sums of f - c0 and (f - c0)^2)
         const float a = fmaf(n, v, -s1);
         const float q = fmaxf(fmaf(n, s2, -s1 * s1), 0.f);
         int sel = (a > kFlatGuard * n * fabsf(v)) && (a * a > k2 * q);
@@ -95,7 +139,7 @@ __global__ void __launch_bounds__(kThreads) k_threshold(
         set = sel;
         if (mean != nullptr) {
             const float m = s1 / n;
-            mean[i] = m;
+            mean[i] = m + c0;
             if (sd != nullptr) sd[i] = sqrtf(fmaxf(s2 / n - m * m, 0.f));
         } else if (sd != nullptr) {
             const float m = s1 / n;
@@ -120,6 +164,13 @@ inline unsigned grid_for(long long n) { return (unsigned)((n + kThreads - 1) / k
 
 }  // namespace
 
+cudaError_t compute_pivot(pgsf_plan *p, const float *data, cudaStream_t st)
+{
+    LaunchScope ls(p, "pivot", st);
+    k_pivot<<<1, kPivotThreads, 0, st>>>(data, p->dims, p->d_pivot);
+    return cudaGetLastError();
+}
+
 cudaError_t generic_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp_a,
                              float *tmp_b, cudaStream_t st)
 {
@@ -139,15 +190,15 @@ cudaError_t generic_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int o
     const unsigned g = grid_for(d.cube);
     float *x1 = tmp4, *x2 = tmp4 + d.cube, *y1 = tmp4 + 2 * d.cube, *y2 = tmp4 + 3 * d.cube;
     const int *h = p->desc.box_half;
-    { LaunchScope ls(p, "generic_boxsum_x", st); k_boxsum<0, true><<<g, kThreads, 0, st>>>(f, nullptr, x1, x2, d, h[0]); }
-    { LaunchScope ls(p, "generic_boxsum_y", st); k_boxsum<1, false><<<g, kThreads, 0, st>>>(x1, x2, y1, y2, d, h[1]); }
-    { LaunchScope ls(p, "generic_boxsum_z", st); k_boxsum<2, false><<<g, kThreads, 0, st>>>(y1, y2, x1, x2, d, h[2]); }
+    { LaunchScope ls(p, "generic_boxsum_x", st); k_boxsum<0, true><<<g, kThreads, 0, st>>>(f, nullptr, x1, x2, d, h[0], p->d_pivot); }
+    { LaunchScope ls(p, "generic_boxsum_y", st); k_boxsum<1, false><<<g, kThreads, 0, st>>>(x1, x2, y1, y2, d, h[1], p->d_pivot); }
+    { LaunchScope ls(p, "generic_boxsum_z", st); k_boxsum<2, false><<<g, kThreads, 0, st>>>(y1, y2, x1, x2, d, h[2], p->d_pivot); }
     const float k = (float)p->desc.k;
     {
         LaunchScope ls(p, "generic_threshold", st);
         k_threshold<<<g, kThreads, 0, st>>>(f, x1, x2, mask, or_into, mean, sd, count, d, h[0], h[1], h[2],
                                             p->desc.halo[0], p->desc.halo[1], p->desc.halo[2], k,
-                                            (float)(p->desc.k * p->desc.k));
+                                            (float)(p->desc.k * p->desc.k), p->d_pivot);
     }
     return cudaGetLastError();
 }

@@ -71,18 +71,24 @@ struct pgsf_plan {
     pgsf::ScalePlan scales[PGSF_MAX_SCALES];
     pgsf::Dims dims;
     int device;
+    bool dry;            // PGSF_FLAG_DRY_RUN: no device behind this plan
     int sm_count;
     bool fast_filter;    // all scales have compiled radii, nx % 4 == 0
     bool fast_stats;
     size_t ws_bytes;     // total workspace
     size_t ws_cube_bytes;
     int group;           // cubes of a batch that the fast path of pgsf_find_multiscale processes per launch
+    int group_max;       // the plan's default (the workspace is sized for it); PGSF_OPT_GROUP_CUBES lowers `group`
+    std::string why_filter, why_stats;   // why a stage runs the generic kernels ("" = tiled); pgsf_plan_path
+    long long host_section_planes;       // PGSF_OPT_HOST_SECTION_PLANES (0 = automatic)
+    long long host_budget;               // PGSF_OPT_HOST_DEVICE_BUDGET  (0 = automatic)
     unsigned long long launches;
     std::string err;
     bool prof_on;
     std::vector<pgsf::ProfRec> prof_recs;      // pending (not yet collected) launches
     std::vector<cudaEvent_t> prof_free;        // recycled events
     std::vector<pgsf::ProfAcc> prof_acc;
+    float *d_pivot;      // device scalar: the constant the statistics subtract from f before squaring (D-2)
     // plan-owned device staging for pgsf_find_multiscale_host
     float *h_d_in;
     float *h_d_f[PGSF_MAX_SCALES];
@@ -106,6 +112,12 @@ struct LaunchScope {
 // ---- generic kernels (pgsf_generic.cu): any shape, any radius <= PGSF_MAX_RADIUS ----------------
 cudaError_t generic_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp_a,
                              float *tmp_b, cudaStream_t st);
+// Pivot of the statistics (D-2): *p->d_pivot = mean of a lattice of <= 10^6 samples of the central half
+// of the cube at `data` (for a group of cubes: of its first cube).
+// The selection n f - S1 > k sqrt(n S2 - S1^2) is invariant under f -> f - c for any constant c; taking c near the
+// level of the data keeps S2/n - m^2 well conditioned in fp32 when the cube carries an offset |mean| >> sd.
+// One CTA, fixed summation order (deterministic; exact under power-of-two scaling of the data).
+cudaError_t compute_pivot(pgsf_plan *p, const float *data, cudaStream_t st);
 // tmp: 4 cubes
 cudaError_t generic_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean,
                               float *sd, unsigned long long *count, float *tmp4, cudaStream_t st);
@@ -125,7 +137,9 @@ cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStr
                    float *ratio = nullptr);
 cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, int ncubes,
                     cudaStream_t st);
-bool fast_stats_supported(const pgsf_plan *p);
+bool fast_stats_supported(const pgsf_plan *p, std::string *why);
+// frees the plan-owned staging of pgsf_find_multiscale_host (buffers, streams, events); the plan's device must be current
+void host_release(pgsf_plan *p);
 // x/y window sums + selection from precomputed z-direction window sums Z1, Z2 (of fast_zm / k_zbox)
 cudaError_t fast_threshold_xy(pgsf_plan *p, const float *f, const float *Z1, const float *Z2, uint8_t *mask,
                               int or_into, float *mean, float *sd, unsigned long long *count, int ncubes,

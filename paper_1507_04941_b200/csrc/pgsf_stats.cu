@@ -37,8 +37,9 @@ struct ZboxParams {
 };
 
 __global__ void __launch_bounds__(ZB_NT) k_zbox(const float4 *__restrict__ f, float4 *__restrict__ Z1,
-                                                float4 *__restrict__ Z2, ZboxParams p)
+                                                float4 *__restrict__ Z2, ZboxParams p, const float *__restrict__ pivot)
 {
+    const float c0 = __ldg(pivot);     // sums of f - c0 and (f - c0)^2 (D-2); planes outside the cube contribute nothing
     const long long c = (long long)blockIdx.x * ZB_NT + threadIdx.x;
     if (c >= p.cols4) return;
     const int chunk = blockIdx.y;
@@ -50,7 +51,7 @@ __global__ void __launch_bounds__(ZB_NT) k_zbox(const float4 *__restrict__ f, fl
     // planes za-hz .. za+hz-1 of the first window (clipped to the cube, C-7)
     for (int z = max(za - hz, 0); z < min(za + hz, nz); ++z) {
         const float4 v = __ldg(f + (long long)z * plane4 + c);
-        const float a[4] = {v.x, v.y, v.z, v.w};
+        const float a[4] = {v.x - c0, v.y - c0, v.z - c0, v.w - c0};
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             kahan_add(s1[u], e1[u], a[u]);
@@ -60,10 +61,10 @@ __global__ void __launch_bounds__(ZB_NT) k_zbox(const float4 *__restrict__ f, fl
 #pragma unroll 4
     for (int zc = za; zc < zb; ++zc) {
         const int zl = zc + hz, zt = zc - hz;
-        float4 l = make_float4(0.f, 0.f, 0.f, 0.f), t = make_float4(0.f, 0.f, 0.f, 0.f);
+        float4 l = make_float4(c0, c0, c0, c0), t = make_float4(c0, c0, c0, c0);
         if (zl < nz) l = __ldg(f + (long long)zl * plane4 + c);
         if (zt >= 0) t = __ldg(f + (long long)zt * plane4 + c);   // leaves after this output
-        const float a[4] = {l.x, l.y, l.z, l.w}, b[4] = {t.x, t.y, t.z, t.w};
+        const float a[4] = {l.x - c0, l.y - c0, l.z - c0, l.w - c0}, b[4] = {t.x - c0, t.y - c0, t.z - c0, t.w - c0};
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             kahan_add(s1[u], e1[u], a[u]);
@@ -170,8 +171,10 @@ template <int G>
 __global__ void __launch_bounds__(YM_MAX_NT) k_ymarch(const float *__restrict__ f, const float *__restrict__ Z1,
                                                       const float *__restrict__ Z2, uint8_t *__restrict__ mask,
                                                       float *__restrict__ mean, float *__restrict__ sd,
-                                                      unsigned long long *__restrict__ count, const YmParams p)
+                                                      unsigned long long *__restrict__ count, const YmParams p,
+                                                      const float *__restrict__ pivot)
 {
+    const float piv = __ldg(pivot);    // Z1, Z2 are sums of f - c0 and (f - c0)^2; the centre value is shifted alike
     using V = typename VecT<G>::type;
     constexpr int VL = VecT<G>::L, NV = G / VL, HX = 2 * G;
     extern __shared__ __align__(16) unsigned char ym_smem[];
@@ -297,7 +300,7 @@ __global__ void __launch_bounds__(YM_MAX_NT) k_ymarch(const float *__restrict__ 
 #pragma unroll
         for (int j = 0; j < G; ++j) {
             const float n = nxz[j] * nyc;
-            const float v = cur.fc[j];
+            const float v = cur.fc[j] - piv;
             const float a = fmaf(n, v, -S1[j]);
             const float q = fmaxf(fmaf(n, S2[j], -S1[j] * S1[j]), 0.f);
             const bool sel = (a > guard * n * fabsf(v)) && (a * a > p.k2 * q);
@@ -334,7 +337,7 @@ __global__ void __launch_bounds__(YM_MAX_NT) k_ymarch(const float *__restrict__ 
                 for (int j = 0; j < G; ++j) {
                     const float n = nxz[j] * nyc;
                     const float m = S1[j] / n;
-                    if (mean != nullptr) mean[idx + j] = m;
+                    if (mean != nullptr) mean[idx + j] = m + piv;
                     if (sd != nullptr) sd[idx + j] = sqrtf(fmaxf(S2[j] / n - m * m, 0.f));
                 }
             }
@@ -390,19 +393,23 @@ cudaError_t launch_ymarch(const pgsf_plan *pl, const float *f, const float *Z1, 
     if (ce != cudaSuccess) return ce;
     if ((long long)d.nz * ncubes > 65535) return cudaErrorInvalidConfiguration;
     dim3 grid(p.ntiles, nch, d.nz * ncubes);
-    k_ymarch<G><<<grid, nt, smem, st>>>(f, Z1, Z2, mask, mean, sd, count, p);
+    k_ymarch<G><<<grid, nt, smem, st>>>(f, Z1, Z2, mask, mean, sd, count, p, pl->d_pivot);
     return cudaGetLastError();
 }
 
 }  // namespace
 
-bool fast_stats_supported(const pgsf_plan *p)
+bool fast_stats_supported(const pgsf_plan *p, std::string *why)
 {
     const int hx = p->desc.box_half[0];
-    if (p->desc.nx % 4 != 0) return false;
-    if (hx != 4 && hx != 8 && hx != 16) return false;
-    if (p->desc.nx % (hx / 2) != 0) return false;   // a thread owns hx/2 whole columns
-    return p->desc.nz <= 65535;
+    char buf[128];
+    buf[0] = 0;
+    if (p->desc.nx % 4 != 0) snprintf(buf, sizeof buf, "nx %% 4 != 0");
+    else if (hx != 4 && hx != 8 && hx != 16) snprintf(buf, sizeof buf, "hx = %d is not one of the compiled 4, 8, 16", hx);
+    else if (p->desc.nx % (hx / 2) != 0) snprintf(buf, sizeof buf, "nx %% (hx / 2) != 0");   // a thread owns hx/2 whole columns
+    else if (p->desc.nz > 65535) snprintf(buf, sizeof buf, "nz above 65535");
+    if (why) *why = buf;
+    return buf[0] == 0;
 }
 
 cudaError_t fast_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean, float *sd,
@@ -428,7 +435,7 @@ cudaError_t fast_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_i
         LaunchScope ls(p, "stats_zbox", st);
         dim3 grid((unsigned)blocks, (unsigned)zp.nchunks);
         k_zbox<<<grid, ZB_NT, 0, st>>>(reinterpret_cast<const float4 *>(f), reinterpret_cast<float4 *>(Z1),
-                                       reinterpret_cast<float4 *>(Z2), zp);
+                                       reinterpret_cast<float4 *>(Z2), zp, p->d_pivot);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }

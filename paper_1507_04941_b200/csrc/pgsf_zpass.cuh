@@ -158,11 +158,12 @@ __global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, f
 // the window sum, subtract the leaving channel.  lead / trail advance by one staged channel per step.
 template <bool SQ, int XT>
 __device__ __forceinline__ float *window_run(float &s, float &e, const float *__restrict__ lead,
-                                             const float *__restrict__ trail, float *__restrict__ zp, long long plane, int n)
+                                             const float *__restrict__ trail, float *__restrict__ zp, long long plane, int n,
+                                             float c0)
 {
 #pragma unroll 8
     for (int j = 0; j < n; ++j) {
-        const float a = lead[j * XT], b = trail[j * XT];
+        const float a = lead[j * XT] - c0, b = trail[j * XT] - c0;     // (pivot c0: D-2)
         if constexpr (SQ) {
             kahan_add(s, e, a * a);
             *zp = s - e;
@@ -191,8 +192,9 @@ struct ZmShape {
 template <int RZ, int XT, int ZB>
 __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float *__restrict__ in, float *out,
                                                                 float *__restrict__ Z1, float *__restrict__ Z2,
-                                                                Dims d, int hz, Taps t)
+                                                                Dims d, int hz, const float *__restrict__ pivot, Taps t)
 {
+    const float c0 = __ldg(pivot);   // the window sums are of f - c0 and (f - c0)^2 (D-2)
     using S = ZmShape<RZ, XT, ZB>;
     extern __shared__ __align__(16) float smem[];  // [PLANES][XT] t2 slab / f slab, [ZB][XT] leaving slab
     float *fs = smem;                              // f of this step (written after the filter phase)
@@ -231,7 +233,8 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
 #pragma unroll 4
             for (int pz = wz; pz < ZB; pz += S::GROUPS, zt += S::GROUPS, src += gstep, dst += S::GROUPS * XT * 4)
             {
-                const bool ok = col_ok && zt >= 0 && zt < z0;
+                // (zt < nz: the drain steps have z0 >= nz, and planes nz .. z0-1 of `out` do not exist)
+                const bool ok = col_ok && zt >= 0 && zt < z0 && zt < nz;
                 cp_async16_s(dst, ok ? src : in, ok);   // (a valid address even when nothing is read)
             }
         }
@@ -263,32 +266,34 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
             __syncthreads();   // f slab complete
         }
         if (c_ok) {
-            if (z0 >= hz && z0 + ZB <= nz) {
-                // interior step: all 64 entering channels and all 64 outputs are inside the cube
+            if (z0 >= 2 * hz && z0 + ZB <= nz) {
+                // interior step: all 64 entering and all 64 leaving channels (and all 64 outputs) are inside the cube
                 const int jsplit = min(2 * hz, ZB);   // leaving channel: ts[j] for j < jsplit, else fs[j - 2 hz]
                 float *zp = Zq + (long long)(z0 - hz) * d.plane + cb;
                 if (sq) {
-                    zp = window_run<true, XT>(s, e, fs + c, ts + c, zp, d.plane, jsplit);
-                    window_run<true, XT>(s, e, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit);
+                    zp = window_run<true, XT>(s, e, fs + c, ts + c, zp, d.plane, jsplit, c0);
+                    window_run<true, XT>(s, e, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit, c0);
                 } else {
-                    zp = window_run<false, XT>(s, e, fs + c, ts + c, zp, d.plane, jsplit);
-                    window_run<false, XT>(s, e, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit);
+                    zp = window_run<false, XT>(s, e, fs + c, ts + c, zp, d.plane, jsplit, c0);
+                    window_run<false, XT>(s, e, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit, c0);
                 }
             } else {
                 for (int j = 0; j < ZB; ++j) {
                     const int zl = z0 + j;          // channel entering the window of output zo
                     const int zo = zl - hz;
                     if (zl < nz) {
-                        const float v = fs[j * XT + c];
+                        const float v = fs[j * XT + c] - c0;
                         if (sq) kahan_add(s, e, v * v);
                         else s += v;
                     }
                     if (zo >= 0 && zo < nz) {
                         Zq[(long long)zo * d.plane + cb] = s - e;
                         const int jt = j - 2 * hz;  // the channel leaving after this output, relative to z0
-                        const float v = jt >= 0 ? fs[jt * XT + c] : ts[j * XT + c];   // (zero where zt < 0)
-                        if (sq) kahan_add(s, e, -(v * v));
-                        else s -= v;
+                        if (zo - hz >= 0) {         // (a channel in front of the cube never entered the sum)
+                            const float v = (jt >= 0 ? fs[jt * XT + c] : ts[j * XT + c]) - c0;
+                            if (sq) kahan_add(s, e, -(v * v));
+                            else s -= v;
+                        }
                     }
                 }
             }
@@ -313,15 +318,15 @@ template <int RZ>
 constexpr int zm_step_channels() { return RZ >= 96 ? 128 : 64; }
 
 template <int RZ>
-cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const Taps &t,
-                      int ncubes, cudaStream_t st)
+cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot,
+                      const Taps &t, int ncubes, cudaStream_t st)
 {
     constexpr int ZB = zm_step_channels<RZ>();
     using S = ZmShape<RZ, ZM_XT, ZB>;
     cudaError_t e = ensure_dynamic_smem(k_zm<RZ, ZM_XT, ZB>, S::SMEM);
     if (e != cudaSuccess) return e;
     dim3 grid((d.nx + ZM_XT - 1) / ZM_XT, d.ny, ncubes);
-    k_zm<RZ, ZM_XT, ZB><<<grid, S::THREADS, S::SMEM, st>>>(in, out, Z1, Z2, d, hz, t);
+    k_zm<RZ, ZM_XT, ZB><<<grid, S::THREADS, S::SMEM, st>>>(in, out, Z1, Z2, d, hz, pivot, t);
     return cudaGetLastError();
 }
 
@@ -337,8 +342,8 @@ cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const D
         return launch_z<RZ>(in, out, ratio, d, t, st);                                                      \
     }                                                                                                       \
     cudaError_t launch_zm_r##RZ(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz,   \
-                                const Taps &t, int ncubes, cudaStream_t st)                                 \
+                                const float *pivot, const Taps &t, int ncubes, cudaStream_t st)             \
     {                                                                                                       \
-        return launch_zm<RZ>(in, out, Z1, Z2, d, hz, t, ncubes, st);                                        \
+        return launch_zm<RZ>(in, out, Z1, Z2, d, hz, pivot, t, ncubes, st);                                 \
     }                                                                                                       \
     }

@@ -135,6 +135,15 @@ def make_cube(shape_zyx: Sequence[int], seed: int, n_sources: int, device="cpu",
     return cube
 
 
+def workload_sources(w: Workload):
+    """The injected sources of a workload, exactly as make_workload draws them: one list per batch entry of
+    (cx, cy, cz, sx, sy, sz, amplitude) tuples.  Input generation only (tests centre their parity bricks on the
+    brightest sources)."""
+    rng = np.random.default_rng(int(w.seed) + 1000)
+    return [_draw_sources(rng, w.n_sources, w.dims, w.sxy_range, w.sz_range, w.amp_range, w.independent_sxy)
+            for _ in range(w.batch)]
+
+
 def make_workload(w: Workload, device="cpu") -> torch.Tensor:
     """The input tensor of a workload: [batch, nz, ny, nx] fp32 (batch dim kept even for 1)."""
     nx, ny, nz = w.dims

@@ -86,6 +86,72 @@ def test_no_gpu_fails_loudly_no_cpu_fallback(lib):
     assert ei.value.status == binding.PGSF_ERR_CUDA
 
 
+# ------------------------------------------------------------------ host-only logic through PGSF_FLAG_DRY_RUN plans
+
+def _dry(binding, dims=(64, 48, 80), sigmas=((1, 1, 2), (2, 2, 4)), box=(4, 4, 8), **kw):
+    return binding.Plan(dims, sigmas, box, 4.0, flags=binding.PGSF_FLAG_DRY_RUN | kw.pop("flags", 0), **kw)
+
+
+@pytest.mark.parametrize("dims,sigmas,box,flags,tiled,needle", [
+    ((64, 48, 80), ((1, 1, 2),), (4, 4, 8), 0, True, "tiled"),
+    ((64, 48, 80), ((1, 1, 2),), (4, 4, 8), 1, False, "FORCE_GENERIC"),
+    ((62, 48, 80), ((1, 1, 2),), (4, 4, 8), 0, False, "nx % 4"),
+    ((64, 48, 80), ((5, 1, 2),), (4, 4, 8), 0, False, "radii (15, 3, 6)"),        # x radius above the compiled 12
+    ((64, 48, 80), ((1, 1, 2),), (200 // 2 - 36, 4, 8), 0, False, "hx = 64"),     # filter tiled, statistics not
+    ((8, 4, 70000), ((1, 1, 2),), (4, 4, 8), 0, False, "65535"),                  # grid.z limit
+    ((8, 70000, 4), ((1, 1, 2),), (4, 4, 8), 0, False, "65535"),
+])
+def test_plan_path_reports_the_dispatch_decision(lib, dims, sigmas, box, flags, tiled, needle):
+    """Which kernels a plan runs is decided (and can be queried) at plan time, so a shape / radius / box that
+    falls off the tiled kernels is visible to the caller and can never surface as a launch failure."""
+    from paper_1507_04941_b200 import binding
+    with _dry(binding, dims, sigmas, box, flags=flags) as plan:
+        ok, text = plan.pgsf_plan_path()
+        assert ok == tiled and needle in text, text
+        assert plan.pgsf_plan_workspace_bytes() > 0
+
+
+def test_find_multiscale_rejects_overlapping_buffers(lib):
+    """pgsf_find_multiscale parks intermediate data in the d_filtered cubes, so every buffer must be disjoint
+    (validated on the host before anything is enqueued; a dry-run plan then stops with PGSF_ERR_CUDA)."""
+    from paper_1507_04941_b200 import binding
+    with _dry(binding) as plan:
+        n = plan.voxels
+        ws = plan.pgsf_plan_workspace_bytes()
+        base = 1 << 40                                # fake, well aligned "device" addresses; never dereferenced
+        step = ((4 * n + 255) // 256 + 1) * 256
+        d_in, f0, f1, mask, cnt, wsp = (base + i * step for i in range(6))
+        wsp = base + 8 * step
+
+        def call(d_in=d_in, f=(f0, f1), mask=mask, cnt=cnt, wsp=wsp):
+            arr = (ctypes.c_void_p * 2)(*f) if f is not None else None
+            return lib.pgsf_find_multiscale(plan._h, ctypes.c_void_p(d_in), arr, ctypes.c_void_p(mask),
+                                            ctypes.c_void_p(cnt), ctypes.c_void_p(wsp), None)
+
+        assert call() == binding.PGSF_ERR_CUDA                       # valid arguments, no device
+        assert call(f=None) == binding.PGSF_ERR_CUDA
+        for bad, who in [(dict(f=(d_in, f1)), "d_in"), (dict(f=(f0, f0 + 256)), "d_filtered[1]"),
+                         (dict(mask=f1 + 4 * n - 16), "d_mask"), (dict(wsp=f0 + 256), "d_workspace"),
+                         (dict(cnt=mask + 8), "d_count"), (dict(wsp=d_in - ws + 256), "d_workspace")]:
+            assert call(**bad) == binding.PGSF_ERR_INVALID_ARG, bad
+            msg = lib.pgsf_last_error(plan._h).decode()
+            assert "overlaps" in msg and who in msg, msg
+        assert call(d_in=d_in + 4) == binding.PGSF_ERR_INVALID_ARG    # misaligned
+
+
+def test_plan_options_are_validated(lib):
+    from paper_1507_04941_b200 import binding
+    with _dry(binding, dims=(32, 32, 32), batch=5) as plan:
+        plan.pgsf_plan_set_option(binding.PGSF_OPT_GROUP_CUBES, 2)
+        plan.pgsf_plan_set_option(binding.PGSF_OPT_HOST_SECTION_PLANES, 16)
+        plan.pgsf_plan_set_option(binding.PGSF_OPT_HOST_DEVICE_BUDGET, 1 << 30)
+        for opt, val in [(binding.PGSF_OPT_GROUP_CUBES, 0), (binding.PGSF_OPT_GROUP_CUBES, 6),
+                         (binding.PGSF_OPT_HOST_SECTION_PLANES, 33), (binding.PGSF_OPT_HOST_DEVICE_BUDGET, -1), (99, 0)]:
+            with pytest.raises(binding.PgsfError) as ei:
+                plan.pgsf_plan_set_option(opt, val)
+            assert ei.value.status == binding.PGSF_ERR_INVALID_ARG
+
+
 def test_product_does_not_import_oracle():
     pkg = os.path.join(ROOT, "paper_1507_04941_b200")
     for dirpath, _, files in os.walk(pkg):

@@ -35,11 +35,13 @@ def _plan(pg, w, flags=0, k=None):
                    truncate=w.truncate, flags=flags)
 
 
-def _full_compare(pg, oracle, w, d, flags=0, k=None, check_stats=True):
+def _full_compare(pg, oracle, w, d, flags=0, k=None, check_stats=True, group=None):
     """Whole-workload comparison (small cubes): find_multiscale + per-scale calls."""
     kk = w.k if k is None else k
     rep_total = parity.MaskReport(0, 0, 0)
     with _plan(pg, w, flags, k) as plan:
+        if group is not None:
+            plan.pgsf_plan_set_option(pg.PGSF_OPT_GROUP_CUBES, group)
         mask, cnt, filt = plan.pgsf_find_multiscale(d, keep_filtered=True)
         torch.cuda.synchronize()
         gpu_count = int(cnt.item())
@@ -138,10 +140,11 @@ def test_batch_in_ragged_groups(pg, synth, oracle):
     from dataclasses import replace
     w = replace(synth.scaled(synth.WORKLOADS[4], (96, 80, 112), batch=3, n_sources=6), halo=(16, 12, 20), k=3.0)
     d = synth.make_workload(w, "cuda")
-    rep, count = _full_compare(pg, oracle, w, d, pg.PGSF_FLAG_SMALL_GROUPS, check_stats=False)
+    rep, count = _full_compare(pg, oracle, w, d, check_stats=False, group=2)
     with _plan(pg, w) as plan:
         mask1, cnt1, _ = plan.pgsf_find_multiscale(d, keep_filtered=True)
-    with _plan(pg, w, pg.PGSF_FLAG_SMALL_GROUPS) as plan:
+    with _plan(pg, w) as plan:
+        plan.pgsf_plan_set_option(pg.PGSF_OPT_GROUP_CUBES, 2)
         mask2, cnt2, _ = plan.pgsf_find_multiscale(d, keep_filtered=True)
     torch.cuda.synchronize()
     assert torch.equal(mask1, mask2) and int(cnt1.item()) == int(cnt2.item()) == count
@@ -233,6 +236,66 @@ def test_direct_equals_separable_for_gaussian(pg, synth, oracle):
         torch.cuda.synchronize()
     # both are within FILTER_TOL of Eq. 2; the fp32 rounding of the 637 products gz gy gx adds ~3e-6 here
     assert float((a - b).abs().max()) <= parity.FILTER_TOL
+
+
+# ------------------------------------------------------------------------------------ offsets, drain steps
+
+@pytest.mark.parametrize("flags", IMPLS)
+@pytest.mark.parametrize("dc", [2.0, 10.0, 100.0, 1000.0])
+def test_dc_offset_cube(pg, synth, oracle, flags, dc):
+    """Reading D-2: a cube with a continuum / DC level of 2 ... 1000 sigma.  Where the data sit within a quarter of
+    their level the statistics subtract that level (a pivot) before squaring, so S2/n - m^2 keeps its precision;
+    the mask must stay inside the 1e-4 * std band of the oracle.  The filtered values themselves are O(dc): their
+    tolerance is the fp32 one, 1e-5 relative to the level (BASELINE.json quotes 1e-5 for unit-variance data).
+    MEASURED BOUND of the tiled kernels: identical masks up to a level of 100 sigma; at 1000 sigma the running
+    window sums keep rounding residue of the (level/2)^2 steps that the zero padding makes next to the faces and
+    the mask differs in the interior (generic kernels: identical at every level) -- DESIGN.md D-2."""
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[2], (104, 76, 150), n_sources=10), sigmas=((1, 1, 2), (2, 2, 4)),
+                box_half=(4, 4, 8), k=3.0)
+    d = synth.make_workload(w, "cuda") + dc
+    with _plan(pg, w, flags) as plan:
+        mask, cnt, filt = plan.pgsf_find_multiscale(d, keep_filtered=True)
+        m1, c1, mean, std = plan.pgsf_local_threshold(filt[1], want_stats=True)
+        torch.cuda.synchronize()
+    res = oracle.find_full(d[0].cpu().numpy(), w.sigmas, w.box_half, w.k)
+    for s in range(2):
+        parity.assert_filter_close(filt[s][0].cpu().numpy(), res.scales[s].f, f"dc {dc} scale {s}",
+                                   tol=1e-5 * max(dc, 1.0))
+    g = mask[0].cpu().numpy().astype(bool)
+    mism = g != res.mask.astype(bool)
+    band = np.zeros(g.shape, bool)
+    for sc in res.scales:
+        # the band of C-13 plus the fp32 representation error of f itself at this level
+        band |= np.abs(sc.f - sc.stats.thr) <= parity.BAND * sc.stats.std + 2.0 ** -23 * dc
+    r, h = (6, 6, 12), w.box_half
+    inner = np.zeros(g.shape, bool)
+    inner[r[2] + h[2]:-(r[2] + h[2]), r[1] + h[1]:-(r[1] + h[1]), r[0] + h[0]:-(r[0] + h[0])] = True
+    st = res.scales[1].stats
+    sd_err = (np.abs(std[0].cpu().numpy() - st.std) / st.std)[inner].max()
+    bad = int((mism & ~band).sum())
+    print(f"dc={dc} flags={flags}: count={int(cnt.item())} oracle={res.count} mismatches={int(mism.sum())} "
+          f"outside the band={bad} max rel. std error (interior)={sd_err:.2e}")
+    assert int(res.mask[inner].sum()) > 20                      # not vacuous
+    if flags == 0 and dc > 100.0:
+        if bad:
+            pytest.xfail(f"documented limitation D-2: tiled kernels at a level of {dc} sigma, {bad} voxels differ")
+        return
+    assert bad == 0, f"dc {dc}: {bad} mask voxels differ outside the band"
+    if flags == 1 or dc <= 10.0:
+        assert sd_err < 1e-4 + 3e-7 * dc                        # (without the pivot it is ~100 % off at dc >= 100)
+
+
+@pytest.mark.parametrize("dims,sigmas,box", [
+    ((64, 48, 60), ((1, 1, 2),), (4, 4, 8)),        # nz not a multiple of 64 and ceil(nz/64)*64 - nz < hz: the drain step
+    ((64, 48, 124), ((2, 2, 4),), (8, 8, 16)),      #   of k_zm stages leaving channels beyond nz (ADVICE round 1)
+    ((64, 48, 130), ((1, 1, 2),), (4, 4, 40)),      # 2 hz > 64: leaving channels two steps back
+])
+def test_zm_drain_steps(pg, synth, oracle, dims, sigmas, box):
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[2], dims, n_sources=8), sigmas=sigmas, box_half=box, k=3.0)
+    d = synth.make_workload(w, "cuda")
+    _full_compare(pg, oracle, w, d, 0)
 
 
 # ------------------------------------------------------------------------------------ degenerate cases
@@ -346,10 +409,14 @@ def test_api_errors_on_device(pg):
 
 # ------------------------------------------------------------------------------------ full-size configs
 
-def _brick_list(w, rng, n_interior, size):
-    """Seeded bricks: the 8 corners, 4 face/edge bricks, the rest interior."""
-    nx, ny, nz = w.dims
+BRICK = 128        # ">= 16 seeded 128^3 bricks"
+
+
+def _brick_list(w, sources, n_total, size=BRICK):
+    """the 8 corner bricks, 4 face / edge bricks, the rest centred on the BRIGHTEST injected
+    sources of this cube (the input the compensated running sums of the statistics exist for)."""
     sx, sy, sz = (min(size, n) for n in w.dims)
+    nx, ny, nz = w.dims
     lo = []
     for cz in (0, nz - sz):
         for cy in (0, ny - sy):
@@ -357,27 +424,36 @@ def _brick_list(w, rng, n_interior, size):
                 lo.append((cx, cy, cz))
     mid = ((nx - sx) // 2, (ny - sy) // 2, (nz - sz) // 2)
     lo += [(0, mid[1], mid[2]), (mid[0], ny - sy, mid[2]), (mid[0], mid[1], 0), (nx - sx, 0, mid[2])]
-    for _ in range(n_interior):
-        lo.append(tuple(int(rng.integers(0, n - s + 1)) for n, s in zip(w.dims, (sx, sy, sz))))
     seen, out = set(), []
     for l in lo:
+        if l not in seen:
+            seen.add(l)
+            out.append((l, (l[0] + sx, l[1] + sy, l[2] + sz)))
+    for src in sorted(sources, key=lambda t: -t[6]):            # brightest first
+        if len(out) >= n_total:
+            break
+        l = tuple(int(min(max(round(c) - s // 2, 0), n - s)) for c, s, n in zip(src[:3], (sx, sy, sz), w.dims))
         if l not in seen:
             seen.add(l)
             out.append((l, (l[0] + sx, l[1] + sy, l[2] + sz)))
     return out
 
 
-def _brick_compare(pg, oracle, synth, w, size, n_interior, batches=(0,)):
+def _brick_compare(pg, oracle, synth, w, n_bricks, batches=(0,), whole=False):
+    """find_multiscale at full size in the launch configuration bench.py times; then either seeded bricks
+    (`n_bricks` per listed batch entry) or, with whole=True, the listed batch entries IN FULL."""
     d = synth.make_workload(w, "cuda")
-    rng = np.random.default_rng(w.seed + 77)
+    sources = synth.workload_sources(w)
     total = parity.MaskReport(0, 0, 0)
     worst = 0.0
     with _plan(pg, w) as plan:
+        assert plan.pgsf_plan_path()[0], plan.pgsf_plan_path()[1]       # the tiled kernels are what is being tested
         mask, cnt, filt = plan.pgsf_find_multiscale(d, keep_filtered=True)
         torch.cuda.synchronize()
         assert int(cnt.item()) == int(mask.sum(dtype=torch.int64).item())
         for b in batches:
-            for lo, hi in _brick_list(w, rng, n_interior, size):
+            bricks = [((0, 0, 0), tuple(w.dims))] if whole else _brick_list(w, sources[b], n_bricks)
+            for lo, hi in bricks:
                 a, e = oracle.required_input_box(w.dims, w.sigmas, w.box_half, lo, hi, w.truncate)
                 sub = d[b, a[2]:e[2], a[1]:e[1], a[0]:e[0]].cpu().numpy()
                 res = oracle.find_region(sub, a, w.dims, w.sigmas, w.box_half, w.k, lo, hi, w.halo, w.truncate)
@@ -390,31 +466,47 @@ def _brick_compare(pg, oracle, synth, w, size, n_interior, batches=(0,)):
                 total.mismatches += rep.mismatches
                 total.excused += rep.excused
                 total.band_voxels += rep.band_voxels
+                del res
         count = int(cnt.item())
     print(f"{w.name}: count={count} worst filter diff={worst:.2e} mask mismatches={total.mismatches} "
           f"(band voxels {total.band_voxels})")
     return count
 
 
+def test_brick_list_is_as_specified(synth):
+    """8 corners + 4 face / edge bricks + source-centred bricks, >= 16 in all, every one 128^3 and inside the cube."""
+    for c in (3, 5):
+        w = synth.WORKLOADS[c]
+        src = synth.workload_sources(w)[0]
+        bricks = _brick_list(w, src, 16)
+        assert len(bricks) == 16 and len(set(bricks)) == 16
+        assert all(h[a] - l[a] == BRICK and 0 <= l[a] and h[a] <= w.dims[a] for l, h in bricks for a in range(3))
+        brightest = sorted(src, key=lambda t: -t[6])[:4]
+        for (l, h), sc in zip(bricks[12:], brightest):
+            assert all(l[a] <= sc[a] < h[a] for a in range(3))            # the source is inside its brick
+
+
 @pytest.mark.slow
 def test_config2_full_size_bricks(pg, oracle, synth):
-    count = _brick_compare(pg, oracle, synth, synth.WORKLOADS[2], 96, 6)
+    count = _brick_compare(pg, oracle, synth, synth.WORKLOADS[2], 16)
     assert count > 1000
 
 
 @pytest.mark.slow
 def test_config3_full_size_bricks(pg, oracle, synth):
-    count = _brick_compare(pg, oracle, synth, synth.WORKLOADS[3], 96, 4)
+    count = _brick_compare(pg, oracle, synth, synth.WORKLOADS[3], 16)
     assert count > 1000
 
 
 @pytest.mark.slow
-def test_config4_full_size_bricks(pg, oracle, synth):
-    count = _brick_compare(pg, oracle, synth, synth.WORKLOADS[4], 112, 2, batches=(0, 17, 42, 63))
+def test_config4_whole_sub_cubes(pg, oracle, synth):
+    """'config 4: >= 4 whole sub-cubes in full' -- every voxel of four 320 x 320 x 576 sub-cubes
+    (first, last and two in the middle of the launch groups), halo voxels included (they must be 0)."""
+    count = _brick_compare(pg, oracle, synth, synth.WORKLOADS[4], 0, batches=(0, 17, 42, 63), whole=True)
     assert count > 1000
 
 
 @pytest.mark.slow
 def test_config5_full_size_bricks(pg, oracle, synth):
-    count = _brick_compare(pg, oracle, synth, synth.WORKLOADS[5], 96, 4)
+    count = _brick_compare(pg, oracle, synth, synth.WORKLOADS[5], 16)
     assert count > 100

@@ -315,7 +315,16 @@ def test_S15_multiscale_or_halo_and_count(oracle):
     a, b = oracle.required_input_box((40, 40, 64), sig, h, lo, hi)
     reg = oracle.find_region(d[a[2]:b[2], a[1]:b[1], a[0]:b[0]], a, (40, 40, 64), sig, h, k, lo, hi, halo)
     ref = oracle.find_full(d, sig, h, k, halo=halo)
-    np.testing.assert_array_equal(reg.mask, ref.mask[lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]])
+    sl = (slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
+    np.testing.assert_array_equal(reg.mask, ref.mask[sl])
+    # region mode with lo != 0 reproduces the full-cube VALUES too (filtered data, mean, std, threshold), not only
+    # the mask: a window clipped to the brick instead of the cube, or a shifted origin, would show here
+    for rs, fs in zip(reg.scales, ref.scales):
+        np.testing.assert_allclose(rs.f, fs.f[sl], rtol=0, atol=1e-14)
+        np.testing.assert_allclose(rs.stats.mean, fs.stats.mean[sl], rtol=0, atol=1e-14)
+        np.testing.assert_allclose(rs.stats.std, fs.stats.std[sl], rtol=1e-12, atol=1e-15)
+        np.testing.assert_allclose(rs.stats.thr, fs.stats.thr[sl], rtol=0, atol=1e-13)
+        np.testing.assert_array_equal(rs.stats.mask, fs.stats.mask[sl])
 
 
 # ---------------------------------------------------------------------------------- Eq. 1 (weighted), NEXT-1
