@@ -271,6 +271,9 @@ def _path_roofline(w, taps, n_vox, ms_step, alu_peak, hbm_peak):
             "roofline_ms": t_path * 1e3, "frac": t_path * 1e3 / ms_step, "bound": "alu" if t_alu >= t_hbm else "hbm"}
 
 
+TUNE = 0      # --tune: PGSF_OPT_TUNE bits (kernel variants for A/B measurements; results are identical)
+
+
 def measure_workload(w, dev, device_index, rank, world, steps, warmup, peaks, sm_count, detail=True):
     """One workload on this rank's GPU: W warm-up steps, K timed steps (CUDA events on the launching stream,
     per-launch profiling events OFF), then -- with detail -- a second, profiled pass for the per-kernel table and
@@ -285,6 +288,8 @@ def measure_workload(w, dev, device_index, rank, world, steps, warmup, peaks, sm
     taps = _taps(w)
     plan = binding.Plan(w.dims, w.sigmas, w.box_half, w.k, batch=w.batch, halo=w.halo, truncate=w.truncate,
                         device=device_index)
+    if TUNE:
+        plan.pgsf_plan_set_option(binding.PGSF_OPT_TUNE, TUNE)
     filt = [torch.empty_like(d) for _ in range(S)]
     mask = torch.empty(d.shape, dtype=torch.uint8, device=dev)
     cnt = torch.zeros(1, dtype=torch.int64, device=dev)
@@ -758,11 +763,14 @@ def main():
                     help="find = the hot path (default); weighted = Eq. 1 of the paper (NEXT-1); direct = Eq. 2 for "
                          "an arbitrary filter array (NEXT-2); the last two single GPU")
     ap.add_argument("--fp64", action="store_true", help="--path direct: accumulate in fp64 as the paper does")
+    ap.add_argument("--tune", type=int, default=0, help="PGSF_OPT_TUNE bits (kernel variants; same results)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true",
                     help="skip the ms-per-step sweep over the other BASELINE.json configs after the headline")
     args = ap.parse_args()
+    global TUNE
+    TUNE = args.tune
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
     from paper_1507_04941_b200 import synth
     w = synth.WORKLOADS[args.config]

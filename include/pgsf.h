@@ -107,11 +107,14 @@ PGSF_API pgsf_status pgsf_plan_destroy(pgsf_plan *plan);
  *                                 cube ("section = core + halo"); 0 = chosen from the device budget.
  *   PGSF_OPT_HOST_DEVICE_BUDGET   pgsf_find_multiscale_host: bytes of device memory its staging may use;
  *                                 0 = 80 % of the memory free at the first call.
+ *   PGSF_OPT_TUNE                 measurement aid, a bit set: 1 = statistics kernel without L2 eviction hints,
+ *                                 2 = the previous statistics kernel (k_ymarch) instead of k_xyb.
  * INVALID_ARG for an unknown option or a value outside its range.
  */
 #define PGSF_OPT_GROUP_CUBES 1
 #define PGSF_OPT_HOST_SECTION_PLANES 2
 #define PGSF_OPT_HOST_DEVICE_BUDGET 3
+#define PGSF_OPT_TUNE 4
 PGSF_API pgsf_status pgsf_plan_set_option(pgsf_plan *plan, int option, long long value);
 
 /*

@@ -243,6 +243,7 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
     else if (!grid_ok) p->why_stats = "ny or nz above 65535";
     p->host_section_planes = 0;
     p->host_budget = 0;
+    p->tune = 0;
 
     // workspace: [scratch filtered cube][filter temporaries][statistics temporaries]
     p->ws_cube_bytes = round256((size_t)p->dims.cube * sizeof(float));
@@ -306,6 +307,10 @@ pgsf_status pgsf_plan_set_option(pgsf_plan *p, int option, long long value)
         if (value < 0) return fail(p, PGSF_ERR_INVALID_ARG, "PGSF_OPT_HOST_DEVICE_BUDGET must be >= 0");
         if (value != p->host_budget && !p->dry) { cudaSetDevice(p->device); pgsf::host_release(p); }
         p->host_budget = value;
+        return PGSF_OK;
+    case PGSF_OPT_TUNE:
+        if (value < 0 || value > 0xffff) return fail(p, PGSF_ERR_INVALID_ARG, "PGSF_OPT_TUNE must be in 0..65535");
+        p->tune = (int)value;
         return PGSF_OK;
     default:
         return fail(p, PGSF_ERR_INVALID_ARG, "unknown option %d", option);
@@ -641,8 +646,12 @@ pgsf_status pgsf_find_multiscale(pgsf_plan *p, const float *d_in, float *const *
                     float *Z1 = w.stmp, *Z2 = w.stmp + (size_t)p->group_max * p->dims.cube;
                     ce = pgsf::fast_zm(p, s, park[s], d_filtered[s] + off, Z1, Z2, nb, st);
                     if (ce != cudaSuccess) return cuda_fail(p, ce, "z filter + window launch");
-                    ce = pgsf::fast_threshold_xy(p, d_filtered[s] + off, Z1, Z2, d_mask + off, s > 0, nullptr,
-                                                 nullptr, (s == S - 1) ? d_count : nullptr, nb, st);
+                    // scales after the first OR into the mask: sparsely where the kernel can (then every scale adds
+                    // its newly set voxels to the count), else densely with the count taken by the last scale
+                    const bool sparse = pgsf::stats_sparse_or(p);
+                    ce = pgsf::fast_threshold_xy(p, d_filtered[s] + off, Z1, Z2, d_mask + off,
+                                                 s == 0 ? 0 : (sparse ? 2 : 1), nullptr, nullptr,
+                                                 (sparse || s == S - 1) ? d_count : nullptr, nb, st);
                     if (ce != cudaSuccess) return cuda_fail(p, ce, "threshold launch");
                     continue;
                 }
@@ -668,8 +677,11 @@ pgsf_status pgsf_find_multiscale(pgsf_plan *p, const float *d_in, float *const *
                 if (ce == cudaSuccess) ce = pgsf::fast_xy_multi(p, &s, 1, d_in + off, t2, 1, st);
                 if (ce == cudaSuccess) ce = pgsf::fast_zm(p, s, w.ftmp, f, Z1, Z2, 1, st);
                 if (ce == cudaSuccess)
-                    ce = pgsf::fast_threshold_xy(p, f, Z1, Z2, d_mask + off, s > 0, nullptr, nullptr,
-                                                 (s == S - 1) ? d_count : nullptr, 1, st);
+                {
+                    const bool sparse = pgsf::stats_sparse_or(p);
+                    ce = pgsf::fast_threshold_xy(p, f, Z1, Z2, d_mask + off, s == 0 ? 0 : (sparse ? 2 : 1), nullptr,
+                                                 nullptr, (sparse || s == S - 1) ? d_count : nullptr, 1, st);
+                }
                 if (ce != cudaSuccess) return cuda_fail(p, ce, "filter / threshold launch");
                 continue;
             }

@@ -82,6 +82,7 @@ struct pgsf_plan {
     std::string why_filter, why_stats;   // why a stage runs the generic kernels ("" = tiled); pgsf_plan_path
     long long host_section_planes;       // PGSF_OPT_HOST_SECTION_PLANES (0 = automatic)
     long long host_budget;               // PGSF_OPT_HOST_DEVICE_BUDGET  (0 = automatic)
+    int tune;                            // PGSF_OPT_TUNE bits (measurement aid; no bit changes a result)
     unsigned long long launches;
     std::string err;
     bool prof_on;
@@ -141,9 +142,16 @@ bool fast_stats_supported(const pgsf_plan *p, std::string *why);
 // frees the plan-owned staging of pgsf_find_multiscale_host (buffers, streams, events); the plan's device must be current
 void host_release(pgsf_plan *p);
 // x/y window sums + selection from precomputed z-direction window sums Z1, Z2 (of fast_zm / k_zbox)
+// mode: 0 overwrite the mask, 1 OR into it (count = all set voxels), 2 sparse OR (only with stats_sparse_or():
+// touches only newly selected bytes, count += voxels that were not set before)
 cudaError_t fast_threshold_xy(pgsf_plan *p, const float *f, const float *Z1, const float *Z2, uint8_t *mask,
-                              int or_into, float *mean, float *sd, unsigned long long *count, int ncubes,
+                              int mode, float *mean, float *sd, unsigned long long *count, int ncubes,
                               cudaStream_t st);
+// k_xyb (pgsf_xyb.cu): the successor of k_ymarch; same arguments
+bool xyb_supported(const pgsf_plan *p);
+inline bool stats_sparse_or(const pgsf_plan *p) { return p->fast_stats && xyb_supported(p) && !(p->tune & 2); }
+cudaError_t xyb_threshold(pgsf_plan *p, const float *f, const float *Z1, const float *Z2, uint8_t *mask, int mode,
+                          float *mean, float *sd, unsigned long long *count, int ncubes, cudaStream_t st);
 // tmp2: 2 cubes (the z-direction window sums of f and f^2)
 cudaError_t fast_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean,
                            float *sd, unsigned long long *count, float *tmp2, cudaStream_t st);

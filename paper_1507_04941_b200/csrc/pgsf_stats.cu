@@ -443,9 +443,12 @@ cudaError_t fast_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_i
 }
 
 cudaError_t fast_threshold_xy(pgsf_plan *p, const float *f, const float *Z1, const float *Z2, uint8_t *mask,
-                              int or_into, float *mean, float *sd, unsigned long long *count, int ncubes,
+                              int mode, float *mean, float *sd, unsigned long long *count, int ncubes,
                               cudaStream_t st)
 {
+    if (xyb_supported(p) && !(p->tune & 2)) return xyb_threshold(p, f, Z1, Z2, mask, mode, mean, sd, count, ncubes, st);
+    if (mode == 2) return cudaErrorNotSupported;   // (callers ask stats_sparse_or() first)
+    const int or_into = mode;
     const Dims &d = p->dims;
     YmParams yp;
     yp.d = d;

@@ -377,6 +377,36 @@ def test_or_into_and_count_semantics(pg, synth):
         assert set(torch.unique(mm).tolist()) <= {0, 1}
 
 
+@pytest.mark.parametrize("dims,box", [((300, 90, 70), (16, 16, 8)), ((520, 60, 40), (8, 5, 6)), ((136, 70, 50), (4, 9, 3))])
+def test_stats_kernel_variants(pg, synth, dims, box):
+    """PGSF_OPT_TUNE changes kernels, never results: k_xyb with and without L2 eviction hints and the previous
+    statistics kernel (k_ymarch) give the same mask and count (both sum the same windows; their y-direction
+    running sums round alike, their x-direction sums associate differently, so voxels inside the band may differ:
+    the masks must agree except where the statistics themselves are within 1e-5 relative)."""
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[2], dims, n_sources=10), sigmas=((1, 1, 2), (2, 2, 4)), box_half=box, k=3.0)
+    d = synth.make_workload(w, "cuda")
+    out = []
+    for tune in (0, 1, 2):
+        with _plan(pg, w) as plan:
+            plan.pgsf_plan_set_option(pg.PGSF_OPT_TUNE, tune)
+            mask, cnt, filt = plan.pgsf_find_multiscale(d, keep_filtered=True)
+            m1, c1, mean, std = plan.pgsf_local_threshold(filt[0], want_stats=True)
+            m2 = m1.clone()
+            _, c2, _, _ = plan.pgsf_local_threshold(filt[1], d_mask=m2, or_into=True)
+            torch.cuda.synchronize()
+            assert int(cnt.item()) == int(mask.sum()) and int(c1.item()) == int(m1.sum())
+            assert int(c2.item()) == int(m2.sum()) and torch.equal(m2, mask)
+            out.append((mask, int(cnt.item()), mean, std))
+    assert out[0][1] > 0
+    assert torch.equal(out[0][0], out[1][0]) and out[0][1] == out[1][1]
+    assert torch.equal(out[0][2], out[1][2]) and torch.equal(out[0][3], out[1][3])
+    ndiff = int((out[0][0] != out[2][0]).sum())
+    assert ndiff <= 2, f"k_xyb and k_ymarch masks differ in {ndiff} voxels"
+    assert float((out[0][2] - out[2][2]).abs().max()) <= 1e-5 * float(out[2][3].max())
+    assert float(((out[0][3] - out[2][3]).abs() / out[2][3]).max()) <= 1e-4
+
+
 def test_host_entry_point_and_stream(pg, synth):
     dims = (64, 48, 80)
     d = synth.make_cube((dims[2], dims[1], dims[0]), 8, 6, device="cuda")[None]
