@@ -211,10 +211,16 @@ PGSF_API pgsf_status pgsf_find_multiscale(pgsf_plan *plan, const float *d_in, fl
                                  void *cuda_stream);
 
 /*
- * pgsf_find_multiscale_host -- same result from HOST buffers: copies h_in to plan-owned device
- * buffers (allocated on first use), runs pgsf_find_multiscale, copies the mask (and, when
- * h_filtered != NULL, the filtered cubes: n_scales host pointers) back, writes *h_count, and
- * synchronises.  Page-locked host memory makes the copies asynchronous but is not required.
+ * pgsf_find_multiscale_host -- same result (bit for bit) from HOST buffers, with plan-owned device
+ * staging (allocated on first use, released by pgsf_plan_destroy or by a change of the two host options).
+ * Plans that run the tiled kernels stream the cube through the device in sections along the frequency axis
+ * (the paper's "section = core + halo", Fig. 1 -- but with the copy in of section i+1 and the copy
+ * out of section i-1 under the compute of section i, every input plane copied once, nothing recomputed at the
+ * seams), so a cube larger than the device memory (or than PGSF_OPT_HOST_DEVICE_BUDGET) still runs; other plans
+ * copy the whole cube in, run pgsf_find_multiscale and copy the results out.  Writes the mask (and, when
+ * h_filtered != NULL, the filtered cubes: n_scales host pointers, NULL entries skipped) and *h_count, and
+ * synchronises.  Page-locked host memory makes the copies asynchronous (and overlapped) but is not required.
+ * OOM if the smallest possible sections do not fit the budget.
  */
 PGSF_API pgsf_status pgsf_find_multiscale_host(pgsf_plan *plan, const float *h_in, float *const *h_filtered,
                                       uint8_t *h_mask, unsigned long long *h_count);

@@ -87,6 +87,7 @@ namespace pgsf {
 
 void host_release(pgsf_plan *p)
 {
+    host_stage_release(p);
     cudaFree(p->h_d_in);
     cudaFree(p->h_d_mask);
     cudaFree(p->h_d_count);
@@ -196,6 +197,7 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
     p->h_d_count = nullptr;
     p->h_d_ws = nullptr;
     p->h_stream = nullptr;
+    p->hs = nullptr;
     for (int s = 0; s < PGSF_MAX_SCALES; ++s) p->h_d_f[s] = nullptr;
 
     const bool force_generic = (desc->flags & PGSF_FLAG_FORCE_GENERIC) != 0;
@@ -703,6 +705,12 @@ pgsf_status pgsf_find_multiscale_host(pgsf_plan *p, const float *h_in, float *co
     if (p->dry) return fail(p, PGSF_ERR_CUDA, "PGSF_FLAG_DRY_RUN plan: arguments are valid, but no device is attached");
     cudaError_t e = cudaSetDevice(p->device);
     if (e != cudaSuccess) return cuda_fail(p, e, "cudaSetDevice");
+    {
+        // the tiled kernels stream the cube through the device in sections (pgsf_host.cu); other plans stage it whole
+        bool handled = false;
+        const pgsf_status rs = pgsf::host_streamed(p, h_in, h_filtered, h_mask, h_count, &handled);
+        if (handled) return rs;
+    }
     const size_t nvox = (size_t)p->dims.cube * p->desc.batch;
     const int S = p->desc.n_scales;
     if (!p->h_d_in) {

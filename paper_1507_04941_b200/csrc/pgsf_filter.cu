@@ -20,17 +20,17 @@
 namespace pgsf {
 // per-radius entry points of the frequency-axis kernels (pgsf_z_r*.cu)
 cudaError_t launch_z_r6(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r6(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st);
+cudaError_t launch_zm_r6(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec);
 cudaError_t launch_z_r12(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r12(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st);
+cudaError_t launch_zm_r12(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec);
 cudaError_t launch_z_r24(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r24(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st);
+cudaError_t launch_zm_r24(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec);
 cudaError_t launch_z_r48(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r48(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st);
+cudaError_t launch_zm_r48(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec);
 cudaError_t launch_z_r72(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r72(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st);
+cudaError_t launch_zm_r72(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec);
 cudaError_t launch_z_r96(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r96(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st);
+cudaError_t launch_zm_r96(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec);
 
 namespace {
 
@@ -336,12 +336,12 @@ static bool xym_dispatch(int n, const int *rc, const float *in, const XymParams 
 // scales are sorted by compiled radius and cut into the largest groups a k_xym instance exists for;
 // every group reads the input once.
 cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *in, float *const *out, int ncubes,
-                          cudaStream_t st, bool box, const float *wgt)
+                          cudaStream_t st, bool box, const float *wgt, int nplanes)
 {
     // the x and y passes do not couple planes: `ncubes` consecutive cubes are one stack of ncubes * nz planes
     Dims d = p->dims;
-    d.nz *= ncubes;
-    d.cube *= ncubes;
+    d.nz = nplanes > 0 ? nplanes : d.nz * ncubes;
+    d.cube = d.plane * d.nz;
     if (d.nz > 65535 || n < 1 || n > PGSF_MAX_SCALES) return cudaErrorInvalidConfiguration;
     int order[PGSF_MAX_SCALES];
     for (int i = 0; i < n; ++i) order[i] = i;
@@ -416,8 +416,10 @@ cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStr
 
 // frequency pass of one scale fused with the z-direction window sums of the statistics:
 // in (x/y-filtered cube) -> out (filtered cube), Z1, Z2
+int zm_step_channels_of(int rz_compiled) { return rz_compiled >= 96 ? 128 : 64; }   // = zm_step_channels<RZ>()
+
 cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, int ncubes,
-                    cudaStream_t st)
+                    cudaStream_t st, const ZmSection *sec)
 {
     const Dims &d = p->dims;
     const ScalePlan &sp = p->scales[scale];
@@ -427,12 +429,12 @@ cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float 
     snprintf(name, sizeof name, "zm_s%d", scale);
     LaunchScope ls(p, name, st);
     switch (sp.rz_c) {
-    case 6: return launch_zm_r6(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st);
-    case 12: return launch_zm_r12(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st);
-    case 24: return launch_zm_r24(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st);
-    case 48: return launch_zm_r48(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st);
-    case 72: return launch_zm_r72(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st);
-    case 96: return launch_zm_r96(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st);
+    case 6: return launch_zm_r6(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec);
+    case 12: return launch_zm_r12(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec);
+    case 24: return launch_zm_r24(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec);
+    case 48: return launch_zm_r48(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec);
+    case 72: return launch_zm_r72(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec);
+    case 96: return launch_zm_r96(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec);
     default: return cudaErrorNotSupported;
     }
 }

@@ -44,23 +44,32 @@ __global__ void __launch_bounds__(kThreads) k_conv1d(const float *__restrict__ i
 constexpr int kPivotThreads = 1024;
 constexpr int kPivotAxis = 100;
 
-__global__ void __launch_bounds__(kPivotThreads) k_pivot(const float *__restrict__ data, Dims d, float *__restrict__ pivot)
+}  // namespace
+
+// the lattice: first sample, stride and number of samples per axis (host and device)
+__host__ __device__ inline void pivot_lattice_hd(const Dims &d, int lo[3], int st[3], int cnt[3])
+{
+    const int n[3] = {d.nx, d.ny, d.nz};
+    for (int a = 0; a < 3; ++a) {
+        lo[a] = n[a] / 4;
+        const int len = n[a] / 2 > 1 ? n[a] / 2 : 1;
+        st[a] = (len + kPivotAxis - 1) / kPivotAxis;
+        cnt[a] = (len + st[a] - 1) / st[a];
+    }
+}
+void pivot_lattice(const Dims &d, int lo[3], int st[3], int cnt[3]) { pivot_lattice_hd(d, lo, st, cnt); }
+
+namespace {
+
+// sample i of the lattice comes from fetch(i); one CTA, fixed summation order
+template <class Fetch>
+__device__ __forceinline__ void pivot_reduce(Fetch fetch, int nsamp, float *__restrict__ pivot)
 {
     __shared__ double part[kPivotThreads];
-    const int lo[3] = {d.nx / 4, d.ny / 4, d.nz / 4};
-    const int len[3] = {max(d.nx / 2, 1), max(d.ny / 2, 1), max(d.nz / 2, 1)};
-    int st[3], cnt[3];
-    for (int a = 0; a < 3; ++a) {
-        st[a] = (len[a] + kPivotAxis - 1) / kPivotAxis;
-        cnt[a] = (len[a] + st[a] - 1) / st[a];
-    }
-    const int nsamp = cnt[0] * cnt[1] * cnt[2];
     __shared__ double part2[kPivotThreads];
     double acc = 0.0, acc2 = 0.0;
     for (int i = threadIdx.x; i < nsamp; i += kPivotThreads) {
-        const int ix = i % cnt[0], iy = (i / cnt[0]) % cnt[1], iz = i / (cnt[0] * cnt[1]);
-        const long long o = (long long)(lo[0] + ix * st[0]) + (long long)d.nx * ((lo[1] + iy * st[1]) + (long long)d.ny * (lo[2] + iz * st[2]));
-        const double v = (double)__ldg(data + o);
+        const double v = (double)fetch(i);
         acc += v;
         acc2 += v * v;
     }
@@ -76,6 +85,24 @@ __global__ void __launch_bounds__(kPivotThreads) k_pivot(const float *__restrict
         const double var = fmax(part2[0] / (double)nsamp - m * m, 0.0);
         *pivot = (m * m >= 16.0 * var && m != 0.0) ? (float)m : 0.f;
     }
+}
+
+__global__ void __launch_bounds__(kPivotThreads) k_pivot(const float *__restrict__ data, Dims d, float *__restrict__ pivot)
+{
+    int lo[3], st[3], cnt[3];
+    pivot_lattice_hd(d, lo, st, cnt);
+    const int nsamp = cnt[0] * cnt[1] * cnt[2];
+    pivot_reduce([&](int i) {
+        const int ix = i % cnt[0], iy = (i / cnt[0]) % cnt[1], iz = i / (cnt[0] * cnt[1]);
+        const long long o = (long long)(lo[0] + ix * st[0]) + (long long)d.nx * ((lo[1] + iy * st[1]) + (long long)d.ny * (lo[2] + iz * st[2]));
+        return __ldg(data + o);
+    }, nsamp, pivot);
+}
+
+// the same reduction over samples gathered beforehand, in lattice order
+__global__ void __launch_bounds__(kPivotThreads) k_pivot_list(const float *__restrict__ list, int nsamp, float *__restrict__ pivot)
+{
+    pivot_reduce([&](int i) { return __ldg(list + i); }, nsamp, pivot);
 }
 
 // One directional sum of P:152 over the window clipped to the cube (C-7).
@@ -163,6 +190,13 @@ __global__ void __launch_bounds__(kThreads) k_threshold(
 inline unsigned grid_for(long long n) { return (unsigned)((n + kThreads - 1) / kThreads); }
 
 }  // namespace
+
+cudaError_t compute_pivot_list(pgsf_plan *p, const float *d_list, int nsamp, cudaStream_t st)
+{
+    LaunchScope ls(p, "pivot", st);
+    k_pivot_list<<<1, kPivotThreads, 0, st>>>(d_list, nsamp, p->d_pivot);
+    return cudaGetLastError();
+}
 
 cudaError_t compute_pivot(pgsf_plan *p, const float *data, cudaStream_t st)
 {

@@ -49,6 +49,14 @@ struct Dims {
     long long cube;      // nx*ny*nz
 };
 
+// A section of the frequency march of k_zm (pgsf_find_multiscale_host): entering channels [c0, c1), multiples of
+// the kernel's step; `state` = 4 planes of floats carrying the running window sums between the sections' launches.
+// The cube pointers of such a launch are VIRTUAL: buffer - (first buffered plane) * plane.
+struct ZmSection {
+    int c0, c1;
+    float *state;
+};
+
 }  // namespace pgsf
 
 namespace pgsf {
@@ -97,6 +105,7 @@ struct pgsf_plan {
     unsigned long long *h_d_count;
     void *h_d_ws;
     cudaStream_t h_stream;
+    struct pgsf_host_stage *hs;          // streamed sections (pgsf_host.cu)
 };
 
 namespace pgsf {
@@ -132,15 +141,21 @@ bool fast_z_radius(int r, int *compiled);
 cudaError_t fast_filter3d(pgsf_plan *p, int scale, const float *in, float *out, float *tmp,
                           cudaStream_t st, bool box = false, const float *wgt = nullptr, float *ratio = nullptr);
 // `ncubes` consecutive cubes (stride dims.cube) per call, for the entry points that take it
+// nplanes > 0: a stack of that many planes instead of ncubes whole cubes (the x and y passes do not couple planes)
 cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *in, float *const *out, int ncubes,
-                          cudaStream_t st, bool box = false, const float *wgt = nullptr);
+                          cudaStream_t st, bool box = false, const float *wgt = nullptr, int nplanes = 0);
 cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStream_t st, bool box = false,
                    float *ratio = nullptr);
 cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, int ncubes,
-                    cudaStream_t st);
+                    cudaStream_t st, const ZmSection *sec = nullptr);
+int zm_step_channels_of(int rz_compiled);      // channels per march step of k_zm<RZ>
 bool fast_stats_supported(const pgsf_plan *p, std::string *why);
 // frees the plan-owned staging of pgsf_find_multiscale_host (buffers, streams, events); the plan's device must be current
 void host_release(pgsf_plan *p);
+void host_stage_release(pgsf_plan *p);      // (pgsf_host.cu)
+// the streamed form of pgsf_find_multiscale_host; *handled = false if this plan / call cannot be streamed
+pgsf_status host_streamed(pgsf_plan *p, const float *h_in, float *const *h_filtered, uint8_t *h_mask,
+                          unsigned long long *h_count, bool *handled);
 // x/y window sums + selection from precomputed z-direction window sums Z1, Z2 (of fast_zm / k_zbox)
 // mode: 0 overwrite the mask, 1 OR into it (count = all set voxels), 2 sparse OR (only with stats_sparse_or():
 // touches only newly selected bytes, count += voxels that were not set before)
@@ -150,8 +165,13 @@ cudaError_t fast_threshold_xy(pgsf_plan *p, const float *f, const float *Z1, con
 // k_xyb (pgsf_xyb.cu): the successor of k_ymarch; same arguments
 bool xyb_supported(const pgsf_plan *p);
 inline bool stats_sparse_or(const pgsf_plan *p) { return p->fast_stats && xyb_supported(p) && !(p->tune & 2); }
+// nplanes > 0: the pointers address planes z_off .. z_off + nplanes - 1 of one cube (a section of the streamed cube)
 cudaError_t xyb_threshold(pgsf_plan *p, const float *f, const float *Z1, const float *Z2, uint8_t *mask, int mode,
-                          float *mean, float *sd, unsigned long long *count, int ncubes, cudaStream_t st);
+                          float *mean, float *sd, unsigned long long *count, int ncubes, cudaStream_t st,
+                          int nplanes = 0, int z_off = 0);
+// pivot from a list of samples already gathered in lattice order (pgsf_find_multiscale_host gathers them on the host)
+void pivot_lattice(const Dims &d, int lo[3], int st[3], int cnt[3]);
+cudaError_t compute_pivot_list(pgsf_plan *p, const float *d_list, int nsamp, cudaStream_t st);
 // tmp2: 2 cubes (the z-direction window sums of f and f^2)
 cudaError_t fast_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean,
                            float *sd, unsigned long long *count, float *tmp2, cudaStream_t st);

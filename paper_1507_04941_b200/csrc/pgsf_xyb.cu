@@ -52,7 +52,8 @@ struct XybShape {
 };
 
 struct XybParams {
-    Dims d;              // one cube
+    Dims d;              // one cube (or, for a section of a streamed cube: d.nz = planes of the launch)
+    int z_off, nz_full;  // channel of plane 0 of the launch inside its cube, channels of the whole cube
     int hy, hz;
     int gx, gy, gz;      // halo excluded from mask and count (C-11)
     int mode;            // 0 overwrite, 1 OR (dense), 2 OR (sparse; counts newly set voxels)
@@ -138,7 +139,7 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nx = p.d.nx, ny = p.d.ny;
     const int zz = blockIdx.z;                         // plane of the stack of cubes
-    const int z = zz % p.d.nz;                         // channel inside its cube
+    const int z = zz % p.d.nz + p.z_off;               // channel inside its cube
     const long long plane_off = (long long)zz * p.d.plane;
     const int ya = blockIdx.y * p.ychunk, yb = min(ya + p.ychunk, ny);
     const int hy = p.hy;
@@ -202,8 +203,8 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
     unsigned core_x[UPW];                              // bit j: column j is outside the x / z halo
     long long voff[UPW];                               // element offset of (xo, row of the current batch's unit)
     {
-        const float nzc = (float)xyb_clipped_len(z, p.hz, p.d.nz);
-        const bool core_z = z >= p.gz && z < p.d.nz - p.gz;
+        const float nzc = (float)xyb_clipped_len(z, p.hz, p.nz_full);
+        const bool core_z = z >= p.gz && z < p.nz_full - p.gz;
 #pragma unroll
         for (int u = 0; u < UPW; ++u) {
             const int unit = warp + 4 * u, strip = blockIdx.x * NSTRIP + unit / RB;
@@ -417,6 +418,7 @@ cudaError_t launch_xyb(const pgsf_plan *pl, const float *f, const float *Z1, con
 {
     using S = XybShape<G>;
     const Dims &d = p.d;
+    (void)pl;
     // balanced strips of whole groups of 8 columns
     int ns = (d.nx + S::WMAX - 1) / S::WMAX;
     p.wo = ((d.nx + ns - 1) / ns + 7) / 8 * 8;
@@ -424,12 +426,10 @@ cudaError_t launch_xyb(const pgsf_plan *pl, const float *f, const float *Z1, con
     ns = (d.nx + p.wo - 1) / p.wo;
     p.nstrips = ns;
     const int gx = (ns + S::NSTRIP - 1) / S::NSTRIP;
-    // y chunks: enough CTAs for a few waves; a chunk start re-reads 2 hy rows
-    const long long resident = (long long)pl->sm_count * 4;
-    const long long base = (long long)gx * d.nz * ncubes;
-    int nch = (int)((4 * resident + base - 1) / base);
-    const int min_rows = 8 * p.hy > 64 ? 8 * p.hy : 64;
-    if (nch > (d.ny + min_rows - 1) / min_rows) nch = (d.ny + min_rows - 1) / min_rows;
+    // y chunks: a function of ny alone -- the running sums of a chunk start afresh, so the rounding of a voxel's
+    // statistics must not depend on how many planes a launch happens to hold (a streamed cube is launched section
+    // by section and must reproduce the resident call bit for bit).  A chunk start re-reads 2 hy rows.
+    int nch = (d.ny + 1535) / 2048;
     if (nch < 1) nch = 1;
     p.ychunk = (d.ny + nch - 1) / nch;
     nch = (d.ny + p.ychunk - 1) / p.ychunk;
@@ -452,10 +452,19 @@ bool xyb_supported(const pgsf_plan *p)
 }
 
 cudaError_t xyb_threshold(pgsf_plan *p, const float *f, const float *Z1, const float *Z2, uint8_t *mask, int mode,
-                          float *mean, float *sd, unsigned long long *count, int ncubes, cudaStream_t st)
+                          float *mean, float *sd, unsigned long long *count, int ncubes, cudaStream_t st, int nplanes,
+                          int z_off)
 {
     XybParams xp;
     xp.d = p->dims;
+    xp.z_off = 0;
+    xp.nz_full = p->dims.nz;
+    if (nplanes > 0) {      // a section of one cube
+        xp.d.nz = nplanes;
+        xp.d.cube = xp.d.plane * nplanes;
+        xp.z_off = z_off;
+        ncubes = 1;
+    }
     xp.hy = p->desc.box_half[1];
     xp.hz = p->desc.box_half[2];
     xp.gx = p->desc.halo[0];

@@ -192,7 +192,8 @@ struct ZmShape {
 template <int RZ, int XT, int ZB>
 __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float *__restrict__ in, float *out,
                                                                 float *__restrict__ Z1, float *__restrict__ Z2,
-                                                                Dims d, int hz, const float *__restrict__ pivot, Taps t)
+                                                                Dims d, int hz, const float *__restrict__ pivot, Taps t,
+                                                                int kbeg, int kend, float *__restrict__ state)
 {
     const float c0 = __ldg(pivot);   // the window sums are of f - c0 and (f - c0)^2 (D-2)
     using S = ZmShape<RZ, XT, ZB>;
@@ -217,10 +218,18 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
     float *Zq = sq ? Z2 : Z1;
     float s = 0.f, e = 0.f;
     const int nz = d.nz;
-    const int nsteps = (nz + hz + ZB - 1) / ZB;   // entering channels 0 .. nz + hz - 1 (the tail drains the window)
+    // march steps kbeg .. kend - 1 of the (nz + hz + ZB - 1) / ZB steps of the whole axis (entering channels
+    // 0 .. nz + hz - 1; the tail drains the window).  A march cut into sections (pgsf_find_multiscale_host streams the
+    // cube through the device) carries the running window sums from one launch to the next in `state`
+    // ([quantity][s, e][row][column]), so that the sections perform exactly the arithmetic of one whole march.
+    float *st_s = nullptr;
+    if (state != nullptr && c_ok) {
+        st_s = state + ((long long)(sq ? 2 : 0) * d.plane + cb);
+        if (kbeg > 0) { s = st_s[0]; e = st_s[d.plane]; }
+    }
     const long long gstep = (long long)S::GROUPS * d.plane;   // staging: a warp group takes every GROUPS-th channel
 
-    for (int k = 0; k < nsteps; ++k) {
+    for (int k = kbeg; k < kend; ++k) {
         const int z0 = k * ZB;
         // channels leaving the window in this step: z0 - 2 hz + j, j = 0..63.  Those written in EARLIER steps
         // (by this CTA: still in L2) are fetched now, together with the t2 slab; those of this step's own
@@ -300,6 +309,7 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
         }
         __syncthreads();   // slabs are overwritten by the next step
     }
+    if (st_s != nullptr) { st_s[0] = s; st_s[d.plane] = e; }
 }
 
 template <int RZ>
@@ -319,14 +329,23 @@ constexpr int zm_step_channels() { return RZ >= 96 ? 128 : 64; }
 
 template <int RZ>
 cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot,
-                      const Taps &t, int ncubes, cudaStream_t st)
+                      const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec)
 {
     constexpr int ZB = zm_step_channels<RZ>();
     using S = ZmShape<RZ, ZM_XT, ZB>;
     cudaError_t e = ensure_dynamic_smem(k_zm<RZ, ZM_XT, ZB>, S::SMEM);
     if (e != cudaSuccess) return e;
+    const int nsteps = (d.nz + hz + ZB - 1) / ZB;
+    int kbeg = 0, kend = nsteps;
+    float *state = nullptr;
+    if (sec != nullptr) {     // entering channels [c0, c1), both multiples of ZB (c1 beyond the axis = to the end)
+        kbeg = sec->c0 / ZB;
+        kend = sec->c1 / ZB < nsteps ? sec->c1 / ZB : nsteps;
+        state = sec->state;
+        if (kbeg >= kend) return cudaSuccess;
+    }
     dim3 grid((d.nx + ZM_XT - 1) / ZM_XT, d.ny, ncubes);
-    k_zm<RZ, ZM_XT, ZB><<<grid, S::THREADS, S::SMEM, st>>>(in, out, Z1, Z2, d, hz, pivot, t);
+    k_zm<RZ, ZM_XT, ZB><<<grid, S::THREADS, S::SMEM, st>>>(in, out, Z1, Z2, d, hz, pivot, t, kbeg, kend, state);
     return cudaGetLastError();
 }
 
@@ -342,8 +361,9 @@ cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const D
         return launch_z<RZ>(in, out, ratio, d, t, st);                                                      \
     }                                                                                                       \
     cudaError_t launch_zm_r##RZ(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz,   \
-                                const float *pivot, const Taps &t, int ncubes, cudaStream_t st)             \
+                                const float *pivot, const Taps &t, int ncubes, cudaStream_t st,             \
+                                const ZmSection *sec)                                                       \
     {                                                                                                       \
-        return launch_zm<RZ>(in, out, Z1, Z2, d, hz, pivot, t, ncubes, st);                                 \
+        return launch_zm<RZ>(in, out, Z1, Z2, d, hz, pivot, t, ncubes, st, sec);                            \
     }                                                                                                       \
     }

@@ -421,6 +421,88 @@ def test_host_entry_point_and_stream(pg, synth):
         assert plan.pgsf_plan_launch_count() > 0
 
 
+# ------------------------------------------------------------------------------------ streamed host entry point (NEXT-3)
+
+def _host_run(pg, w, d_host, section=None, budget=None, keep=False, flags=0):
+    with _plan(pg, w, flags) as plan:
+        if section is not None:
+            plan.pgsf_plan_set_option(pg.PGSF_OPT_HOST_SECTION_PLANES, section)
+        if budget is not None:
+            plan.pgsf_plan_set_option(pg.PGSF_OPT_HOST_DEVICE_BUDGET, budget)
+        hf = [torch.empty(d_host.shape, dtype=torch.float32).pin_memory() for _ in w.sigmas] if keep else None
+        h_mask, count = plan.pgsf_find_multiscale_host(d_host, h_filtered=hf)
+        return h_mask, count, hf
+
+
+@pytest.mark.parametrize("dims,sigmas,box,section", [
+    ((96, 80, 400), ((1, 1, 2), (2, 2, 4)), (4, 4, 8), 64),        # 7 sections of one march step
+    ((96, 80, 400), ((1, 1, 2), (2, 2, 4)), (4, 4, 8), 128),
+    ((64, 48, 333), ((2, 2, 8), (1, 1, 4)), (8, 4, 40), 128),      # 2 hz > one step; nz not a multiple of the step
+    ((64, 48, 150), ((1, 1, 2),), (4, 4, 8), 0),                   # automatic section size
+])
+def test_streamed_host_equals_resident(pg, synth, oracle, dims, sigmas, box, section):
+    """pgsf_find_multiscale_host streams the cube through the device section by section; mask, count and
+    filtered cubes must equal the device-resident call BIT FOR BIT (nothing is recomputed at the seams: the march
+    carries its state), and the seams must be invisible to the oracle comparison as well."""
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[2], dims, n_sources=12), sigmas=sigmas, box_half=box, k=3.0)
+    d = synth.make_workload(w, "cuda")
+    with _plan(pg, w) as plan:
+        mask, cnt, filt = plan.pgsf_find_multiscale(d, keep_filtered=True)
+        torch.cuda.synchronize()
+    h_in = d.cpu().pin_memory()
+    h_mask, count, hf = _host_run(pg, w, h_in, section=section, keep=True)
+    assert count == int(cnt.item()) > 0
+    assert torch.equal(h_mask, mask.cpu())
+    for s in range(len(sigmas)):
+        assert torch.equal(hf[s], filt[s].cpu()), f"filtered cube {s} differs"
+    # pageable (not page-locked) input: the pivot samples are gathered on the host
+    h_mask2, count2, _ = _host_run(pg, w, d.cpu(), section=section)
+    assert count2 == count and torch.equal(h_mask2, h_mask)
+    # the oracle sees no seams
+    res = oracle.find_full(d[0].cpu().numpy(), w.sigmas, w.box_half, w.k)
+    rep = parity.assert_mask_ok(h_mask[0].numpy(), res, None, "streamed OR mask")
+    assert abs(count - res.count) <= rep.mismatches
+
+
+def test_streamed_host_under_a_small_device_budget(pg, synth):
+    """A cube whose resident footprint (input + filtered cubes + workspace) exceeds the staging budget still runs,
+    in the smallest sections, to the same mask; a budget below even those is an OOM error, not a crash."""
+    from dataclasses import replace
+    dims = (128, 96, 512)
+    w = replace(synth.scaled(synth.WORKLOADS[2], dims, n_sources=12), sigmas=((1, 1, 2), (2, 2, 4)), box_half=(4, 4, 8), k=3.0)
+    d = synth.make_workload(w, "cuda")
+    with _plan(pg, w) as plan:
+        mask, cnt, _ = plan.pgsf_find_multiscale(d)
+        resident = d.numel() * 4 * 3 + plan.pgsf_plan_workspace_bytes()
+        torch.cuda.synchronize()
+    h_in = d.cpu().pin_memory()
+    budget = resident // 3
+    h_mask, count, _ = _host_run(pg, w, h_in, budget=budget)
+    assert count == int(cnt.item()) > 0 and torch.equal(h_mask, mask.cpu())
+    with pytest.raises(pg.PgsfError) as ei:
+        _host_run(pg, w, h_in, budget=1 << 20)
+    assert ei.value.status == pg.PGSF_ERR_OOM
+
+
+def test_streamed_host_batch_with_halo_and_offset(pg, synth):
+    """Batches go through the same sections cube after cube (config-4-like, halo excluded); a DC level makes the
+    pivot of the statistics non-zero, and it must be the pivot of the resident call."""
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[4], (96, 80, 200), batch=3, n_sources=6), halo=(16, 12, 20), k=3.0)
+    d = synth.make_workload(w, "cuda") + 50.0
+    with _plan(pg, w) as plan:
+        plan.pgsf_plan_set_option(pg.PGSF_OPT_GROUP_CUBES, 2)
+        mask, cnt, _ = plan.pgsf_find_multiscale(d)
+        torch.cuda.synchronize()
+    for host in (d.cpu().pin_memory(), d.cpu()):
+        with _plan(pg, w) as plan:
+            plan.pgsf_plan_set_option(pg.PGSF_OPT_GROUP_CUBES, 2)
+            plan.pgsf_plan_set_option(pg.PGSF_OPT_HOST_SECTION_PLANES, 64)
+            h_mask, count = plan.pgsf_find_multiscale_host(host)
+        assert count == int(cnt.item()) > 0 and torch.equal(h_mask, mask.cpu())
+
+
 def test_api_errors_on_device(pg):
     with pg.Plan((32, 32, 32), [(1, 1, 2)], (2, 2, 2), 4.0) as plan:
         d = torch.zeros((1, 32, 32, 32), device="cuda")
