@@ -108,7 +108,9 @@ PGSF_API pgsf_status pgsf_plan_destroy(pgsf_plan *plan);
  *   PGSF_OPT_HOST_DEVICE_BUDGET   pgsf_find_multiscale_host: bytes of device memory its staging may use;
  *                                 0 = 80 % of the memory free at the first call.
  *   PGSF_OPT_TUNE                 measurement aid, a bit set: 1 = statistics kernel without L2 eviction hints,
- *                                 2 = the previous statistics kernel (k_ymarch) instead of k_xyb.
+ *                                 2 = the previous statistics kernel (k_ymarch) instead of k_xyb,
+ *                                 4 = cp.async staging of every z-pass slab, 8 = TMA bulk tensor copies for every
+ *                                 z-pass slab (default: TMA up to a compiled radius of 24, cp.async above).
  * INVALID_ARG for an unknown option or a value outside its range.
  */
 #define PGSF_OPT_GROUP_CUBES 1

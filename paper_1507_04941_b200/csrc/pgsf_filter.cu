@@ -19,18 +19,18 @@
 
 namespace pgsf {
 // per-radius entry points of the frequency-axis kernels (pgsf_z_r*.cu)
-cudaError_t launch_z_r6(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r6(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec);
-cudaError_t launch_z_r12(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r12(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec);
-cudaError_t launch_z_r24(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r24(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec);
-cudaError_t launch_z_r48(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r48(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec);
-cudaError_t launch_z_r72(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r72(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec);
-cudaError_t launch_z_r96(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st);
-cudaError_t launch_zm_r96(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec);
+cudaError_t launch_z_r6(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st, bool tma);
+cudaError_t launch_zm_r6(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec, bool tma);
+cudaError_t launch_z_r12(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st, bool tma);
+cudaError_t launch_zm_r12(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec, bool tma);
+cudaError_t launch_z_r24(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st, bool tma);
+cudaError_t launch_zm_r24(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec, bool tma);
+cudaError_t launch_z_r48(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st, bool tma);
+cudaError_t launch_zm_r48(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec, bool tma);
+cudaError_t launch_z_r72(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st, bool tma);
+cudaError_t launch_zm_r72(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec, bool tma);
+cudaError_t launch_z_r96(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st, bool tma);
+cudaError_t launch_zm_r96(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot, const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec, bool tma);
 
 namespace {
 
@@ -403,13 +403,17 @@ cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStr
     snprintf(name, sizeof name, box ? "bz_s%d" : "z_s%d", scale);
     LaunchScope ls(p, name, st);
     const Taps &tz = box ? sp.tz_box : sp.tz;
+    // slab by TMA up to RZ = 24; above, 128 - 256 threads issuing cp.async keep more copies in flight than one TMA
+    // box of 160 - 256 rows of 256 bytes (measured at config 3, RZ = 48: 11.7 ms with TMA, 11.0 ms without).
+    // PGSF_OPT_TUNE bit 2 = cp.async everywhere, bit 3 = TMA everywhere.
+    const bool tma = (p->tune & 8) != 0 || ((p->tune & 4) == 0 && sp.rz_c <= 24);
     switch (sp.rz_c) {
-    case 6: return launch_z_r6(in, out, ratio, d, tz, st);
-    case 12: return launch_z_r12(in, out, ratio, d, tz, st);
-    case 24: return launch_z_r24(in, out, ratio, d, tz, st);
-    case 48: return launch_z_r48(in, out, ratio, d, tz, st);
-    case 72: return launch_z_r72(in, out, ratio, d, tz, st);
-    case 96: return launch_z_r96(in, out, ratio, d, tz, st);
+    case 6: return launch_z_r6(in, out, ratio, d, tz, st, tma);
+    case 12: return launch_z_r12(in, out, ratio, d, tz, st, tma);
+    case 24: return launch_z_r24(in, out, ratio, d, tz, st, tma);
+    case 48: return launch_z_r48(in, out, ratio, d, tz, st, tma);
+    case 72: return launch_z_r72(in, out, ratio, d, tz, st, tma);
+    case 96: return launch_z_r96(in, out, ratio, d, tz, st, tma);
     default: return cudaErrorNotSupported;
     }
 }
@@ -428,13 +432,14 @@ cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float 
     char name[32];
     snprintf(name, sizeof name, "zm_s%d", scale);
     LaunchScope ls(p, name, st);
+    const bool tma = (p->tune & 8) != 0 || ((p->tune & 4) == 0 && sp.rz_c <= 24);     // (see fast_z)
     switch (sp.rz_c) {
-    case 6: return launch_zm_r6(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec);
-    case 12: return launch_zm_r12(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec);
-    case 24: return launch_zm_r24(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec);
-    case 48: return launch_zm_r48(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec);
-    case 72: return launch_zm_r72(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec);
-    case 96: return launch_zm_r96(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec);
+    case 6: return launch_zm_r6(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec, tma);
+    case 12: return launch_zm_r12(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec, tma);
+    case 24: return launch_zm_r24(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec, tma);
+    case 48: return launch_zm_r48(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec, tma);
+    case 72: return launch_zm_r72(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec, tma);
+    case 96: return launch_zm_r96(in, out, Z1, Z2, d, hz, p->d_pivot, sp.tz, ncubes, st, sec, tma);
     default: return cudaErrorNotSupported;
     }
 }

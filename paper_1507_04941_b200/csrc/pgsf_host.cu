@@ -271,7 +271,7 @@ pgsf_status host_streamed(pgsf_plan *p, const float *h_in, float *const *h_filte
             for (int s = 0; s < S; ++s) {
                 float *fv = virt(h->f[s], (long long)c0 - 2 * hz, plane);
                 float *z1v = virt(h->Z1, (long long)c0 - hz, plane), *z2v = virt(h->Z2, (long long)c0 - hz, plane);
-                ZmSection zs{c0, last ? (1 << 30) : c1, h->state[s]};
+                ZmSection zs{c0, last ? (1 << 30) : c1, h->state[s], h->t2[s], c0 - p->scales[s].rz_c, hi_prev};
                 HCHECK(fast_zm(p, s, t2v[s], fv, z1v, z2v, 1, sc, &zs), "z filter + window launch");
                 if (zs1 > zs0)
                     HCHECK(xyb_threshold(p, fv + (size_t)zs0 * plane, z1v + (size_t)zs0 * plane, z2v + (size_t)zs0 * plane,

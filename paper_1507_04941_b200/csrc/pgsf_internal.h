@@ -55,6 +55,8 @@ struct Dims {
 struct ZmSection {
     int c0, c1;
     float *state;
+    const float *t2_buf;     // the buffer behind the virtual input pointer: channels t2_base .. t2_hi - 1 (for the TMA map)
+    int t2_base, t2_hi;
 };
 
 }  // namespace pgsf

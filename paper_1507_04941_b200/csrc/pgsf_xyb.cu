@@ -7,7 +7,7 @@
 //
 //   y phase   a thread owns ONE PAIR of adjacent columns and keeps the y-direction window sums
 //             Y1 = sum_{|o|<=hy} Z1(y+o), Y2 likewise, in registers: the row entering the window is added,
-//             the row leaving it subtracted (Y2 Kahan-compensated, see k_zm).  The entering row comes from
+//             the row leaving it subtracted (Y2 compensated, see comp_add2).  The entering row comes from
 //             HBM; the leaving row was read 2 hy rows earlier by the same thread.  Only 256 columns x 3-4 CTAs
 //             are resident per SM, so the 2 hy + 1 live rows of all resident CTAs (~30-40 MB) stay in L2 and
 //             the leaving row never goes back to HBM -- k_ymarch kept 8 columns and ~20 registers per column
@@ -79,21 +79,28 @@ __device__ __forceinline__ float2 sub2(float2 a, float2 b)
     asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(rd) : "l"(ra), "l"(rb));
     return *reinterpret_cast<float2 *>(&rd);
 }
-// Kahan-compensated s += v on a pair of columns (e holds the running low-order error)
-__device__ __forceinline__ void kahan_add2(float2 &s, float2 &e, float2 v)
+// Compensated running sum on a pair of columns: (s, c) += v, the value is s + c.  The rounding error of s + v is
+// recovered exactly (Knuth's branch-free two-sum) and gathered in c, so what the sum retains after a large addend has
+// come and gone is O(eps^2) of it.  (Kahan's form, which folds the compensation into the NEXT addend, commits an
+// untracked eps |v| there: a source 10^3 - 10^4 x the noise in f^2 left 2e-5 of relative error in the sum of f^2 of
+// every later row of its column -- a fifth of the mask band.)
+__device__ __forceinline__ void comp_add2(float2 &s, float2 &c, float2 v)
 {
-    const float2 y = sub2(v, e);
-    const float2 t = add2(s, y);
-    e = sub2(sub2(t, s), y);
+    const float2 t = add2(s, v);
+    const float2 bp = sub2(t, s);
+    const float2 da = sub2(s, sub2(t, bp));
+    const float2 db = sub2(v, bp);
+    c = add2(c, add2(da, db));
     s = t;
 }
-
-// s -= v, compensated alike
-__device__ __forceinline__ void kahan_sub2(float2 &s, float2 &e, float2 v)
+// (s, c) -= v
+__device__ __forceinline__ void comp_sub2(float2 &s, float2 &c, float2 v)
 {
-    const float2 y = add2(v, e);          // -( (-v) - e )
-    const float2 t = sub2(s, y);
-    e = add2(sub2(t, s), y);              // (t - s) - (-y)
+    const float2 t = sub2(s, v);
+    const float2 bp = sub2(t, s);          // ~ -v
+    const float2 da = sub2(s, sub2(t, bp));
+    const float2 nb = add2(v, bp);         // -((-v) - bp)
+    c = add2(c, sub2(da, nb));
     s = t;
 }
 
@@ -267,11 +274,11 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
 #pragma unroll
         for (int i = 0; i < RB; ++i) {
             Y1 = add2(Y1, e1[i]);
-            kahan_add2(Y2, E2, e2[i]);
-            const float2 y2 = sub2(Y2, E2);
+            comp_add2(Y2, E2, e2[i]);
+            const float2 y2 = add2(Y2, E2);
             yw[par * (RB * 128) + i * 128] = make_float4(Y1.x, y2.x, Y1.y, y2.y);
             Y1 = sub2(Y1, l1[i]);                      // the row leaving the window after this output
-            kahan_sub2(Y2, E2, l2[i]);
+            comp_sub2(Y2, E2, l2[i]);
         }
         if (b + 1 < nb) load_rows(b + 1);              // in flight during the x phase
         __syncthreads();

@@ -2,7 +2,9 @@
 // radius RZ.  Every radius is instantiated in its own translation unit (pgsf_z_r*.cu) so that the long,
 // fully unrolled tap walks compile in parallel.
 #pragma once
+#include <string.h>
 #include "pgsf_device.cuh"
+#include "pgsf_tma.cuh"
 
 namespace pgsf {
 namespace {
@@ -78,12 +80,13 @@ __device__ __forceinline__ void z_accumulate(const float *__restrict__ base, con
     }
 }
 
-template <int RZ>
+template <int RZ, bool TMA>
 __global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, float *__restrict__ out,
-                                                 float *__restrict__ ratio, Dims d, Taps t)
+                                                 float *__restrict__ ratio, Dims d, Taps t,
+                                                 const __grid_constant__ CUtensorMap tmap)
 {
     using S = ZShape<RZ>;
-    extern __shared__ __align__(16) float smem[];  // [PLANES][Z_XT]
+    extern __shared__ __align__(128) float smem[];  // [PLANES][Z_XT]
     const int tid = threadIdx.x, lane = tid & 31, wz = tid >> 5;
     const int z0 = blockIdx.x * Z_ZB, x0 = blockIdx.y * Z_XT, y = blockIdx.z;
     const int gx = x0 + 4 * lane;
@@ -91,7 +94,16 @@ __global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, f
     const float *col_in = in + (long long)y * d.nx + (col_ok ? gx : 0);
 
     // stage channels z0-RZ .. z0+ZB+RZ-1 of this 128-column strip; outside the cube -> 0 (C-5)
-    {   // (running source pointer and shared-memory address: a handful of instructions per row)
+    if constexpr (TMA) {   // one bulk tensor copy, zero fill by the TMA unit
+        __shared__ unsigned long long bar;
+        if (tid == 0) mbar_init(&bar, 1);
+        __syncthreads();
+        if (tid == 0) {
+            mbar_arrive_expect_tx(&bar, S::SMEM);
+            tma_load_4d(smem, &tmap, x0, y, z0 - RZ, 0, &bar);
+        }
+        mbar_wait(&bar, 0);
+    } else {   // (running source pointer and shared-memory address: a handful of instructions per row)
         const float *src = col_in + (long long)(z0 - RZ + wz) * d.plane;   // dereferenced only where gz is inside the cube
         const long long step = (long long)Z_WARPS * d.plane;
         unsigned dst = (unsigned)__cvta_generic_to_shared(smem + wz * Z_XT + 4 * lane);
@@ -102,9 +114,9 @@ __global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, f
             const bool ok = col_ok && (unsigned)gz < (unsigned)d.nz;
             cp_async16_s(dst, ok ? src : in, ok);   // (a valid address even when nothing is read)
         }
+        cp_async_wait_all();
+        __syncthreads();
     }
-    cp_async_wait_all();
-    __syncthreads();
 
     // Eq. 5: f[z] = sum_o t2[z+o] gz[o]; the thread walks along z, PZ accumulators x 4 columns.
     float2 acc[Z_PZ][2];
@@ -189,15 +201,22 @@ struct ZmShape {
     static constexpr int SMEM = (PLANES + ZB) * XT * 4;   // + slab of the channels leaving the window
 };
 
-template <int RZ, int XT, int ZB>
+template <int RZ, int XT, int ZB, bool TMA>
 __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float *__restrict__ in, float *out,
                                                                 float *__restrict__ Z1, float *__restrict__ Z2,
                                                                 Dims d, int hz, const float *__restrict__ pivot, Taps t,
-                                                                int kbeg, int kend, float *__restrict__ state)
+                                                                int kbeg, int kend, float *__restrict__ state,
+                                                                const __grid_constant__ CUtensorMap tmap, int zmap_lo)
 {
     const float c0 = __ldg(pivot);   // the window sums are of f - c0 and (f - c0)^2 (D-2)
     using S = ZmShape<RZ, XT, ZB>;
-    extern __shared__ __align__(16) float smem[];  // [PLANES][XT] t2 slab / f slab, [ZB][XT] leaving slab
+    extern __shared__ __align__(128) float smem[];  // [PLANES][XT] t2 slab / f slab, [ZB][XT] leaving slab
+    __shared__ unsigned long long bar;             // TMA: completion of the t2 slab
+    unsigned phase = 0;
+    if constexpr (TMA) {
+        if (threadIdx.x == 0) mbar_init(&bar, 1);
+        __syncthreads();
+    }
     float *fs = smem;                              // f of this step (written after the filter phase)
     float *ts = smem + S::PLANES * XT;             // f of the channels leaving the window in this step
     const int tid = threadIdx.x, lx = tid % S::LX, wz = tid / S::LX;
@@ -247,7 +266,19 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
                 cp_async16_s(dst, ok ? src : in, ok);   // (a valid address even when nothing is read)
             }
         }
-        if (z0 < nz) {
+        if (TMA && z0 < nz) {
+            // channels z0-RZ .. z0+ZB+RZ-1 of t2 as one (or two) bulk tensor copies; outside the cube -> 0 (C-5).  The
+            // slab was read and rewritten (f slab) through the generic proxy in the previous step: fence, then copy.
+            if (tid == 0) {
+                constexpr int NBOX = S::PLANES > 256 ? 2 : 1, BZ = S::PLANES / NBOX;
+                fence_proxy_async_smem();
+                mbar_arrive_expect_tx(&bar, S::PLANES * XT * 4);
+#pragma unroll
+                for (int bx = 0; bx < NBOX; ++bx)
+                    tma_load_4d(smem + bx * BZ * XT, &tmap, x0, y, z0 - RZ + bx * BZ - zmap_lo, blockIdx.z, &bar);
+            }
+        }
+        if (!TMA && z0 < nz) {
             // stage channels z0-RZ .. z0+ZB+RZ-1 of t2; outside the cube -> 0 (C-5)
             const float *src = col_in + (long long)(z0 - RZ + wz) * d.plane;
             unsigned dst = (unsigned)__cvta_generic_to_shared(smem + wz * XT + 4 * lx);
@@ -260,6 +291,10 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
             }
         }
         cp_async_wait_all();
+        if (TMA && z0 < nz) {
+            mbar_wait(&bar, phase);
+            phase ^= 1;
+        }
         __syncthreads();
         if (z0 < nz) {
             float2 acc[Z_PZ][2];
@@ -313,12 +348,20 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
 }
 
 template <int RZ>
-cudaError_t launch_z(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st)
+cudaError_t launch_z(const float *in, float *out, float *ratio, const Dims &d, const Taps &t, cudaStream_t st, bool tma)
 {
-    cudaError_t e = ensure_dynamic_smem(k_z<RZ>, ZShape<RZ>::SMEM);
-    if (e != cudaSuccess) return e;
     dim3 grid((d.nz + Z_ZB - 1) / Z_ZB, (d.nx + Z_XT - 1) / Z_XT, d.ny);
-    k_z<RZ><<<grid, Z_THREADS, ZShape<RZ>::SMEM, st>>>(in, out, ratio, d, t);
+    alignas(64) CUtensorMap map;
+    if (tma && make_slab_map(&map, in, d.nx, d.ny, d.nz, 1, Z_XT, ZShape<RZ>::PLANES)) {
+        cudaError_t e = ensure_dynamic_smem(k_z<RZ, true>, ZShape<RZ>::SMEM);
+        if (e != cudaSuccess) return e;
+        k_z<RZ, true><<<grid, Z_THREADS, ZShape<RZ>::SMEM, st>>>(in, out, ratio, d, t, map);
+        return cudaGetLastError();
+    }
+    memset(&map, 0, sizeof map);
+    cudaError_t e = ensure_dynamic_smem(k_z<RZ, false>, ZShape<RZ>::SMEM);
+    if (e != cudaSuccess) return e;
+    k_z<RZ, false><<<grid, Z_THREADS, ZShape<RZ>::SMEM, st>>>(in, out, ratio, d, t, map);
     return cudaGetLastError();
 }
 
@@ -329,12 +372,11 @@ constexpr int zm_step_channels() { return RZ >= 96 ? 128 : 64; }
 
 template <int RZ>
 cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot,
-                      const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec)
+                      const Taps &t, int ncubes, cudaStream_t st, const ZmSection *sec, bool tma)
 {
     constexpr int ZB = zm_step_channels<RZ>();
     using S = ZmShape<RZ, ZM_XT, ZB>;
-    cudaError_t e = ensure_dynamic_smem(k_zm<RZ, ZM_XT, ZB>, S::SMEM);
-    if (e != cudaSuccess) return e;
+    cudaError_t e;
     const int nsteps = (d.nz + hz + ZB - 1) / ZB;
     int kbeg = 0, kend = nsteps;
     float *state = nullptr;
@@ -345,7 +387,27 @@ cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const D
         if (kbeg >= kend) return cudaSuccess;
     }
     dim3 grid((d.nx + ZM_XT - 1) / ZM_XT, d.ny, ncubes);
-    k_zm<RZ, ZM_XT, ZB><<<grid, S::THREADS, S::SMEM, st>>>(in, out, Z1, Z2, d, hz, pivot, t, kbeg, kend, state);
+    alignas(64) CUtensorMap map;
+    constexpr int BZ = S::PLANES > 256 ? S::PLANES / 2 : S::PLANES;
+    int zmap_lo = 0;
+    bool ok = tma;
+    if (ok && sec != nullptr && sec->t2_buf != nullptr) {
+        // a section: the buffer holds channels t2_base .. t2_hi - 1; the map covers those that exist in the cube
+        const int lo = sec->t2_base > 0 ? sec->t2_base : 0, hi = sec->t2_hi < d.nz ? sec->t2_hi : d.nz;
+        zmap_lo = lo;
+        ok = make_slab_map(&map, sec->t2_buf + (long long)(lo - sec->t2_base) * d.plane, d.nx, d.ny, hi - lo, 1, ZM_XT, BZ);
+    } else if (ok) {
+        ok = make_slab_map(&map, in, d.nx, d.ny, d.nz, ncubes, ZM_XT, BZ);
+    }
+    if (ok) {
+        if ((e = ensure_dynamic_smem(k_zm<RZ, ZM_XT, ZB, true>, S::SMEM)) != cudaSuccess) return e;
+        k_zm<RZ, ZM_XT, ZB, true><<<grid, S::THREADS, S::SMEM, st>>>(in, out, Z1, Z2, d, hz, pivot, t, kbeg, kend, state,
+                                                                     map, zmap_lo);
+        return cudaGetLastError();
+    }
+    memset(&map, 0, sizeof map);
+    if ((e = ensure_dynamic_smem(k_zm<RZ, ZM_XT, ZB, false>, S::SMEM)) != cudaSuccess) return e;
+    k_zm<RZ, ZM_XT, ZB, false><<<grid, S::THREADS, S::SMEM, st>>>(in, out, Z1, Z2, d, hz, pivot, t, kbeg, kend, state, map, 0);
     return cudaGetLastError();
 }
 
@@ -356,14 +418,14 @@ cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const D
 #define PGSF_INSTANTIATE_Z(RZ)                                                                              \
     namespace pgsf {                                                                                        \
     cudaError_t launch_z_r##RZ(const float *in, float *out, float *ratio, const Dims &d, const Taps &t,     \
-                               cudaStream_t st)                                                             \
+                               cudaStream_t st, bool tma)                                                   \
     {                                                                                                       \
-        return launch_z<RZ>(in, out, ratio, d, t, st);                                                      \
+        return launch_z<RZ>(in, out, ratio, d, t, st, tma);                                                 \
     }                                                                                                       \
     cudaError_t launch_zm_r##RZ(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz,   \
                                 const float *pivot, const Taps &t, int ncubes, cudaStream_t st,             \
-                                const ZmSection *sec)                                                       \
+                                const ZmSection *sec, bool tma)                                             \
     {                                                                                                       \
-        return launch_zm<RZ>(in, out, Z1, Z2, d, hz, pivot, t, ncubes, st, sec);                            \
+        return launch_zm<RZ>(in, out, Z1, Z2, d, hz, pivot, t, ncubes, st, sec, tma);                       \
     }                                                                                                       \
     }

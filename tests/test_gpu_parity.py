@@ -403,6 +403,14 @@ def test_stats_kernel_variants(pg, synth, dims, box):
     assert torch.equal(out[0][2], out[1][2]) and torch.equal(out[0][3], out[1][3])
     ndiff = int((out[0][0] != out[2][0]).sum())
     assert ndiff <= 2, f"k_xyb and k_ymarch masks differ in {ndiff} voxels"
+    # z-pass slabs by cp.async everywhere (4) and by TMA everywhere (8): the same bytes land in shared memory
+    for tune in (4, 8):
+        with _plan(pg, w) as plan:
+            plan.pgsf_plan_set_option(pg.PGSF_OPT_TUNE, tune)
+            mask, cnt, filt = plan.pgsf_find_multiscale(d, keep_filtered=True)
+            f1 = plan.pgsf_filter3d(1, d)
+            torch.cuda.synchronize()
+            assert torch.equal(mask, out[0][0]) and int(cnt.item()) == out[0][1] and torch.equal(f1, filt[1])
     assert float((out[0][2] - out[2][2]).abs().max()) <= 1e-5 * float(out[2][3].max())
     assert float(((out[0][3] - out[2][3]).abs() / out[2][3]).max()) <= 1e-4
 
