@@ -67,6 +67,10 @@ typedef enum {
                                         validation of every call can be exercised on a machine without a GPU;
                                         a compute call that passes validation returns PGSF_ERR_CUDA */
 
+#define PGSF_FLAG_TENSOR_ZPASS 0x8u  /* OPTIONAL variant: the frequency pass of pgsf_find_multiscale as a banded-Toeplitz
+                                        GEMM on the tensor cores (tcgen05, 3 x TF32 split) for scales whose z radius
+                                        is >= 13 (compiled radius 24 and above); same tolerances, different rounding */
+
 #define PGSF_MAX_SCALES 8
 #define PGSF_MAX_RADIUS 96 /* largest supported ceil(truncate*sigma) on any axis */
 #define PGSF_MAX_BOX_HALF 128

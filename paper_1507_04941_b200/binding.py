@@ -18,6 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libpgsf.so")
 PGSF_OK, PGSF_ERR_INVALID_ARG, PGSF_ERR_UNSUPPORTED, PGSF_ERR_OOM, PGSF_ERR_CUDA = range(5)
 PGSF_FLAG_FORCE_GENERIC = 0x1
 PGSF_FLAG_DRY_RUN = 0x4
+PGSF_FLAG_TENSOR_ZPASS = 0x8
 PGSF_OPT_GROUP_CUBES, PGSF_OPT_HOST_SECTION_PLANES, PGSF_OPT_HOST_DEVICE_BUDGET, PGSF_OPT_TUNE = 1, 2, 3, 4
 PGSF_WEIGHTED_AS_PRINTED = 0
 PGSF_WEIGHTED_NORMALISED = 1

@@ -198,6 +198,8 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
     p->h_d_ws = nullptr;
     p->h_stream = nullptr;
     p->hs = nullptr;
+    p->tensor_z = false;
+    for (int s = 0; s < PGSF_MAX_SCALES; ++s) p->d_tc_strips[s] = nullptr;
     for (int s = 0; s < PGSF_MAX_SCALES; ++s) p->h_d_f[s] = nullptr;
 
     const bool force_generic = (desc->flags & PGSF_FLAG_FORCE_GENERIC) != 0;
@@ -269,6 +271,17 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
             return fail(nullptr, PGSF_ERR_OOM, "plan constants: %s", cudaGetErrorString(e));
         }
     }
+    if (!dry && (desc->flags & PGSF_FLAG_TENSOR_ZPASS) && p->fast_filter && p->fast_stats) {
+        const cudaError_t e = pgsf::ztc_prepare(p);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            pgsf::ztc_release(p);
+            cudaFree(p->d_pivot);
+            delete p;
+            return fail(nullptr, PGSF_ERR_OOM, "tensor-core operands: %s", cudaGetErrorString(e));
+        }
+        p->tensor_z = true;
+    }
     const size_t cubes = 1 + (p->fast_filter ? (size_t)p->group : 2) + (p->fast_stats ? 2 * (size_t)p->group : 4);
     p->ws_bytes = cubes * p->ws_cube_bytes;
     *out = p;
@@ -281,6 +294,7 @@ pgsf_status pgsf_plan_destroy(pgsf_plan *p)
     if (!p->dry) {
         cudaSetDevice(p->device);      // (events, streams and staging buffers belong to the plan's device)
         pgsf::host_release(p);
+        pgsf::ztc_release(p);
         cudaFree(p->d_pivot);
         for (auto &r : p->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
         for (auto e : p->prof_free) cudaEventDestroy(e);

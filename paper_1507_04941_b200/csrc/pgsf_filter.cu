@@ -428,6 +428,10 @@ cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float 
     const Dims &d = p->dims;
     const ScalePlan &sp = p->scales[scale];
     if (d.ny > 65535 || ncubes < 1 || ncubes > 65535) return cudaErrorInvalidConfiguration;
+    if (p->tensor_z) {      // the optional tensor-core variant (pgsf_ztc.cu) where the plan asks for it and it applies
+        const cudaError_t te = fast_ztc(p, scale, in, out, Z1, Z2, ncubes, st, sec);
+        if (te != cudaErrorNotSupported) return te;
+    }
     const int hz = p->desc.box_half[2];
     char name[32];
     snprintf(name, sizeof name, "zm_s%d", scale);

@@ -108,6 +108,8 @@ struct pgsf_plan {
     void *h_d_ws;
     cudaStream_t h_stream;
     struct pgsf_host_stage *hs;          // streamed sections (pgsf_host.cu)
+    bool tensor_z;                       // PGSF_FLAG_TENSOR_ZPASS: k_ztc for compiled z radii >= 24 (pgsf_ztc.cu)
+    float *d_tc_strips[PGSF_MAX_SCALES]; // its band-matrix operands
 };
 
 namespace pgsf {
@@ -151,6 +153,12 @@ cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStr
 cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, int ncubes,
                     cudaStream_t st, const ZmSection *sec = nullptr);
 int zm_step_channels_of(int rz_compiled);      // channels per march step of k_zm<RZ>
+// the tensor-core variant of fast_zm (pgsf_ztc.cu): cudaErrorNotSupported = not for this plan / scale, run fast_zm
+bool ztc_radius(int rz_compiled);
+cudaError_t ztc_prepare(pgsf_plan *p);
+void ztc_release(pgsf_plan *p);
+cudaError_t fast_ztc(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, int ncubes,
+                     cudaStream_t st, const ZmSection *sec = nullptr);
 bool fast_stats_supported(const pgsf_plan *p, std::string *why);
 // frees the plan-owned staging of pgsf_find_multiscale_host (buffers, streams, events); the plan's device must be current
 void host_release(pgsf_plan *p);

@@ -67,8 +67,11 @@ inline EncodeTiledFn encode_tiled_fn()
     return fn;
 }
 
-// fp32 cube stack [ncubes][nz][ny][nx] at `base`, boxes of bx columns x 1 row x bz channels x 1 cube, zero fill
-inline bool make_slab_map(CUtensorMap *map, const float *base, int nx, int ny, int nz, int ncubes, int bx, int bz)
+// fp32 cube stack [ncubes][nz][ny][nx] at `base`, boxes of bx columns x 1 row x bz channels x 1 cube, zero fill;
+// swizzle128: 128-byte rows with their 32-byte granules XOR-ed with (row & 3) -- the only layout tcgen05 takes for an
+// MN-major TF32 operand (UMMA SWIZZLE_128B_BASE32B)
+inline bool make_slab_map(CUtensorMap *map, const float *base, int nx, int ny, int nz, int ncubes, int bx, int bz,
+                          bool swizzle128 = false)
 {
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn || bx > 256 || bz > 256 || nz < 1) return false;
@@ -77,7 +80,8 @@ inline bool make_slab_map(CUtensorMap *map, const float *base, int nx, int ny, i
     const cuuint32_t box[4] = {(cuuint32_t)bx, 1, (cuuint32_t)bz, 1};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<float *>(base), dims, strides, box, estr,
-              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B : CU_TENSOR_MAP_SWIZZLE_NONE,
+              CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 

@@ -429,6 +429,38 @@ def test_host_entry_point_and_stream(pg, synth):
         assert plan.pgsf_plan_launch_count() > 0
 
 
+# ------------------------------------------------------------------------------------ optional tensor-core z pass
+
+@pytest.mark.parametrize("dims,sigmas,box", [
+    ((96, 40, 300), ((2, 2, 8), (1, 1, 16)), (4, 4, 8)),          # compiled z radii 24 and 48
+    ((104, 36, 200), ((1, 1, 24), (1, 1, 2)), (4, 4, 40)),        # radius 72 (two TMA boxes), a ragged last strip;
+                                                                   #   the scale of radius 6 stays on the CUDA cores
+    ((64, 24, 150), ((1, 1, 32),), (8, 8, 16)),                   # radius 96 > nz / 2
+])
+def test_tensor_core_z_pass(pg, synth, oracle, dims, sigmas, box):
+    """PGSF_FLAG_TENSOR_ZPASS: the frequency pass as a banded-Toeplitz GEMM on the tensor cores (tcgen05, 3 x TF32
+    split).  Same bar as every other path: filtered max|diff| <= 1e-5, masks identical outside the band; and the
+    variant must be close to the CUDA-core path (the split leaves ~2^-22 relative)."""
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[2], dims, n_sources=10), sigmas=sigmas, box_half=box, k=3.0)
+    d = synth.make_workload(w, "cuda")
+    rep, count = _full_compare(pg, oracle, w, d, pg.PGSF_FLAG_TENSOR_ZPASS, check_stats=False)
+    with _plan(pg, w, pg.PGSF_FLAG_TENSOR_ZPASS) as plan:
+        m_tc, c_tc, f_tc = plan.pgsf_find_multiscale(d, keep_filtered=True)
+        names = plan.launched_kernels() if hasattr(plan, "launched_kernels") else None
+    with _plan(pg, w) as plan:
+        m_cc, c_cc, f_cc = plan.pgsf_find_multiscale(d, keep_filtered=True)
+    torch.cuda.synchronize()
+    dmax = max(float((a - b).abs().max()) for a, b in zip(f_tc, f_cc))
+    print(f"tensor-core z pass: count={count} mismatches={rep.mismatches} band={rep.band_voxels} "
+          f"max |tc - cuda core| = {dmax:.2e}")
+    assert 0.0 < dmax <= 4e-6                     # (> 0: the variant really ran; ~2^-21 of the brightest source)
+    assert int((m_tc != m_cc).sum()) <= rep.band_voxels + 2
+    # the streamed host entry point cuts the same march into sections
+    h_mask, hcount, _ = _host_run(pg, w, d.cpu().pin_memory(), section=128, flags=pg.PGSF_FLAG_TENSOR_ZPASS)
+    assert hcount == int(c_tc.item()) and torch.equal(h_mask, m_tc.cpu())
+
+
 # ------------------------------------------------------------------------------------ streamed host entry point (NEXT-3)
 
 def _host_run(pg, w, d_host, section=None, budget=None, keep=False, flags=0):
