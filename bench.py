@@ -271,6 +271,7 @@ def _path_roofline(w, taps, n_vox, ms_step, alu_peak, hbm_peak):
             "roofline_ms": t_path * 1e3, "frac": t_path * 1e3 / ms_step, "bound": "alu" if t_alu >= t_hbm else "hbm"}
 
 
+FLAGS = 0     # --flags: PGSF_FLAG_* plan flags (8 = the optional tensor-core z pass)
 TUNE = 0      # --tune: PGSF_OPT_TUNE bits (kernel variants for A/B measurements; results are identical)
 
 
@@ -287,7 +288,7 @@ def measure_workload(w, dev, device_index, rank, world, steps, warmup, peaks, sm
     S = len(w.sigmas)
     taps = _taps(w)
     plan = binding.Plan(w.dims, w.sigmas, w.box_half, w.k, batch=w.batch, halo=w.halo, truncate=w.truncate,
-                        device=device_index)
+                        device=device_index, flags=FLAGS)
     if TUNE:
         plan.pgsf_plan_set_option(binding.PGSF_OPT_TUNE, TUNE)
     filt = [torch.empty_like(d) for _ in range(S)]
@@ -763,14 +764,16 @@ def main():
                     help="find = the hot path (default); weighted = Eq. 1 of the paper (NEXT-1); direct = Eq. 2 for "
                          "an arbitrary filter array (NEXT-2); the last two single GPU")
     ap.add_argument("--fp64", action="store_true", help="--path direct: accumulate in fp64 as the paper does")
+    ap.add_argument("--flags", type=int, default=0, help="plan flags (8 = PGSF_FLAG_TENSOR_ZPASS, the optional variant)")
     ap.add_argument("--tune", type=int, default=0, help="PGSF_OPT_TUNE bits (kernel variants; same results)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true",
                     help="skip the ms-per-step sweep over the other BASELINE.json configs after the headline")
     args = ap.parse_args()
-    global TUNE
+    global TUNE, FLAGS
     TUNE = args.tune
+    FLAGS = args.flags
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
     from paper_1507_04941_b200 import synth
     w = synth.WORKLOADS[args.config]

@@ -145,13 +145,16 @@ __global__ void __launch_bounds__(TC_NT) k_ztc(float *out, float *__restrict__ Z
             const bool ok = zt >= 0 && zt < z0 && zt < nz && x0 + 4 * ch < d.nx;
             cp_async16(ts + j * TC_XT + 4 * ch, ok ? row_out + (long long)zt * d.plane + 4 * ch : out, ok);
         }
-        if (z0 < nz && tid == 0) {
+        if (z0 < nz && warp == 0) {
+          if (tid == 0) {
             // slab channels z0 - rz .. z0 + 127 + rz: bulk tensor copies, zeros outside the cube (C-5)
             fence_proxy_async_smem();
             mbar_arrive_expect_tx(&bar_tma, K * TC_XT * 4);
             const int bz = K / p.nbox;
             for (int b = 0; b < p.nbox; ++b)
                 tma_load_4d(Bh + b * bz * TC_XT, &tmap, x0, y, z0 - p.rz + b * bz - p.zmap_lo, blockIdx.z, &bar_tma);
+          }
+          __syncwarp();
         }
         cp_async_wait_all();
         if (z0 < nz) {
@@ -170,7 +173,8 @@ __global__ void __launch_bounds__(TC_NT) k_ztc(float *out, float *__restrict__ Z
             fence_proxy_async_smem();
             tc_fence_before();
             __syncthreads();
-            if (tid == 0) {
+            if (warp == 0) {       // one lane issues; its warp waits at the __syncwarp, not spinning on the barrier
+              if (tid == 0) {
                 tc_fence_after();
                 for (int ks = 0; ks < K / 8; ++ks) {
                     // A: K-major, no swizzle, Hankel strip (LBO 128 B between the two K chunks, SBO 256 B between row groups)
@@ -185,6 +189,8 @@ __global__ void __launch_bounds__(TC_NT) k_ztc(float *out, float *__restrict__ Z
                     umma_tf32(tmem, ah, bl, 1);
                 }
                 umma_commit(&bar_mma);
+              }
+              __syncwarp();
             }
             mbar_wait(&bar_mma, ph_mma);
             ph_mma ^= 1;
@@ -213,7 +219,28 @@ __global__ void __launch_bounds__(TC_NT) k_ztc(float *out, float *__restrict__ Z
             tc_fence_before();
         }
         __syncthreads();      // f slab and leaving slab complete; the accumulator has been read
-        if (c_ok) {
+        if (c_ok && z0 >= 2 * hz && z0 + TC_ZB <= nz) {
+            // interior step: all entering and leaving channels (and all outputs) are inside the cube
+            const int jsplit = min(2 * hz, TC_ZB);     // leaving channel: ts[j] for j < jsplit, else fs[j - 2 hz]
+            float *zp = Zq + (long long)(z0 - hz) * d.plane + cb;
+            const int cx = ((c >> 2) << 2), cl = c & 3;
+#pragma unroll 4
+            for (int j = 0; j < TC_ZB; ++j) {
+                const float a = fs[j * TC_XT + ((cx ^ ((j & 7) << 2)) | cl)] - c0;
+                const int jt = j - 2 * hz;
+                const float b = (j < jsplit ? ts[j * TC_XT + c] : fs[jt * TC_XT + ((cx ^ ((jt & 7) << 2)) | cl)]) - c0;
+                if (sq) {
+                    kahan_add(s, e, a * a);
+                    *zp = s - e;
+                    kahan_add(s, e, -(b * b));
+                } else {
+                    s += a;
+                    *zp = s;
+                    s -= b;
+                }
+                zp += d.plane;
+            }
+        } else if (c_ok) {
             for (int j = 0; j < TC_ZB; ++j) {
                 const int zl = z0 + j, zo = zl - hz;       // channel entering the window of output zo
                 if (zl < nz) {
