@@ -506,7 +506,7 @@ def run_e2e(args, w, ctx):
     assert count == expect, f"host entry point count {count} != device path count {expect}"
     return {"value": w.voxels * S * world / sec / 1e9, "unit": UNIT, "ms_per_step": sec * 1e3, "steps": steps,
             "h2d_bytes_per_step": w.voxels * 4, "d2h_bytes_per_step": w.voxels + 8,
-            "api": "pgsf_find_multiscale_host (pinned host cube in; mask + count out)"}
+            "api": "pgsf_find_multiscale_host (pinned host cube in; mask + count out; streamed in z sections, copies overlapped with compute)"}
 
 
 CPU_SAMPLE_1T = (128, 128, 128)    # the 1-thread leg: a smaller brick of the same cube (~10 s)

@@ -338,8 +338,10 @@ int pgsf_plan_path(const pgsf_plan *p, char *text, int cap)
     if (!p || !text || cap < 1) return -1;
     const bool tiled = p->fast_filter && p->fast_stats;
     snprintf(text, (size_t)cap, "filter: %s%s%s; stats: %s%s%s",
-             p->fast_filter ? "tiled (k_xym + k_z / k_zm)" : "generic (k_conv1d) because ", p->fast_filter ? "" : p->why_filter.c_str(), "",
-             p->fast_stats ? "tiled (k_zm / k_zbox + k_ymarch)" : "generic (k_boxsum + k_threshold) because ",
+             p->fast_filter ? (p->tensor_z ? "tiled (k_xym + k_z / k_zm, k_ztc on the tensor cores for z radii >= 13)" : "tiled (k_xym + k_z / k_zm)")
+                            : "generic (k_conv1d) because ", p->fast_filter ? "" : p->why_filter.c_str(), "",
+             p->fast_stats ? (pgsf::stats_sparse_or(p) ? "tiled (k_zm / k_zbox + k_xyb)" : "tiled (k_zm / k_zbox + k_ymarch)")
+                           : "generic (k_boxsum + k_threshold) because ",
              p->fast_stats ? "" : p->why_stats.c_str(), "");
     return tiled ? 1 : 0;
 }

@@ -139,14 +139,30 @@ def test_find_multiscale_rejects_overlapping_buffers(lib):
         assert call(d_in=d_in + 4) == binding.PGSF_ERR_INVALID_ARG    # misaligned
 
 
+def test_statistics_kernel_and_tensor_flag_in_the_plan_path(lib):
+    """The plan path names the statistics kernel that will run (k_xyb, or k_ymarch under PGSF_OPT_TUNE bit 1) and a
+    dry-run plan accepts PGSF_FLAG_TENSOR_ZPASS without touching a device (the operands are built on a real one)."""
+    from paper_1507_04941_b200 import binding
+    with _dry(binding, dims=(64, 48, 80), sigmas=((1, 1, 2), (1, 1, 16)), box=(8, 8, 16),
+              flags=binding.PGSF_FLAG_TENSOR_ZPASS) as plan:
+        ok, text = plan.pgsf_plan_path()
+        assert ok and "k_xyb" in text, text
+        plan.pgsf_plan_set_option(binding.PGSF_OPT_TUNE, 2)
+        ok, text = plan.pgsf_plan_path()
+        assert ok and "k_ymarch" in text, text
+
+
 def test_plan_options_are_validated(lib):
     from paper_1507_04941_b200 import binding
     with _dry(binding, dims=(32, 32, 32), batch=5) as plan:
         plan.pgsf_plan_set_option(binding.PGSF_OPT_GROUP_CUBES, 2)
         plan.pgsf_plan_set_option(binding.PGSF_OPT_HOST_SECTION_PLANES, 16)
         plan.pgsf_plan_set_option(binding.PGSF_OPT_HOST_DEVICE_BUDGET, 1 << 30)
+        plan.pgsf_plan_set_option(binding.PGSF_OPT_TUNE, 2 | 4)
+        plan.pgsf_plan_set_option(binding.PGSF_OPT_TUNE, 0)
         for opt, val in [(binding.PGSF_OPT_GROUP_CUBES, 0), (binding.PGSF_OPT_GROUP_CUBES, 6),
-                         (binding.PGSF_OPT_HOST_SECTION_PLANES, 33), (binding.PGSF_OPT_HOST_DEVICE_BUDGET, -1), (99, 0)]:
+                         (binding.PGSF_OPT_HOST_SECTION_PLANES, 33), (binding.PGSF_OPT_HOST_DEVICE_BUDGET, -1),
+                         (binding.PGSF_OPT_TUNE, -1), (binding.PGSF_OPT_TUNE, 1 << 16), (99, 0)]:
             with pytest.raises(binding.PgsfError) as ei:
                 plan.pgsf_plan_set_option(opt, val)
             assert ei.value.status == binding.PGSF_ERR_INVALID_ARG
