@@ -420,7 +420,7 @@ cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStr
 
 // frequency pass of one scale fused with the z-direction window sums of the statistics:
 // in (x/y-filtered cube) -> out (filtered cube), Z1, Z2
-int zm_step_channels_of(int rz_compiled) { return rz_compiled >= 96 ? 128 : 64; }   // = zm_step_channels<RZ>()
+int zm_step_channels_of(int rz_compiled) { return zm_step_rule(rz_compiled); }   // = zm_step_channels<RZ>()
 
 cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, int ncubes,
                     cudaStream_t st, const ZmSection *sec)

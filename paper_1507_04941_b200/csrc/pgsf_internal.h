@@ -152,7 +152,13 @@ cudaError_t fast_z(pgsf_plan *p, int scale, const float *in, float *out, cudaStr
                    float *ratio = nullptr);
 cudaError_t fast_zm(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, int ncubes,
                     cudaStream_t st, const ZmSection *sec = nullptr);
-int zm_step_channels_of(int rz_compiled);      // channels per march step of k_zm<RZ>
+// channels per march step of k_zm<RZ>: 64, or 128 where the slab of 64 + 2 RZ channels would leave room for two 4-warp
+// CTAs only (RZ = 96) and -- PGSF_ZM_WIDE_STEP_MAX_RZ, a build-time experiment -- for small radii
+#ifndef PGSF_ZM_WIDE_STEP_MAX_RZ
+#define PGSF_ZM_WIDE_STEP_MAX_RZ 0
+#endif
+constexpr int zm_step_rule(int rz_compiled) { return (rz_compiled >= 96 || rz_compiled <= PGSF_ZM_WIDE_STEP_MAX_RZ) ? 128 : 64; }
+int zm_step_channels_of(int rz_compiled);
 // the tensor-core variant of fast_zm (pgsf_ztc.cu): cudaErrorNotSupported = not for this plan / scale, run fast_zm
 bool ztc_radius(int rz_compiled);
 cudaError_t ztc_prepare(pgsf_plan *p);

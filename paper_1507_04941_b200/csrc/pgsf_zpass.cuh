@@ -368,7 +368,7 @@ cudaError_t launch_z(const float *in, float *out, float *ratio, const Dims &d, c
 // channels per march step: 64 (4 warps per CTA) up to RZ = 48; 128 (8 warps) above, where the slab of
 // 64 + 2 RZ channels would leave room for two 4-warp CTAs only
 template <int RZ>
-constexpr int zm_step_channels() { return RZ >= 96 ? 128 : 64; }
+constexpr int zm_step_channels() { return zm_step_rule(RZ); }
 
 template <int RZ>
 cudaError_t launch_zm(const float *in, float *out, float *Z1, float *Z2, const Dims &d, int hz, const float *pivot,

@@ -137,130 +137,145 @@ __global__ void __launch_bounds__(TC_NT) k_ztc(float *out, float *__restrict__ Z
     unsigned ph_tma = 0, ph_mma = 0;
     const float *row_out = out + (long long)y * d.nx + x0;     // column x0 of row y, channel 0
 
-    for (int k = p.kbeg; k < p.kend; ++k) {
-        const int z0 = k * TC_ZB;
-        // channels leaving the window in this step that earlier steps wrote: z0 - 2 hz + j < z0 (cp.async, L2)
+    // ---- the pieces of one step (z0 = 128 k) -------------------------------------------------------------------
+    auto issue_tma = [&](int z0) {        // slab channels z0 - rz .. z0 + 127 + rz: bulk tensor copies, zeros outside (C-5)
+        if (warp == 0) {
+            if (tid == 0) {
+                fence_proxy_async_smem();
+                mbar_arrive_expect_tx(&bar_tma, K * TC_XT * 4);
+                const int bz = K / p.nbox;
+                for (int b = 0; b < p.nbox; ++b)
+                    tma_load_4d(Bh + b * bz * TC_XT, &tmap, x0, y, z0 - p.rz + b * bz - p.zmap_lo, blockIdx.z, &bar_tma);
+            }
+            __syncwarp();
+        }
+    };
+    auto split_and_mma = [&]() {
+        mbar_wait(&bar_tma, ph_tma);
+        ph_tma ^= 1;
+        // split the slab: hi in place, lo beside it (element-wise, so the swizzle is irrelevant here)
+        float4 *bh4 = reinterpret_cast<float4 *>(Bh), *bl4 = reinterpret_cast<float4 *>(Bl);
+        for (int i = tid; i < K * 8; i += TC_NT) {
+            const float4 v = bh4[i];
+            float4 h, l;
+            h.x = rna_tf32(v.x); h.y = rna_tf32(v.y); h.z = rna_tf32(v.z); h.w = rna_tf32(v.w);
+            l.x = rna_tf32(v.x - h.x); l.y = rna_tf32(v.y - h.y); l.z = rna_tf32(v.z - h.z); l.w = rna_tf32(v.w - h.w);
+            bh4[i] = h;
+            bl4[i] = l;
+        }
+        fence_proxy_async_smem();
+        tc_fence_before();
+        __syncthreads();
+        if (warp == 0) {       // one lane issues; its warp waits at the __syncwarp, not spinning on a barrier
+            if (tid == 0) {
+                tc_fence_after();
+                // A: K-major, no swizzle, Hankel strip (LBO 128 B between the two K chunks, SBO 256 B between row groups),
+                //    256 bytes further per K step.  B: MN-major TF32 = 128-byte swizzle with 32-byte atoms (the only MN-major
+                //    layout for 32-bit operands): two atoms of 4 channels x 32 columns per K step, SBO 512 B between them.
+                unsigned long long ah = umma_desc(ah_addr, 128, 256, 0), al = umma_desc(al_addr, 128, 256, 0);
+                unsigned long long bh = umma_desc(bh_addr, 1024, 512, 1), bl = umma_desc(bl_addr, 1024, 512, 1);
+                for (int ks = 0; ks < K / 8; ++ks) {
+                    umma_tf32(tmem, ah, bh, ks > 0);
+                    umma_tf32(tmem, al, bh, 1);
+                    umma_tf32(tmem, ah, bl, 1);
+                    ah += 16; al += 16; bh += 64; bl += 64;        // (start-address field, units of 16 bytes)
+                }
+                umma_commit(&bar_mma);
+            }
+            __syncwarp();
+        }
+    };
+    auto stage_leaving = [&](int z0) {    // channels leaving the window in the step that earlier steps wrote (cp.async, L2)
         for (int i = tid; i < TC_ZB * 8; i += TC_NT) {
             const int j = i >> 3, ch = i & 7, zt = z0 - 2 * hz + j;
             const bool ok = zt >= 0 && zt < z0 && zt < nz && x0 + 4 * ch < d.nx;
             cp_async16(ts + j * TC_XT + 4 * ch, ok ? row_out + (long long)zt * d.plane + 4 * ch : out, ok);
         }
-        if (z0 < nz && warp == 0) {
-          if (tid == 0) {
-            // slab channels z0 - rz .. z0 + 127 + rz: bulk tensor copies, zeros outside the cube (C-5)
-            fence_proxy_async_smem();
-            mbar_arrive_expect_tx(&bar_tma, K * TC_XT * 4);
-            const int bz = K / p.nbox;
-            for (int b = 0; b < p.nbox; ++b)
-                tma_load_4d(Bh + b * bz * TC_XT, &tmap, x0, y, z0 - p.rz + b * bz - p.zmap_lo, blockIdx.z, &bar_tma);
-          }
-          __syncwarp();
-        }
-        cp_async_wait_all();
-        if (z0 < nz) {
-            mbar_wait(&bar_tma, ph_tma);
-            ph_tma ^= 1;
-            // split the slab: hi in place, lo beside it (element-wise, so the swizzle is irrelevant here)
-            float4 *bh4 = reinterpret_cast<float4 *>(Bh), *bl4 = reinterpret_cast<float4 *>(Bl);
-            for (int i = tid; i < K * 8; i += TC_NT) {
-                const float4 v = bh4[i];
-                float4 h, l;
-                h.x = rna_tf32(v.x); h.y = rna_tf32(v.y); h.z = rna_tf32(v.z); h.w = rna_tf32(v.w);
-                l.x = rna_tf32(v.x - h.x); l.y = rna_tf32(v.y - h.y); l.z = rna_tf32(v.z - h.z); l.w = rna_tf32(v.w - h.w);
-                bh4[i] = h;
-                bl4[i] = l;
-            }
-            fence_proxy_async_smem();
-            tc_fence_before();
-            __syncthreads();
-            if (warp == 0) {       // one lane issues; its warp waits at the __syncwarp, not spinning on the barrier
-              if (tid == 0) {
-                tc_fence_after();
-                for (int ks = 0; ks < K / 8; ++ks) {
-                    // A: K-major, no swizzle, Hankel strip (LBO 128 B between the two K chunks, SBO 256 B between row groups)
-                    // B: MN-major TF32 = 128-byte swizzle with 32-byte atoms (the only MN-major layout for 32-bit operands): two
-                    //    atoms of 4 channels x 32 columns per K step, SBO 512 B between them
-                    const unsigned long long ah = umma_desc(ah_addr + ks * 256, 128, 256, 0);
-                    const unsigned long long al = umma_desc(al_addr + ks * 256, 128, 256, 0);
-                    const unsigned long long bh = umma_desc(bh_addr + ks * 1024, 1024, 512, 1);
-                    const unsigned long long bl = umma_desc(bl_addr + ks * 1024, 1024, 512, 1);
-                    umma_tf32(tmem, ah, bh, ks > 0);
-                    umma_tf32(tmem, al, bh, 1);
-                    umma_tf32(tmem, ah, bl, 1);
-                }
-                umma_commit(&bar_mma);
-              }
-              __syncwarp();
-            }
-            mbar_wait(&bar_mma, ph_mma);
-            ph_mma ^= 1;
-#if defined(ZTC_DEBUG) && ZTC_DEBUG == 3
-            for (int w8 = 0; w8 < 50; ++w8) __nanosleep(10000);
-#endif
-            tc_fence_after();
-            // epilogue: TMEM lane L = row m' = 127 - (channel - z0); this thread takes lane tid
-            float v[32];
-            tmem_ld32(tmem + ((unsigned)(warp * 32) << 16), v);
-            const int j = TC_ZB - 1 - tid, gz = z0 + j;
-#ifdef ZTC_DEBUG
-#if ZTC_DEBUG == 1      // the slab as TMA landed it (hi part), channel of the output
-            { const int r = j + p.rz; for (int c2 = 0; c2 < 32; ++c2) v[c2] = Bh[r * 32 + ((((c2 >> 3) ^ (r & 3)) << 3) | (c2 & 7))]; }
-#elif ZTC_DEBUG == 2    // the band matrix row m' = tid, k = rz + 127 - tid + (c2 - 16)
-            { for (int c2 = 0; c2 < 32; ++c2) { const int u = tid + p.rz + 127 - tid + c2 - 16; const int t = u / 4; v[c2] = Ah[t * 32 + (u & 3)]; } }
-#endif
-#endif
-            float *g = out + (long long)gz * d.plane + (long long)y * d.nx + x0;
+    };
+    auto epilogue = [&](int z0) {         // TMEM lane L = row m' = 127 - (channel - z0); this thread takes lane tid
+        mbar_wait(&bar_mma, ph_mma);
+        ph_mma ^= 1;
+        tc_fence_after();
+        float v[32];
+        tmem_ld32(tmem + ((unsigned)(warp * 32) << 16), v);
+        const int j = TC_ZB - 1 - tid, gz = z0 + j;
+        float *g = out + (long long)gz * d.plane + (long long)y * d.nx + x0;
 #pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                const float4 w = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
-                *reinterpret_cast<float4 *>(fs + j * TC_XT + ((q ^ (j & 7)) << 2)) = w;
-                if (gz < nz && x0 + 4 * q < d.nx) *reinterpret_cast<float4 *>(g + 4 * q) = w;
-            }
-            tc_fence_before();
+        for (int q = 0; q < 8; ++q) {
+            const float4 w = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+            *reinterpret_cast<float4 *>(fs + j * TC_XT + ((q ^ (j & 7)) << 2)) = w;
+            if (gz < nz && x0 + 4 * q < d.nx) *reinterpret_cast<float4 *>(g + 4 * q) = w;
         }
-        __syncthreads();      // f slab and leaving slab complete; the accumulator has been read
-        if (c_ok && z0 >= 2 * hz && z0 + TC_ZB <= nz) {
-            // interior step: all entering and leaving channels (and all outputs) are inside the cube
+        tc_fence_before();
+    };
+    // window sums of one step.  The running value is s + e (two-sum compensated: the rounding error of every addition is
+    // recovered exactly and gathered in e).  In the interior the channel entering and the channel that left one output
+    // earlier are combined OFF the dependent chain, so the chain is one addition per channel.
+    auto acc_add = [&](float v) {
+        const float t = s + v, bp = t - s;
+        e += (s - (t - bp)) + (v - bp);
+        s = t;
+    };
+    auto window = [&](int z0) {
+        if (!c_ok) return;
+        const int cx = ((c >> 2) << 2), cl = c & 3;
+        if (z0 >= 2 * hz && z0 + TC_ZB <= nz) {
             const int jsplit = min(2 * hz, TC_ZB);     // leaving channel: ts[j] for j < jsplit, else fs[j - 2 hz]
             float *zp = Zq + (long long)(z0 - hz) * d.plane + cb;
-            const int cx = ((c >> 2) << 2), cl = c & 3;
+            float pb = 0.f;                            // the leaving term of the previous output, not yet subtracted
 #pragma unroll 4
             for (int j = 0; j < TC_ZB; ++j) {
                 const float a = fs[j * TC_XT + ((cx ^ ((j & 7) << 2)) | cl)] - c0;
                 const int jt = j - 2 * hz;
                 const float b = (j < jsplit ? ts[j * TC_XT + c] : fs[jt * TC_XT + ((cx ^ ((jt & 7) << 2)) | cl)]) - c0;
-                if (sq) {
-                    kahan_add(s, e, a * a);
-                    *zp = s - e;
-                    kahan_add(s, e, -(b * b));
-                } else {
-                    s += a;
-                    *zp = s;
-                    s -= b;
-                }
+                const float va = sq ? a * a : a, vb = sq ? b * b : b;
+                acc_add(va - pb);
+                pb = vb;
+                *zp = s + e;
                 zp += d.plane;
             }
-        } else if (c_ok) {
+            acc_add(-pb);
+        } else {
             for (int j = 0; j < TC_ZB; ++j) {
                 const int zl = z0 + j, zo = zl - hz;       // channel entering the window of output zo
                 if (zl < nz) {
                     const float a = fs[fs_idx(j, c)] - c0;
-                    if (sq) kahan_add(s, e, a * a);
-                    else s += a;
+                    acc_add(sq ? a * a : a);
                 }
                 if (zo >= 0 && zo < nz) {
-                    Zq[(long long)zo * d.plane + cb] = s - e;
+                    Zq[(long long)zo * d.plane + cb] = s + e;
                     const int jt = j - 2 * hz;             // the channel leaving after this output, relative to z0
                     if (zo - hz >= 0) {
                         const float b = (jt >= 0 ? fs[fs_idx(jt, c)] : ts[j * TC_XT + c]) - c0;
-                        if (sq) kahan_add(s, e, -(b * b));
-                        else s -= b;
+                        acc_add(sq ? -(b * b) : -b);
                     }
                 }
             }
         }
-        __syncthreads();      // slabs are overwritten by the next step
+    };
+
+    // ---- the march: the window sums of step k - 1 run under the MMAs of step k; the slab of step k + 1 is requested
+    //      as soon as the MMAs of step k have retired
+    bool pending = false;
+    int pending_z0 = 0;
+    if (p.kbeg < p.kend && p.kbeg * TC_ZB < nz) issue_tma(p.kbeg * TC_ZB);
+    for (int k = p.kbeg; k < p.kend; ++k) {
+        const int z0 = k * TC_ZB;
+        const bool have = z0 < nz;
+        if (have) split_and_mma();
+        if (pending) window(pending_z0);
+        __syncthreads();                  // the window walk is done with the f and leaving slabs
+        stage_leaving(z0);
+        if (have) {
+            epilogue(z0);
+            if (k + 1 < p.kend && (k + 1) * TC_ZB < nz) issue_tma((k + 1) * TC_ZB);
+        }
+        cp_async_wait_all();
+        __syncthreads();                  // f slab and leaving slab of step k complete; the accumulator has been read
+        pending = true;
+        pending_z0 = z0;
     }
+    if (pending) window(pending_z0);
     if (st_s != nullptr) { st_s[0] = s; st_s[d.plane] = e; }
     tc_fence_before();
     __syncthreads();
