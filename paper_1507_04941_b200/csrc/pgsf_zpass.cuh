@@ -169,21 +169,23 @@ __global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, f
 // n steps of the sliding window of one (column, quantity; the sum of f^2 Kahan-compensated): add the entering channel, write
 // the window sum, subtract the leaving channel.  lead / trail advance by one staged channel per step.
 template <bool SQ, int XT>
-__device__ __forceinline__ float *window_run(float &s, float &e, const float *__restrict__ lead,
+__device__ __forceinline__ float *window_run(float &s, float &e, float &pb, const float *__restrict__ lead,
                                              const float *__restrict__ trail, float *__restrict__ zp, long long plane, int n,
                                              float c0)
 {
+    // pb = the leaving term of the previous output, not yet subtracted: it is combined with the entering term off the
+    // dependent chain, so the running sum sees ONE (compensated) addition per channel instead of two
 #pragma unroll 8
     for (int j = 0; j < n; ++j) {
         const float a = lead[j * XT] - c0, b = trail[j * XT] - c0;     // (pivot c0: D-2)
         if constexpr (SQ) {
-            kahan_add(s, e, a * a);
+            kahan_add(s, e, a * a - pb);
+            pb = b * b;
             *zp = s - e;
-            kahan_add(s, e, -(b * b));
         } else {                // sum of f: enters only through the mean, whose tolerance is ~n times looser
-            s += a;
+            s += a - pb;
+            pb = b;
             *zp = s;
-            s -= b;
         }
         zp += plane;
     }
@@ -314,12 +316,15 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
                 // interior step: all 64 entering and all 64 leaving channels (and all 64 outputs) are inside the cube
                 const int jsplit = min(2 * hz, ZB);   // leaving channel: ts[j] for j < jsplit, else fs[j - 2 hz]
                 float *zp = Zq + (long long)(z0 - hz) * d.plane + cb;
+                float pb = 0.f;
                 if (sq) {
-                    zp = window_run<true, XT>(s, e, fs + c, ts + c, zp, d.plane, jsplit, c0);
-                    window_run<true, XT>(s, e, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit, c0);
+                    zp = window_run<true, XT>(s, e, pb, fs + c, ts + c, zp, d.plane, jsplit, c0);
+                    window_run<true, XT>(s, e, pb, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit, c0);
+                    kahan_add(s, e, -pb);
                 } else {
-                    zp = window_run<false, XT>(s, e, fs + c, ts + c, zp, d.plane, jsplit, c0);
-                    window_run<false, XT>(s, e, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit, c0);
+                    zp = window_run<false, XT>(s, e, pb, fs + c, ts + c, zp, d.plane, jsplit, c0);
+                    window_run<false, XT>(s, e, pb, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit, c0);
+                    s -= pb;
                 }
             } else {
                 for (int j = 0; j < ZB; ++j) {
