@@ -374,8 +374,22 @@ def measure_workload(w, dev, device_index, rank, world, steps, warmup, peaks, sm
                          "timed": "per-launch CUDA events in a separate pass of %d steps (%.3f ms per step with the "
                                   "events on; the headline loop runs with them off)" % (psteps, ms_prof_total / psteps)})
     out["roofline"] = roofline
-    out["kernels"] = [{"name": k["name"], "launches": k["launches"], "ms_per_launch": round(k["ms_per_launch"], 4),
-                       "share": round(k["share"], 4)} for k in kern]
+    def _entry(k):
+        # every kernel against its own roofline (algorithmic work as _kernel_work counts it) and, where the committed
+        # ncu launch list has it, the DRAM bytes it really moved as a fraction of the HBM peak
+        sec = max(k["ms_per_launch"] * 1e-3, 1e-12)
+        f_alu = k["flops"] / sec / 1e12 / alu_peak
+        f_hbm = k["bytes"] / sec / 1e9 / hbm_peak
+        tr = _dram_traffic(w.name, k["name"])
+        e = {"name": k["name"], "launches": k["launches"], "ms_per_launch": round(k["ms_per_launch"], 4),
+             "share": round(k["share"], 4), "bound": "alu" if f_alu >= f_hbm else "hbm",
+             "frac": round(max(f_alu, f_hbm), 4)}
+        if tr is not None:
+            e["traffic_frac_of_hbm_peak"] = round(tr / sec / 1e9 / hbm_peak, 4)
+        return e
+    out["kernels"] = [_entry(k) for k in kern]
+    if roofline is not None and roofline.get("traffic"):
+        roofline["traffic_frac_of_hbm_peak"] = roofline["traffic"] / (roofline["ms_per_launch"] * 1e-3) / 1e9 / hbm_peak
 
     # ---- SURVEY.md 8(d) metric (i): per scale, N / (t_filter3d + t_local_threshold) through the per-scale calls
     per_scale = []

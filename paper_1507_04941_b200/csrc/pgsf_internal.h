@@ -180,7 +180,12 @@ cudaError_t fast_threshold_xy(pgsf_plan *p, const float *f, const float *Z1, con
                               cudaStream_t st);
 // k_xyb (pgsf_xyb.cu): the successor of k_ymarch; same arguments
 bool xyb_supported(const pgsf_plan *p);
-inline bool stats_sparse_or(const pgsf_plan *p) { return p->fast_stats && xyb_supported(p) && !(p->tune & 2); }
+inline bool stats_sparse_or(const pgsf_plan *p)
+{
+    const int hx = p->desc.box_half[0];
+    const bool legacy_ok = (hx == 4 || hx == 8 || hx == 16) && p->desc.nx % (hx / 2) == 0;
+    return p->fast_stats && xyb_supported(p) && (!(p->tune & 2) || !legacy_ok);
+}
 // nplanes > 0: the pointers address planes z_off .. z_off + nplanes - 1 of one cube (a section of the streamed cube)
 cudaError_t xyb_threshold(pgsf_plan *p, const float *f, const float *Z1, const float *Z2, uint8_t *mask, int mode,
                           float *mean, float *sd, unsigned long long *count, int ncubes, cudaStream_t st,

@@ -405,8 +405,8 @@ bool fast_stats_supported(const pgsf_plan *p, std::string *why)
     char buf[128];
     buf[0] = 0;
     if (p->desc.nx % 4 != 0) snprintf(buf, sizeof buf, "nx %% 4 != 0");
-    else if (hx != 4 && hx != 8 && hx != 16) snprintf(buf, sizeof buf, "hx = %d is not one of the compiled 4, 8, 16", hx);
-    else if (p->desc.nx % (hx / 2) != 0) snprintf(buf, sizeof buf, "nx %% (hx / 2) != 0");   // a thread owns hx/2 whole columns
+    else if (xyb_supported(p)) { /* k_xyb: hx in {4, 8, 12, 16}, any nx that is a multiple of 4 */ }
+    else if (hx != 4 && hx != 8 && hx != 12 && hx != 16) snprintf(buf, sizeof buf, "hx = %d is not one of the compiled 4, 8, 12, 16", hx);
     else if (p->desc.nz > 65535) snprintf(buf, sizeof buf, "nz above 65535");
     if (why) *why = buf;
     return buf[0] == 0;
@@ -446,7 +446,10 @@ cudaError_t fast_threshold_xy(pgsf_plan *p, const float *f, const float *Z1, con
                               int mode, float *mean, float *sd, unsigned long long *count, int ncubes,
                               cudaStream_t st)
 {
-    if (xyb_supported(p) && !(p->tune & 2)) return xyb_threshold(p, f, Z1, Z2, mask, mode, mean, sd, count, ncubes, st);
+    // k_ymarch (PGSF_OPT_TUNE bit 1) exists for hx = 4, 8, 16 with nx a multiple of hx / 2 only
+    const int hx0 = p->desc.box_half[0];
+    const bool legacy_ok = (hx0 == 4 || hx0 == 8 || hx0 == 16) && p->desc.nx % (hx0 / 2) == 0;
+    if (xyb_supported(p) && (!(p->tune & 2) || !legacy_ok)) return xyb_threshold(p, f, Z1, Z2, mask, mode, mean, sd, count, ncubes, st);
     if (mode == 2) return cudaErrorNotSupported;   // (callers ask stats_sparse_or() first)
     const int or_into = mode;
     const Dims &d = p->dims;

@@ -43,12 +43,14 @@ struct XybShape {
     static constexpr int HX = 2 * G;
     static constexpr int SWS = 32 * G;             // staged columns of one strip (one warp-row of the x phase)
     static constexpr int WMAX = SWS - 2 * HX;      // output columns of one strip
-    static constexpr int NSTRIP = 256 / SWS;       // strips per CTA
+    static constexpr int NSTRIP = 256 / SWS;       // strips per CTA (G = 6: one strip of 192 columns, 32 threads without a y pair)
     static constexpr int NT = 128;                 // threads: one per pair of the 256 staged columns
     static constexpr int RB = 4;                   // rows per batch
     static constexpr int UPW = NSTRIP * RB / 4;    // (strip, row) units of the x phase per warp and batch
     static constexpr int TPS = SWS / 2;            // y-phase threads per strip
     static constexpr int CPL = G / 2;              // 16-byte chunks (column pairs) per x-phase lane
+    static constexpr int VL = (G % 4 == 0) ? 4 : 2; // columns per global load / mask word of the x phase
+    static constexpr int NV = G / VL;
 };
 
 struct XybParams {
@@ -140,7 +142,7 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
                                                 const float *__restrict__ pivot, const float *__restrict__ zeros)
 {
     using S = XybShape<G>;
-    constexpr int HX = S::HX, NSTRIP = S::NSTRIP, RB = S::RB, UPW = S::UPW, TPS = S::TPS, CPL = S::CPL;
+    constexpr int HX = S::HX, NSTRIP = S::NSTRIP, RB = S::RB, UPW = S::UPW, TPS = S::TPS, CPL = S::CPL, VL = S::VL, NV = S::NV;
     __shared__ __align__(16) float4 ybuf[2][RB][128];
     __shared__ unsigned wsum[4];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -158,7 +160,7 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
     //      on a buffer of zeros with stride 0.
     const int ystrip = blockIdx.x * NSTRIP + tid / TPS;
     const int cy = ystrip * p.wo - HX + 2 * (tid % TPS);
-    const bool ycol_ok = ystrip < p.nstrips && cy >= 0 && cy + 2 <= nx;
+    const bool ycol_ok = tid / TPS < NSTRIP && ystrip < p.nstrips && cy >= 0 && cy + 2 <= nx;
     const int r0 = ya - hy;                            // first row entering the window of output row ya
     const int nrows = (yb - ya) + 2 * hy;              // entering rows r0 .. yb - 1 + hy
     const int nb = (nrows + RB - 1) / RB;
@@ -209,6 +211,7 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
     float nxz[UPW][G];                                 // clipped window lengths along x times along z
     unsigned core_x[UPW];                              // bit j: column j is outside the x / z halo
     long long voff[UPW];                               // element offset of (xo, row of the current batch's unit)
+    int nvq[UPW];                                      // load / store words of the group that lie inside the cube
     {
         const float nzc = (float)xyb_clipped_len(z, p.hz, p.nz_full);
         const bool core_z = z >= p.gz && z < p.nz_full - p.gz;
@@ -217,6 +220,7 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
             const int unit = warp + 4 * u, strip = blockIdx.x * NSTRIP + unit / RB;
             const int xo = strip * p.wo + G * lane;
             out_ok[u] = strip < p.nstrips && G * lane < p.wo && xo < nx;
+            nvq[u] = min(NV, max(0, (nx - xo) / VL));          // (the last group of a row may stick out of the cube)
             core_x[u] = 0;
 #pragma unroll
             for (int j = 0; j < G; ++j) {
@@ -245,19 +249,20 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
     load_rows(0);
     // centre values (and previous mask bytes) of the outputs of batch b: fetched one batch ahead, so that they are in
     // flight for a whole batch (two register sets used alternately)
-    auto load_centre = [&](int b, float (&fv)[UPW][G], unsigned (&mk)[UPW][(G + 3) / 4]) {
+    auto load_centre = [&](int b, float (&fv)[UPW][G], unsigned (&mk)[UPW][NV]) {
 #pragma unroll
         for (int u = 0; u < UPW; ++u) {
             const int yo = r0 - hy + RB * b + (warp + 4 * u) % RB;
-            const bool ok = out_ok[u] && yo >= ya && yo < yb;
+            const bool okr = out_ok[u] && yo >= ya && yo < yb;
             const long long o = voff[u] + (long long)(RB * b) * nx;
-            if constexpr (G == 2) {
-                const float2 t = ok ? __ldg(reinterpret_cast<const float2 *>(f + o)) : make_float2(0.f, 0.f);
-                fv[u][0] = t.x; fv[u][1] = t.y;
-                mk[u][0] = (MODE == 1 && ok) ? *reinterpret_cast<const unsigned short *>(mask + o) : 0u;
-            } else {
 #pragma unroll
-                for (int q = 0; q < G / 4; ++q) {
+            for (int q = 0; q < NV; ++q) {
+                const bool ok = okr && q < nvq[u];
+                if constexpr (VL == 2) {
+                    const float2 t = ok ? __ldg(reinterpret_cast<const float2 *>(f + o) + q) : make_float2(0.f, 0.f);
+                    fv[u][2 * q] = t.x; fv[u][2 * q + 1] = t.y;
+                    mk[u][q] = (MODE == 1 && ok) ? *reinterpret_cast<const unsigned short *>(mask + o + 2 * q) : 0u;
+                } else {
                     const float4 t = ok ? __ldg(reinterpret_cast<const float4 *>(f + o) + q) : make_float4(0.f, 0.f, 0.f, 0.f);
                     fv[u][4 * q] = t.x; fv[u][4 * q + 1] = t.y; fv[u][4 * q + 2] = t.z; fv[u][4 * q + 3] = t.w;
                     mk[u][q] = (MODE == 1 && ok) ? *reinterpret_cast<const unsigned *>(mask + o + 4 * q) : 0u;
@@ -265,8 +270,8 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
             }
         }
     };
-    auto batch = [&](int b, float (&fv)[UPW][G], unsigned (&mk)[UPW][(G + 3) / 4], float (&fvn)[UPW][G],
-                     unsigned (&mkn)[UPW][(G + 3) / 4]) {
+    auto batch = [&](int b, float (&fv)[UPW][G], unsigned (&mk)[UPW][NV], float (&fvn)[UPW][G],
+                     unsigned (&mkn)[UPW][NV]) {
         const int par = b & 1;
         const int yrow = r0 - hy + RB * b;             // output row of batch row 0
         if (b + 1 < nb) load_centre(b + 1, fvn, mkn);
@@ -349,27 +354,29 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
                 }
             } else {
                 if constexpr (MODE == 1) {   // previous mask: any non-zero byte counts as set
-                    if constexpr (G == 2) {
-                        bits |= ((mk[u][0] & 0xffu) ? 1u : 0u) | ((mk[u][0] & 0xff00u) ? 2u : 0u);
-                    } else {
 #pragma unroll
-                        for (int q4 = 0; q4 < G / 4; ++q4) {
-                            const unsigned old = mk[u][q4];
+                    for (int q = 0; q < NV; ++q) {
+                        const unsigned old = mk[u][q];
+                        if constexpr (VL == 2) {
+                            bits |= (((old & 0xffu) ? 1u : 0u) | ((old & 0xff00u) ? 2u : 0u)) << (2 * q);
+                        } else {
                             const unsigned nzb = ((old | ((old & 0x7f7f7f7fu) + 0x7f7f7f7fu)) >> 7) & 0x01010101u;
-                            bits |= ((nzb & 1u) | ((nzb >> 7) & 2u) | ((nzb >> 14) & 4u) | ((nzb >> 21) & 8u)) << (4 * q4);
+                            bits |= ((nzb & 1u) | ((nzb >> 7) & 2u) | ((nzb >> 14) & 4u) | ((nzb >> 21) & 8u)) << (4 * q);
                         }
                     }
                     bits = core_y ? (bits & core_x[u]) : 0u;
                 }
                 my_count += __popc(bits);
-                if constexpr (G == 2) {
-                    *reinterpret_cast<unsigned short *>(mask + idx) = (unsigned short)((bits & 1u) | ((bits & 2u) << 7));
-                } else {
 #pragma unroll
-                    for (int q4 = 0; q4 < G / 4; ++q4) {
-                        const unsigned b4 = (bits >> (4 * q4)) & 15u;
+                for (int q = 0; q < NV; ++q) {
+                    if (q >= nvq[u]) break;
+                    if constexpr (VL == 2) {
+                        const unsigned b2 = (bits >> (2 * q)) & 3u;
+                        *reinterpret_cast<unsigned short *>(mask + idx + 2 * q) = (unsigned short)((b2 & 1u) | ((b2 & 2u) << 7));
+                    } else {
+                        const unsigned b4 = (bits >> (4 * q)) & 15u;
                         // bit i -> byte i: the partial products i + 7 k land on a multiple of 8 only for k = i
-                        *reinterpret_cast<unsigned *>(mask + idx + 4 * q4) = (b4 * 0x00204081u) & 0x01010101u;
+                        *reinterpret_cast<unsigned *>(mask + idx + 4 * q) = (b4 * 0x00204081u) & 0x01010101u;
                     }
                 }
             }
@@ -378,6 +385,7 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
                 for (int j = 0; j < G; ++j) {
                     const float n = nxz[u][j] * nyc;
                     const float m = S1[j] / n;
+                    if (j >= VL * nvq[u]) break;
                     if (mean != nullptr) mean[idx + j] = m + piv;
                     if (sd != nullptr) sd[idx + j] = sqrtf(fmaxf(S2[j] / n - m * m, 0.f));
                 }
@@ -386,7 +394,7 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
     };
     {
         float fvA[UPW][G], fvB[UPW][G];
-        unsigned mkA[UPW][(G + 3) / 4], mkB[UPW][(G + 3) / 4];
+        unsigned mkA[UPW][NV], mkB[UPW][NV];
         load_centre(0, fvA, mkA);
         for (int b = 0; b < nb; b += 2) {
             batch(b, fvA, mkA, fvB, mkB);
@@ -426,9 +434,10 @@ cudaError_t launch_xyb(const pgsf_plan *pl, const float *f, const float *Z1, con
     using S = XybShape<G>;
     const Dims &d = p.d;
     (void)pl;
-    // balanced strips of whole groups of 8 columns
+    // balanced strips of whole column groups
     int ns = (d.nx + S::WMAX - 1) / S::WMAX;
-    p.wo = ((d.nx + ns - 1) / ns + 7) / 8 * 8;
+    constexpr int WQ = (G == 6) ? 24 : 8;          // whole groups of G columns and whole 32-byte sectors
+    p.wo = ((d.nx + ns - 1) / ns + WQ - 1) / WQ * WQ;
     if (p.wo > S::WMAX) p.wo = S::WMAX;
     ns = (d.nx + p.wo - 1) / p.wo;
     p.nstrips = ns;
@@ -455,7 +464,7 @@ cudaError_t launch_xyb(const pgsf_plan *pl, const float *f, const float *Z1, con
 bool xyb_supported(const pgsf_plan *p)
 {
     const int hx = p->desc.box_half[0];
-    return p->desc.nx % 4 == 0 && (hx == 4 || hx == 8 || hx == 16) && p->desc.nz <= 65535;
+    return p->desc.nx % 4 == 0 && (hx == 4 || hx == 8 || hx == 12 || hx == 16) && p->desc.nz <= 65535;
 }
 
 cudaError_t xyb_threshold(pgsf_plan *p, const float *f, const float *Z1, const float *Z2, uint8_t *mask, int mode,
@@ -484,6 +493,7 @@ cudaError_t xyb_threshold(pgsf_plan *p, const float *f, const float *Z1, const f
     switch (p->desc.box_half[0]) {
     case 4: return launch_xyb<2>(p, f, Z1, Z2, mask, mean, sd, count, xp, ncubes, st);
     case 8: return launch_xyb<4>(p, f, Z1, Z2, mask, mean, sd, count, xp, ncubes, st);
+    case 12: return launch_xyb<6>(p, f, Z1, Z2, mask, mean, sd, count, xp, ncubes, st);
     case 16: return launch_xyb<8>(p, f, Z1, Z2, mask, mean, sd, count, xp, ncubes, st);
     default: return cudaErrorNotSupported;
     }

@@ -94,6 +94,8 @@ def _dry(binding, dims=(64, 48, 80), sigmas=((1, 1, 2), (2, 2, 4)), box=(4, 4, 8
 
 @pytest.mark.parametrize("dims,sigmas,box,flags,tiled,needle", [
     ((64, 48, 80), ((1, 1, 2),), (4, 4, 8), 0, True, "tiled"),
+    ((100, 48, 80), ((1, 1, 2),), (12, 12, 24), 0, True, "k_xyb"),                # hx = 12, nx % 6 != 0: still tiled
+    ((64, 48, 80), ((1, 1, 2),), (10, 4, 8), 0, False, "hx = 10"),
     ((64, 48, 80), ((1, 1, 2),), (4, 4, 8), 1, False, "FORCE_GENERIC"),
     ((62, 48, 80), ((1, 1, 2),), (4, 4, 8), 0, False, "nx % 4"),
     ((64, 48, 80), ((5, 1, 2),), (4, 4, 8), 0, False, "radii (15, 3, 6)"),        # x radius above the compiled 12

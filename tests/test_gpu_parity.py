@@ -98,6 +98,9 @@ def test_config1_full(pg, synth, oracle, flags, k):
     ((200, 150, 90), ((3, 3, 8),), (8, 8, 16)),
     ((101, 67, 83), ((1, 1.5, 2), (2.5, 2, 4)), (3, 4, 5)),       # nx % 4 != 0 -> generic kernels
     ((36, 300, 40), ((2, 1, 3),), (16, 2, 7)),
+    ((200, 70, 60), ((1, 1, 2), (2, 2, 4)), (12, 12, 24)),        # hx = 12 on the tiled statistics kernel (k_xyb<6>)
+    ((236, 40, 50), ((1, 1, 2),), (16, 6, 5)),                    # nx % 8 == 4: the last column group sticks out
+    ((100, 40, 50), ((1, 1, 2),), (12, 3, 4)),                    # nx % 6 != 0 with hx = 12
 ])
 def test_ragged_cubes_full(pg, synth, oracle, flags, dims, sigmas, box):
     from dataclasses import replace
