@@ -263,8 +263,10 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
     p->group_max = p->group;
     if (!dry) {
         cudaError_t e = cudaSetDevice(device);
-        if (e == cudaSuccess) e = cudaMalloc(&p->d_pivot, 256);
-        if (e == cudaSuccess) e = cudaMemset(p->d_pivot, 0, 256);
+        // constant block: [0] the pivot, bytes 64.. zeros (k_xyb's source for columns outside the cube), bytes 1024.. the
+        // partial sums of the pivot reduction
+        if (e == cudaSuccess) e = cudaMalloc(&p->d_pivot, 4096);
+        if (e == cudaSuccess) e = cudaMemset(p->d_pivot, 0, 4096);
         if (e != cudaSuccess) {
             cudaGetLastError();
             delete p;

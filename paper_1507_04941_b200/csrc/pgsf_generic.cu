@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(kThreads) k_conv1d(const float *__restrict__ i
 // the data), fp64, fixed summation order.  The pivot is applied only where it is free of cost: when the samples
 // sit within a quarter of their mean (|mean| >= 4 sd), f - c is an exact fp32 subtraction for nearly every voxel
 // (Sterbenz: c/2 <= f <= 2c); for data scattered around zero the pivot is 0 and nothing changes.
-constexpr int kPivotThreads = 1024;
+constexpr int kPivotThreads = 256;
 constexpr int kPivotAxis = 100;
 
 }  // namespace
@@ -62,13 +62,20 @@ void pivot_lattice(const Dims &d, int lo[3], int st[3], int cnt[3]) { pivot_latt
 namespace {
 
 // sample i of the lattice comes from fetch(i); one CTA, fixed summation order
+// Two deterministic stages: kPivotBlocks CTAs each reduce a contiguous range of the samples (fixed order inside the
+// CTA) to a partial (sum, sum of squares) in the plan's constant block; one CTA then adds the partials in index order.
+constexpr int kPivotBlocks = 64;
+constexpr int kPivotPartialOffset = 128;     // in doubles from the start of the constant block (= byte 1024)
+
 template <class Fetch>
-__device__ __forceinline__ void pivot_reduce(Fetch fetch, int nsamp, float *__restrict__ pivot)
+__device__ __forceinline__ void pivot_partial(Fetch fetch, int nsamp, double *__restrict__ partial)
 {
     __shared__ double part[kPivotThreads];
     __shared__ double part2[kPivotThreads];
+    const int chunk = (nsamp + kPivotBlocks - 1) / kPivotBlocks;
+    const int i0 = blockIdx.x * chunk, i1 = min(i0 + chunk, nsamp);
     double acc = 0.0, acc2 = 0.0;
-    for (int i = threadIdx.x; i < nsamp; i += kPivotThreads) {
+    for (int i = i0 + threadIdx.x; i < i1; i += kPivotThreads) {
         const double v = (double)fetch(i);
         acc += v;
         acc2 += v * v;
@@ -80,29 +87,35 @@ __device__ __forceinline__ void pivot_reduce(Fetch fetch, int nsamp, float *__re
         if ((int)threadIdx.x < w) { part[threadIdx.x] += part[threadIdx.x + w]; part2[threadIdx.x] += part2[threadIdx.x + w]; }
         __syncthreads();
     }
-    if (threadIdx.x == 0) {
-        const double m = part[0] / (double)nsamp;
-        const double var = fmax(part2[0] / (double)nsamp - m * m, 0.0);
-        *pivot = (m * m >= 16.0 * var && m != 0.0) ? (float)m : 0.f;
-    }
+    if (threadIdx.x == 0) { partial[2 * blockIdx.x] = part[0]; partial[2 * blockIdx.x + 1] = part2[0]; }
 }
 
-__global__ void __launch_bounds__(kPivotThreads) k_pivot(const float *__restrict__ data, Dims d, float *__restrict__ pivot)
+__global__ void __launch_bounds__(kPivotThreads) k_pivot(const float *__restrict__ data, Dims d, float *__restrict__ cblock)
 {
     int lo[3], st[3], cnt[3];
     pivot_lattice_hd(d, lo, st, cnt);
     const int nsamp = cnt[0] * cnt[1] * cnt[2];
-    pivot_reduce([&](int i) {
+    pivot_partial([&](int i) {
         const int ix = i % cnt[0], iy = (i / cnt[0]) % cnt[1], iz = i / (cnt[0] * cnt[1]);
         const long long o = (long long)(lo[0] + ix * st[0]) + (long long)d.nx * ((lo[1] + iy * st[1]) + (long long)d.ny * (lo[2] + iz * st[2]));
         return __ldg(data + o);
-    }, nsamp, pivot);
+    }, nsamp, reinterpret_cast<double *>(cblock) + kPivotPartialOffset);
 }
 
 // the same reduction over samples gathered beforehand, in lattice order
-__global__ void __launch_bounds__(kPivotThreads) k_pivot_list(const float *__restrict__ list, int nsamp, float *__restrict__ pivot)
+__global__ void __launch_bounds__(kPivotThreads) k_pivot_list(const float *__restrict__ list, int nsamp, float *__restrict__ cblock)
 {
-    pivot_reduce([&](int i) { return __ldg(list + i); }, nsamp, pivot);
+    pivot_partial([&](int i) { return __ldg(list + i); }, nsamp, reinterpret_cast<double *>(cblock) + kPivotPartialOffset);
+}
+
+__global__ void k_pivot_final(float *__restrict__ cblock, int nsamp)
+{
+    const double *partial = reinterpret_cast<const double *>(cblock) + kPivotPartialOffset;
+    double s = 0.0, s2 = 0.0;
+    for (int b = 0; b < kPivotBlocks; ++b) { s += partial[2 * b]; s2 += partial[2 * b + 1]; }
+    const double m = s / (double)nsamp;
+    const double var = fmax(s2 / (double)nsamp - m * m, 0.0);
+    cblock[0] = (m * m >= 16.0 * var && m != 0.0) ? (float)m : 0.f;
 }
 
 // One directional sum of P:152 over the window clipped to the cube (C-7).
@@ -194,14 +207,20 @@ inline unsigned grid_for(long long n) { return (unsigned)((n + kThreads - 1) / k
 cudaError_t compute_pivot_list(pgsf_plan *p, const float *d_list, int nsamp, cudaStream_t st)
 {
     LaunchScope ls(p, "pivot", st);
-    k_pivot_list<<<1, kPivotThreads, 0, st>>>(d_list, nsamp, p->d_pivot);
+    p->launches += 1;          // (two kernels)
+    k_pivot_list<<<kPivotBlocks, kPivotThreads, 0, st>>>(d_list, nsamp, p->d_pivot);
+    k_pivot_final<<<1, 1, 0, st>>>(p->d_pivot, nsamp);
     return cudaGetLastError();
 }
 
 cudaError_t compute_pivot(pgsf_plan *p, const float *data, cudaStream_t st)
 {
     LaunchScope ls(p, "pivot", st);
-    k_pivot<<<1, kPivotThreads, 0, st>>>(data, p->dims, p->d_pivot);
+    p->launches += 1;          // (two kernels)
+    int lo[3], s3[3], cnt[3];
+    pivot_lattice_hd(p->dims, lo, s3, cnt);
+    k_pivot<<<kPivotBlocks, kPivotThreads, 0, st>>>(data, p->dims, p->d_pivot);
+    k_pivot_final<<<1, 1, 0, st>>>(p->d_pivot, cnt[0] * cnt[1] * cnt[2]);
     return cudaGetLastError();
 }
 

@@ -130,7 +130,8 @@ cudaError_t generic_filter3d(pgsf_plan *p, int scale, const float *in, float *ou
 // of the cube at `data` (for a group of cubes: of its first cube).
 // The selection n f - S1 > k sqrt(n S2 - S1^2) is invariant under f -> f - c for any constant c; taking c near the
 // level of the data keeps S2/n - m^2 well conditioned in fp32 when the cube carries an offset |mean| >> sd.
-// One CTA, fixed summation order (deterministic; exact under power-of-two scaling of the data).
+// 64 CTAs reduce fixed ranges of the samples, one thread adds their partial sums in order (deterministic; exact under
+// power-of-two scaling of the data).
 cudaError_t compute_pivot(pgsf_plan *p, const float *data, cudaStream_t st);
 // tmp: 4 cubes
 cudaError_t generic_threshold(pgsf_plan *p, const float *f, uint8_t *mask, int or_into, float *mean,
