@@ -21,7 +21,7 @@
  * Also here: Eq. 1, the weighted convolution (NEXT-1 of SURVEY.md 8(f)), at both levels, and Eq. 2
  * for an arbitrary non-separable filter array (NEXT-2).
  *
- * Pins: tests/test_oracle_pins.py (S1-S15, W1-W6 and G1-G3 of DESIGN.md).  Nothing here is "parity unpinned"
+ * Pins: tests/test_oracle_pins.py (S1-S15, W1-W6, G1-G3 and L1-L4 of DESIGN.md).  Nothing here is "parity unpinned"
  * except agreement with the authors' own PGSF output on their simulated cube, which is not
  * available (no code, no data).
  */
@@ -467,4 +467,41 @@ void pgsf_oracle_filter_general(const float *d, int nx, int ny, int nz, const do
                 }
                 c[(i64)x + (i64)nx * ((i64)y + (i64)ny * z)] = sum;
             }
+}
+
+/* ---------------------------------------------------------------- NEXT-4: mask -> candidate objects
+ * The paper merges the selected voxels into sources and "combin[es] the results to a single, parameterised
+ * catalogue" (the selection step is P:282) without saying how voxels are joined.  Reading C-19: an
+ * object is a connected component of the OR mask under 26-connectivity (voxels touching by a face, an edge or a corner
+ * belong together), every cube of a batch on its own.  Label of a component = 1 + the smallest linear index
+ * x + nx (y + ny z) of its voxels; background = 0.  Plain flood fill in index order, so the first voxel met of a
+ * component IS its smallest index.  Returns the number of components. */
+i64 pgsf_oracle_label26(const uint8_t *mask, int nx, int ny, int nz, uint32_t *labels)
+{
+    const i64 n = (i64)nx * ny * nz;
+    i64 *stack = (i64 *)malloc(sizeof(i64) * (size_t)(n > 0 ? n : 1));
+    i64 count = 0;
+    memset(labels, 0, sizeof(uint32_t) * (size_t)n);
+    for (i64 i = 0; i < n; ++i) {
+        if (!mask[i] || labels[i]) continue;
+        const uint32_t lab = (uint32_t)(i + 1);
+        i64 top = 0;
+        stack[top++] = i;
+        labels[i] = lab;
+        ++count;
+        while (top > 0) {
+            const i64 v = stack[--top];
+            const int x = (int)(v % nx), y = (int)((v / nx) % ny), z = (int)(v / ((i64)nx * ny));
+            for (int dz = -1; dz <= 1; ++dz)
+                for (int dy = -1; dy <= 1; ++dy)
+                    for (int dx = -1; dx <= 1; ++dx) {
+                        const int xx = x + dx, yy = y + dy, zz = z + dz;
+                        if (xx < 0 || yy < 0 || zz < 0 || xx >= nx || yy >= ny || zz >= nz) continue;
+                        const i64 u = xx + (i64)nx * (yy + (i64)ny * zz);
+                        if (mask[u] && !labels[u]) { labels[u] = lab; stack[top++] = u; }
+                    }
+        }
+    }
+    free(stack);
+    return count;
 }

@@ -78,6 +78,8 @@ def _load():
             c_dbl_p, c_int_p, c_int_p, c_int_p, c_int_p, ctypes.c_double,
             c_int_p, c_int_p, c_dbl_p, c_dbl_p, c_dbl_p, c_u8_p]
         lib.pgsf_oracle_threshold_region.restype = ctypes.c_int
+        lib.pgsf_oracle_label26.argtypes = [c_u8_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_uint32)]
+        lib.pgsf_oracle_label26.restype = ctypes.c_int64
         _lib = lib
     return _lib
 
@@ -159,6 +161,17 @@ def filter_general(d: np.ndarray, f: np.ndarray) -> np.ndarray:
     _load().pgsf_oracle_filter_general(_p(d, ctypes.c_float), nx, ny, nz, _p(f, ctypes.c_double), rx, ry, rz,
                                        _p(out, ctypes.c_double))
     return out
+
+
+def label26(mask: np.ndarray):
+    """NEXT-4 (reading C-19): connected components of a mask [nz, ny, nx] under 26-connectivity by flood fill.
+    Returns (labels uint32 [nz, ny, nx], count); label = 1 + smallest linear index of the component, 0 = background."""
+    m = np.ascontiguousarray(mask, dtype=np.uint8)
+    assert m.ndim == 3
+    nz, ny, nx = m.shape
+    labels = np.empty(m.shape, dtype=np.uint32)
+    n = _load().pgsf_oracle_label26(_p(m, ctypes.c_uint8), nx, ny, nz, _p(labels, ctypes.c_uint32))
+    return labels, int(n)
 
 
 def _wfilter(fn, d, w, sigma3, mode, truncate):

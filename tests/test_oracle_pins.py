@@ -469,3 +469,92 @@ def test_G3_general_against_scipy_correlate(oracle):
     f2 = rng.standard_normal((29, 1, 3))
     ref2 = ndi.correlate(d.astype(np.float64), f2, mode="constant", cval=0.0)
     assert np.max(np.abs(oracle.filter_general(d, f2) - ref2)) <= 1e-13
+
+
+# ------------------------------------------------------------------------------------ NEXT-4: object labelling (C-19)
+
+def _mask(shape, voxels):
+    m = np.zeros(shape, np.uint8)
+    for z, y, x in voxels:
+        m[z, y, x] = 1
+    return m
+
+
+def test_L1_hand_built_masks(oracle):
+    """26-connectivity on masks whose components can be counted by eye; a wrong neighbourhood (6 or 18) or a wrong
+    axis stride fails one of them."""
+    sh = (5, 6, 7)
+    lin = lambda z, y, x: x + 7 * (y + 6 * z)
+    cases = [
+        ([], 0),
+        ([(0, 0, 0)], 1),
+        ([(1, 1, 1), (2, 2, 2)], 1),                       # corner contact only: one object (two under 6 / 18)
+        ([(1, 1, 1), (1, 2, 2)], 1),                       # edge contact only (two under 6-connectivity)
+        ([(1, 1, 1), (1, 1, 3)], 2),                       # a gap of one voxel along x
+        ([(0, 0, 6), (0, 1, 0)], 2),                       # end of one row / start of the next: adjacent in memory only
+        ([(0, 5, 3), (1, 0, 3)], 2),                       # last row of a plane / first row of the next plane
+        ([(0, 0, 0), (1, 1, 1), (2, 2, 2), (3, 3, 3), (4, 4, 4)], 1),          # a space diagonal
+        ([(2, y, x) for y in range(1, 5) for x in range(1, 6) if y in (1, 4) or x in (1, 5)], 1),      # a ring
+        ([(2, y, x) for y in range(1, 5) for x in range(1, 6) if y in (1, 4) or x in (1, 5)] + [(2, 2, 3)], 1),
+        ([(4, 5, 6), (0, 0, 0), (2, 3, 3)], 3),
+    ]
+    for vox, expect in cases:
+        m = _mask(sh, vox)
+        labels, n = oracle.label26(m)
+        assert n == expect, (vox, n)
+        assert np.array_equal(labels != 0, m != 0)
+        for z, y, x in vox:                                # label = 1 + smallest index of the voxel's component
+            comp = np.argwhere(labels == labels[z, y, x])
+            assert labels[z, y, x] == 1 + min(lin(*c) for c in comp)
+
+
+def test_L2_scipy_label_partition(oracle):
+    """Library cross-check: scipy.ndimage.label with the full 3 x 3 x 3 structure gives the same partition."""
+    ndi = pytest.importorskip("scipy.ndimage")
+    rng = np.random.default_rng(7)
+    for shape, dens in [((9, 11, 13), 0.08), ((16, 16, 16), 0.15), ((3, 40, 5), 0.3), ((1, 1, 50), 0.5)]:
+        m = (rng.random(shape) < dens).astype(np.uint8)
+        labels, n = oracle.label26(m)
+        ref, nref = ndi.label(m, structure=np.ones((3, 3, 3)))
+        assert n == nref
+        # same partition: the map oracle label -> scipy label is a bijection on the set voxels
+        pairs = set(zip(labels[m != 0].tolist(), ref[m != 0].tolist()))
+        assert len(pairs) == n and len({a for a, _ in pairs}) == n and len({b for _, b in pairs}) == n
+
+
+def test_L3_brute_force_closure(oracle):
+    """Definition level: components as the transitive closure of 'Chebyshev distance 1' on tiny masks."""
+    rng = np.random.default_rng(11)
+    for _ in range(20):
+        shape = tuple(rng.integers(1, 6, 3))
+        m = (rng.random(shape) < 0.35).astype(np.uint8)
+        pts = np.argwhere(m != 0)
+        comp = list(range(len(pts)))
+        changed = True
+        while changed:
+            changed = False
+            for i in range(len(pts)):
+                for j in range(len(pts)):
+                    if np.max(np.abs(pts[i] - pts[j])) <= 1 and comp[i] != comp[j]:
+                        comp[i] = comp[j] = min(comp[i], comp[j])
+                        changed = True
+        labels, n = oracle.label26(m)
+        assert n == len(set(comp))
+        for i in range(len(pts)):
+            for j in range(len(pts)):
+                same = labels[tuple(pts[i])] == labels[tuple(pts[j])]
+                assert same == (comp[i] == comp[j])
+
+
+def test_L4_invariances(oracle):
+    """The count is invariant under flips and axis permutations; a full cube is one object; an isolated-voxel lattice
+    of spacing 2 has as many objects as voxels."""
+    rng = np.random.default_rng(3)
+    m = (rng.random((10, 12, 14)) < 0.1).astype(np.uint8)
+    _, n = oracle.label26(m)
+    for t in (m[::-1], m[:, ::-1], m[:, :, ::-1], m.transpose(2, 0, 1), m.transpose(1, 2, 0)):
+        assert oracle.label26(np.ascontiguousarray(t))[1] == n
+    assert oracle.label26(np.ones((4, 5, 6), np.uint8))[1] == 1
+    lat = np.zeros((7, 7, 7), np.uint8)
+    lat[::2, ::2, ::2] = 1
+    assert oracle.label26(lat)[1] == 64
