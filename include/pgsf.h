@@ -231,6 +231,20 @@ PGSF_API pgsf_status pgsf_find_multiscale(pgsf_plan *plan, const float *d_in, fl
 PGSF_API pgsf_status pgsf_find_multiscale_host(pgsf_plan *plan, const float *h_in, float *const *h_filtered,
                                       uint8_t *h_mask, unsigned long long *h_count);
 
+/*
+ * pgsf_label_objects -- NEXT-4: the selected voxels merged into candidate OBJECTS.  The paper combines the voxels it
+ * selects into sources of "a single, parameterised catalogue" without defining the merge; reading C-19:
+ * an object is a connected component of the mask under 26-connectivity (voxels that touch by a face, an edge or a
+ * corner), every cube of the batch on its own.
+ * d_mask: the mask of pgsf_find_multiscale / pgsf_local_threshold (any non-zero byte = set), never written.
+ * d_labels: DEVICE, one uint32 per voxel (16-byte aligned, disjoint from d_mask): 0 for background, else
+ *   1 + the smallest linear index x + nx*(y + ny*z) (inside its cube) of the voxels of the component -- a unique
+ *   labelling.  d_count (nullable, 8-byte aligned): the number of objects of all cubes.
+ * INVALID_ARG for NULL / misaligned / overlapping buffers; UNSUPPORTED if one cube has more than 2^32 - 2 voxels.
+ */
+PGSF_API pgsf_status pgsf_label_objects(pgsf_plan *plan, const uint8_t *d_mask, uint32_t *d_labels,
+                               unsigned long long *d_count, void *cuda_stream);
+
 /* Number of kernels this library has launched on behalf of `plan` since creation (bench.py's
  * gpu_launches evidence). */
 PGSF_API unsigned long long pgsf_plan_launch_count(const pgsf_plan *plan);

@@ -31,7 +31,7 @@ _STATUS = {0: "PGSF_OK", 1: "PGSF_ERR_INVALID_ARG", 2: "PGSF_ERR_UNSUPPORTED", 3
 EXPORTS = ["pgsf_plan_create", "pgsf_plan_destroy", "pgsf_plan_set_option", "pgsf_plan_path",
            "pgsf_plan_workspace_bytes", "pgsf_last_error",
            "pgsf_plan_get_taps", "pgsf_filter3d", "pgsf_filter3d_weighted", "pgsf_filter3d_direct", "pgsf_local_threshold", "pgsf_find_multiscale",
-           "pgsf_find_multiscale_host", "pgsf_plan_launch_count", "pgsf_plan_set_profiling",
+           "pgsf_find_multiscale_host", "pgsf_label_objects", "pgsf_plan_launch_count", "pgsf_plan_set_profiling",
            "pgsf_plan_profile_collect", "pgsf_plan_profile_entry"]
 
 
@@ -81,6 +81,8 @@ def load_library() -> ctypes.CDLL:
         lib.pgsf_filter3d_weighted.restype = i
         lib.pgsf_filter3d_direct.argtypes = [vp, vp, i, i, i, vp, vp, ctypes.c_uint, vp]
         lib.pgsf_filter3d_direct.restype = i
+        lib.pgsf_label_objects.argtypes = [vp, vp, vp, vp, vp]
+        lib.pgsf_label_objects.restype = i
         lib.pgsf_local_threshold.argtypes = [vp, vp, vp, i, vp, vp, vp, vp, vp]
         lib.pgsf_local_threshold.restype = i
         lib.pgsf_find_multiscale.argtypes = [vp, vp, ctypes.POINTER(vp), vp, vp, vp, vp]
@@ -257,6 +259,17 @@ class Plan:
         self._check(self._lib.pgsf_filter3d_direct(self._h, _ptr(d_filter), rx, ry, rz, _ptr(d_in), _ptr(d_out),
                                                    PGSF_DIRECT_FP64_ACCUM if fp64_accum else 0, _stream_ptr(stream)))
         return d_out
+
+    def pgsf_label_objects(self, d_mask: torch.Tensor, d_labels: Optional[torch.Tensor] = None, stream=None):
+        """NEXT-4: connected components (26-connectivity) of the mask.  Returns (labels int32 tensor holding the uint32
+        labels, count tensor); label = 1 + smallest linear index of the component inside its cube, 0 = background."""
+        self._check_cube(d_mask, torch.uint8, "d_mask")
+        if d_labels is None:
+            d_labels = torch.empty(d_mask.shape, dtype=torch.int32, device=d_mask.device)
+        self._check_cube(d_labels, torch.int32, "d_labels")
+        cnt = torch.zeros(1, dtype=torch.int64, device=d_mask.device)
+        self._check(self._lib.pgsf_label_objects(self._h, _ptr(d_mask), _ptr(d_labels), _ptr(cnt), _stream_ptr(stream)))
+        return d_labels, cnt
 
     def pgsf_local_threshold(self, d_filtered: torch.Tensor, d_mask: Optional[torch.Tensor] = None,
                              or_into: bool = False, want_stats: bool = False, want_count: bool = True,

@@ -715,6 +715,31 @@ pgsf_status pgsf_find_multiscale(pgsf_plan *p, const float *d_in, float *const *
     return PGSF_OK;
 }
 
+pgsf_status pgsf_label_objects(pgsf_plan *p, const uint8_t *d_mask, uint32_t *d_labels, unsigned long long *d_count,
+                               void *stream)
+{
+    if (!p) return PGSF_ERR_INVALID_ARG;
+    if (!d_mask || !d_labels) return fail(p, PGSF_ERR_INVALID_ARG, "NULL mask or label pointer");
+    if (!aligned16(d_labels)) return fail(p, PGSF_ERR_INVALID_ARG, "d_labels must be 16-byte aligned");
+    if (d_count && (reinterpret_cast<uintptr_t>(d_count) & 7u))
+        return fail(p, PGSF_ERR_INVALID_ARG, "d_count must be 8-byte aligned");
+    if ((unsigned long long)p->dims.cube > 0xfffffffeULL)
+        return fail(p, PGSF_ERR_UNSUPPORTED, "a cube of more than 2^32 - 2 voxels cannot be labelled with 32-bit labels");
+    {
+        const size_t nvox = (size_t)p->dims.cube * p->desc.batch;
+        Range r[3] = {{"d_mask", d_mask, nvox}, {"d_labels", d_labels, nvox * sizeof(uint32_t)},
+                      {"d_count", d_count, sizeof(unsigned long long)}};
+        int a = 0, b = 0;
+        if (find_overlap(r, 3, &a, &b)) return fail(p, PGSF_ERR_INVALID_ARG, "%s overlaps %s", r[a].name, r[b].name);
+    }
+    if (p->dry) return fail(p, PGSF_ERR_CUDA, "PGSF_FLAG_DRY_RUN plan: arguments are valid, but no device is attached");
+    cudaError_t e = cudaSetDevice(p->device);
+    if (e != cudaSuccess) return cuda_fail(p, e, "cudaSetDevice");
+    e = pgsf::label_objects(p, d_mask, d_labels, d_count, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(p, e, "label launch");
+    return PGSF_OK;
+}
+
 pgsf_status pgsf_find_multiscale_host(pgsf_plan *p, const float *h_in, float *const *h_filtered,
                                       uint8_t *h_mask, unsigned long long *h_count)
 {

@@ -203,6 +203,9 @@ cudaError_t weighted_mul(pgsf_plan *p, const float *d, const float *w, float *pr
 cudaError_t weighted_boxsum(pgsf_plan *p, int scale, const float *w, float *a, float *b, cudaStream_t st);
 cudaError_t weighted_div(pgsf_plan *p, float *c, const float *den, cudaStream_t st);
 
+// ---- NEXT-4: connected components of the mask (pgsf_label.cu): the whole batch per call
+cudaError_t label_objects(pgsf_plan *p, const uint8_t *mask, unsigned *labels, unsigned long long *count, cudaStream_t st);
+
 // ---- Eq. 2 for an arbitrary filter array, direct summation (pgsf_direct.cu): one cube per call
 bool direct_supported(const pgsf_plan *p, int rx, int ry, int rz, int *smem_bytes);
 cudaError_t direct_filter3d(pgsf_plan *p, const float *filt, int rx, int ry, int rz, const float *in, float *out,

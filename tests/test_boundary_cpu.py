@@ -154,6 +154,22 @@ def test_statistics_kernel_and_tensor_flag_in_the_plan_path(lib):
         assert ok and "k_ymarch" in text, text
 
 
+def test_label_objects_validates_its_arguments(lib):
+    from paper_1507_04941_b200 import binding
+    with _dry(binding) as plan:
+        n = plan.voxels
+        base = 1 << 40
+        call = lambda m, l, c: lib.pgsf_label_objects(plan._h, ctypes.c_void_p(m), ctypes.c_void_p(l), ctypes.c_void_p(c), None)
+        assert call(base, base + (1 << 30), base + (1 << 31)) == binding.PGSF_ERR_CUDA     # valid, no device
+        assert call(0, base, 0) == binding.PGSF_ERR_INVALID_ARG
+        assert call(base, base + (1 << 30) + 4, 0) == binding.PGSF_ERR_INVALID_ARG          # misaligned labels
+        assert call(base, base + n - 16, 0) == binding.PGSF_ERR_INVALID_ARG                 # labels overlap the mask
+        assert "overlaps" in lib.pgsf_last_error(plan._h).decode()
+    with _dry(binding, dims=(2048, 2048, 1100)) as plan:                                    # > 2^32 - 2 voxels per cube
+        assert lib.pgsf_label_objects(plan._h, ctypes.c_void_p(1 << 40), ctypes.c_void_p(1 << 44), None, None) == \
+            binding.PGSF_ERR_UNSUPPORTED
+
+
 def test_plan_options_are_validated(lib):
     from paper_1507_04941_b200 import binding
     with _dry(binding, dims=(32, 32, 32), batch=5) as plan:

@@ -432,6 +432,39 @@ def test_host_entry_point_and_stream(pg, synth):
         assert plan.pgsf_plan_launch_count() > 0
 
 
+# ------------------------------------------------------------------------------------ NEXT-4: object labelling
+
+def test_label_objects(pg, synth, oracle):
+    """pgsf_label_objects against the flood-fill oracle, element by element (the labelling is unique: 1 + smallest
+    index of the component): random masks of several densities incl. percolating ones, a batch (cubes are labelled
+    separately), long thin shapes, and the OR mask of a real run."""
+    from dataclasses import replace
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    cases = [((40, 33, 52), 1, 0.02), ((40, 33, 52), 1, 0.12), ((64, 48, 30), 2, 0.3), ((1, 1, 300), 1, 0.5),
+             ((7, 260, 3), 3, 0.2), ((96, 96, 96), 1, 0.06)]
+    for dims, batch, dens in cases:
+        m = (torch.rand((batch, dims[2], dims[1], dims[0]), device="cuda", generator=gen) < dens).to(torch.uint8)
+        with pg.Plan(dims, [(1, 1, 2)], (4, 4, 8), 4.0, batch=batch) as plan:
+            labels, cnt = plan.pgsf_label_objects(m)
+            torch.cuda.synchronize()
+        total = 0
+        for b in range(batch):
+            ref, n = oracle.label26(m[b].cpu().numpy())
+            total += n
+            assert np.array_equal(labels[b].cpu().numpy().view(np.uint32), ref), (dims, dens, b)
+        assert int(cnt.item()) == total
+    w = replace(synth.scaled(synth.WORKLOADS[2], (120, 90, 160), n_sources=25), k=3.0)
+    d = synth.make_workload(w, "cuda")
+    with _plan(pg, w) as plan:
+        mask, count, _ = plan.pgsf_find_multiscale(d)
+        labels, nobj = plan.pgsf_label_objects(mask)
+        torch.cuda.synchronize()
+    ref, n = oracle.label26(mask[0].cpu().numpy())
+    assert np.array_equal(labels[0].cpu().numpy().view(np.uint32), ref) and int(nobj.item()) == n
+    assert 0 < n < int(count.item())          # objects, not voxels
+    print(f"label_objects: {int(count.item())} selected voxels -> {n} objects")
+
+
 # ------------------------------------------------------------------------------------ optional tensor-core z pass
 
 @pytest.mark.parametrize("dims,sigmas,box", [
