@@ -415,6 +415,25 @@ def measure_workload(w, dev, device_index, rank, world, steps, warmup, peaks, sm
                           "ms_local_threshold": round(times[1], 4),
                           "gvoxel_per_s": n_vox * world / (t_sum * 1e-3) / 1e9})
     out["per_scale"] = per_scale
+
+    # ---- NEXT-4: the mask of the last step merged into objects (26-connected components), timed on its own
+    try:
+        labels = torch.empty(d.shape, dtype=torch.int32, device=dev)
+        best = None
+        for rep in range(3):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            _, nobj = plan.pgsf_label_objects(mask, d_labels=labels, stream=stream)
+            b.record(stream)
+            torch.cuda.synchronize()
+            if rep:
+                t = a.elapsed_time(b)
+                best = t if best is None else min(best, t)
+        out["label_objects"] = {"ms": round(best, 4), "objects": int(nobj.item()), "set_voxels": count,
+                                "what": "pgsf_label_objects on the step's OR mask (not part of the timed step)"}
+        del labels
+    except Exception as exc:                      # (an extra leg must never cost the headline line)
+        out["label_objects"] = {"error": str(exc)}
     return out, ctx
 
 
@@ -455,7 +474,7 @@ def run_b200(args, w):
                    "kernel_path": ctx["plan"].pgsf_plan_path()[1],
                    "parallelism": "replicas only (no collective)"},
         "clocks": res["clocks"], "gpu_launches": res["launches"], "roofline": res["roofline"],
-        "path_roofline": res["path_roofline"], "kernels": res["kernels"], "per_scale": res["per_scale"],
+        "path_roofline": res["path_roofline"], "kernels": res["kernels"], "per_scale": res["per_scale"], "label_objects": res.get("label_objects"),
     }
     ctx["peaks"], ctx["sm_count"], ctx["local_rank"] = peaks, props.multi_processor_count, local_rank
     return line, ctx
