@@ -282,6 +282,220 @@ __global__ void __launch_bounds__(TC_NT) k_ztc(float *out, float *__restrict__ Z
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 32;" ::"r"(tmem) : "memory");
 }
 
+// ------------------------------------------------------------------------------------ k_ztc2
+// The same GEMM with 64 columns per CTA and two warp groups, for the radii whose operands fit one CTA per SM
+// (RZ <= 72).  Group B (warps 4-7) waits for the slab of step k, splits it and issues its MMAs; group A (warps 0-3:
+// one thread per (column, quantity)) meanwhile walks the window sums of step k-1; all eight warps then drain the
+// accumulator (warp w: TMEM lanes 32 (w & 3).., columns 32 (w >> 2)..) and stage the leaving slab.
+constexpr int T2_XT = 64, T2_NT = 256;
+constexpr unsigned kIdescTf32N64 = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 16) | ((T2_XT >> 3) << 17) | ((TC_ZB >> 4) << 24);
+
+__device__ __forceinline__ void umma_tf32_n64(unsigned d_tmem, unsigned long long adesc, unsigned long long bdesc, unsigned accumulate)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(kIdescTf32N64), "r"(accumulate) : "memory");
+}
+
+__global__ void __launch_bounds__(T2_NT, 1) k_ztc2(float *out, float *__restrict__ Z1, float *__restrict__ Z2,
+                                                   const float *__restrict__ pivot, const float *__restrict__ strips,
+                                                   float *__restrict__ state, const __grid_constant__ CUtensorMap tmap,
+                                                   const ZtcParams p)
+{
+    extern __shared__ __align__(1024) unsigned char ztc_smem[];
+    __shared__ unsigned long long bar_tma, bar_mma;
+    __shared__ unsigned tmem_slot;
+    const int K = p.K, T = K / 4 + 30;
+    float *Bh = reinterpret_cast<float *>(ztc_smem);      // [2 column atoms][K][32], hi part (32-byte-atom swizzle)
+    float *Bl = Bh + 2 * K * 32;                          // lo part
+    float *fs = Bl + 2 * K * 32;                          // [128][64] f of a step, 16-byte chunks XOR-ed with (row & 7)
+    float *ts = fs + TC_ZB * T2_XT;                       // [128][64] f of the channels leaving the window
+    float *Ah = ts + TC_ZB * T2_XT;
+    float *Al = Ah + T * 32;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const bool grpB = warp >= 4;
+    const Dims &d = p.d;
+    const int x0 = blockIdx.x * T2_XT, y = blockIdx.y, nz = d.nz, hz = p.hz;
+    const long long cube_off = (long long)blockIdx.z * d.cube;
+    out += cube_off; Z1 += cube_off; Z2 += cube_off;
+    const float c0 = __ldg(pivot);
+
+    if (tid == 0) { mbar_init(&bar_tma, 1); mbar_init(&bar_mma, 1); tma_prefetch_desc(&tmap); }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 64;" ::"r"(smem_u32(&tmem_slot)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    for (int i = tid; i < 2 * T * 32; i += T2_NT) Ah[i] = __ldg(strips + i);
+    fence_proxy_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const unsigned tmem = tmem_slot;
+    const unsigned ah_addr = smem_u32(Ah), al_addr = smem_u32(Al), bh_addr = smem_u32(Bh), bl_addr = smem_u32(Bl);
+
+    // group A: one thread per (column, quantity)
+    const int c = tid & 63;
+    const bool sq = tid >= 64;
+    const bool c_ok = !grpB && x0 + c < d.nx;
+    const long long cb = (long long)y * d.nx + x0 + c;
+    float *Zq = sq ? Z2 : Z1;
+    float s = 0.f, e = 0.f;
+    float *st_s = nullptr;
+    if (state != nullptr && c_ok) {
+        st_s = state + ((long long)(sq ? 2 : 0) * d.plane + cb);
+        if (p.kbeg > 0) { s = st_s[0]; e = st_s[d.plane]; }
+    }
+    unsigned ph_tma = 0, ph_mma = 0;
+    const float *row_out = out + (long long)y * d.nx + x0;
+
+    auto issue_tma = [&](int z0) {        // (called by warp 4)
+        if (lane == 0) {
+            fence_proxy_async_smem();
+            mbar_arrive_expect_tx(&bar_tma, K * T2_XT * 4);
+            const int bz = K / p.nbox;
+            for (int a = 0; a < 2; ++a)
+                for (int b = 0; b < p.nbox; ++b)
+                    tma_load_4d(Bh + a * K * 32 + b * bz * 32, &tmap, x0 + 32 * a, y, z0 - p.rz + b * bz - p.zmap_lo,
+                                blockIdx.z, &bar_tma);
+        }
+        __syncwarp();
+    };
+    auto acc_add = [&](float v) {
+        const float t = s + v, bp = t - s;
+        e += (s - (t - bp)) + (v - bp);
+        s = t;
+    };
+    auto fidx = [&](int j, int cc) { return j * T2_XT + (((((cc >> 2) & 7) ^ (j & 7)) | ((cc >> 2) & 8)) << 2 | (cc & 3)); };
+    auto window = [&](int z0) {
+        if (!c_ok) return;
+        if (z0 >= 2 * hz && z0 + TC_ZB <= nz && (hz & 3) == 0) {
+            const int jsplit = min(2 * hz, TC_ZB);     // (a multiple of 8) leaving channel: ts[j] below it, fs[j - 2 hz] from it on
+            float *zp = Zq + (long long)(z0 - hz) * d.plane + cb;
+            float pb = 0.f;
+            int off[8];                                // column offset inside a row for (row & 7) = 0 .. 7
+#pragma unroll
+            for (int r = 0; r < 8; ++r) off[r] = ((((c >> 2) & 7) ^ r) | ((c >> 2) & 8)) << 2 | (c & 3);
+            for (int jb = 0; jb < jsplit; jb += 8) {
+#pragma unroll
+                for (int r = 0; r < 8; ++r) {
+                    const int j = jb + r;
+                    const float a = fs[j * T2_XT + off[r]] - c0, b = ts[j * T2_XT + c] - c0;
+                    acc_add((sq ? a * a : a) - pb);
+                    pb = sq ? b * b : b;
+                    *zp = s + e;
+                    zp += d.plane;
+                }
+            }
+            for (int jb = jsplit; jb < TC_ZB; jb += 8) {
+#pragma unroll
+                for (int r = 0; r < 8; ++r) {
+                    const int j = jb + r;              // (j - 2 hz) & 7 == r as well
+                    const float a = fs[j * T2_XT + off[r]] - c0, b = fs[(j - 2 * hz) * T2_XT + off[r]] - c0;
+                    acc_add((sq ? a * a : a) - pb);
+                    pb = sq ? b * b : b;
+                    *zp = s + e;
+                    zp += d.plane;
+                }
+            }
+            acc_add(-pb);
+        } else {
+            for (int j = 0; j < TC_ZB; ++j) {
+                const int zl = z0 + j, zo = zl - hz;
+                if (zl < nz) {
+                    const float a = fs[fidx(j, c)] - c0;
+                    acc_add(sq ? a * a : a);
+                }
+                if (zo >= 0 && zo < nz) {
+                    Zq[(long long)zo * d.plane + cb] = s + e;
+                    const int jt = j - 2 * hz;
+                    if (zo - hz >= 0) {
+                        const float b = (jt >= 0 ? fs[fidx(jt, c)] : ts[j * T2_XT + c]) - c0;
+                        acc_add(sq ? -(b * b) : -b);
+                    }
+                }
+            }
+        }
+    };
+
+    bool pending = false;
+    int pending_z0 = 0;
+    if (warp == 4 && p.kbeg < p.kend && p.kbeg * TC_ZB < nz) issue_tma(p.kbeg * TC_ZB);
+    for (int k = p.kbeg; k < p.kend; ++k) {
+        const int z0 = k * TC_ZB;
+        const bool have = z0 < nz;
+        if (grpB) {
+            if (have) {
+                mbar_wait(&bar_tma, ph_tma);
+                ph_tma ^= 1;
+                float4 *bh4 = reinterpret_cast<float4 *>(Bh), *bl4 = reinterpret_cast<float4 *>(Bl);
+                for (int i = tid - 128; i < K * 16; i += 128) {
+                    const float4 v = bh4[i];
+                    float4 h, l;
+                    h.x = rna_tf32(v.x); h.y = rna_tf32(v.y); h.z = rna_tf32(v.z); h.w = rna_tf32(v.w);
+                    l.x = rna_tf32(v.x - h.x); l.y = rna_tf32(v.y - h.y); l.z = rna_tf32(v.z - h.z); l.w = rna_tf32(v.w - h.w);
+                    bh4[i] = h;
+                    bl4[i] = l;
+                }
+                fence_proxy_async_smem();
+                tc_fence_before();
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                if (warp == 4) {
+                    if (lane == 0) {
+                        tc_fence_after();
+                        // A: Hankel strip (K-major, LBO 128 B, SBO 256 B).  B: two column atoms K x 128 bytes apart (LBO), 4-channel
+                        // atoms 512 B apart (SBO), 1 KB per K step.
+                        unsigned long long ah = umma_desc(ah_addr, 128, 256, 0), al = umma_desc(al_addr, 128, 256, 0);
+                        unsigned long long bh = umma_desc(bh_addr, K * 128, 512, 1), bl = umma_desc(bl_addr, K * 128, 512, 1);
+                        for (int ks = 0; ks < K / 8; ++ks) {
+                            umma_tf32_n64(tmem, ah, bh, ks > 0);
+                            umma_tf32_n64(tmem, al, bh, 1);
+                            umma_tf32_n64(tmem, ah, bl, 1);
+                            ah += 16; al += 16; bh += 64; bl += 64;
+                        }
+                        umma_commit(&bar_mma);
+                    }
+                    __syncwarp();
+                }
+            }
+        } else if (pending) {
+            window(pending_z0);
+        }
+        __syncthreads();                  // the window walk is done with the f and leaving slabs; the MMAs are in flight
+        for (int i = tid; i < TC_ZB * 16; i += T2_NT) {
+            const int j = i >> 4, ch = i & 15, zt = z0 - 2 * hz + j;
+            const bool ok = zt >= 0 && zt < z0 && zt < nz && x0 + 4 * ch < d.nx;
+            cp_async16(ts + j * T2_XT + 4 * ch, ok ? row_out + (long long)zt * d.plane + 4 * ch : out, ok);
+        }
+        if (have) {
+            mbar_wait(&bar_mma, ph_mma);
+            ph_mma ^= 1;
+            tc_fence_after();
+            if (warp == 4 && k + 1 < p.kend && (k + 1) * TC_ZB < nz) issue_tma((k + 1) * TC_ZB);
+            float v[32];
+            const int quarter = warp & 3, half = warp >> 2;
+            tmem_ld32(tmem + ((unsigned)(quarter * 32) << 16) + (unsigned)(half * 32), v);
+            const int j = TC_ZB - 1 - (quarter * 32 + lane), gz = z0 + j;
+            float *g = out + (long long)gz * d.plane + (long long)y * d.nx + x0 + 32 * half;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const float4 w = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+                *reinterpret_cast<float4 *>(fs + j * T2_XT + ((half * 8 + (q ^ (j & 7))) << 2)) = w;
+                if (gz < nz && x0 + 32 * half + 4 * q < d.nx) *reinterpret_cast<float4 *>(g + 4 * q) = w;
+            }
+            tc_fence_before();
+        }
+        cp_async_wait_all();
+        __syncthreads();                  // f slab and leaving slab of step k complete; the accumulator has been read
+        pending = true;
+        pending_z0 = z0;
+    }
+    if (!grpB && pending) window(pending_z0);
+    if (st_s != nullptr) { st_s[0] = s; st_s[d.plane] = e; }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 64;" ::"r"(tmem) : "memory");
+}
+
 }  // namespace
 
 // host: round to the nearest TF32 (ties away from zero, as cvt.rna.tf32.f32)
@@ -363,6 +577,17 @@ cudaError_t fast_ztc(pgsf_plan *p, int scale, const float *in, float *out, float
     }
     if (!ok) return cudaErrorNotSupported;
     const int T = zp.K / 4 + 30;
+    const int smem2 = (2 * zp.K * T2_XT + 2 * TC_ZB * T2_XT + 2 * T * 32) * (int)sizeof(float);
+    if (smem2 <= 227 * 1024 && !(p->tune & 32)) {          // 64 columns per CTA, two warp groups (PGSF_OPT_TUNE bit 5: k_ztc)
+        cudaError_t e2 = ensure_dynamic_smem(k_ztc2, smem2);
+        if (e2 != cudaSuccess) return e2;
+        char name2[32];
+        snprintf(name2, sizeof name2, "ztc_s%d", scale);
+        LaunchScope ls2(p, name2, st);
+        dim3 grid2((d.nx + T2_XT - 1) / T2_XT, d.ny, ncubes);
+        k_ztc2<<<grid2, T2_NT, smem2, st>>>(out, Z1, Z2, p->d_pivot, p->d_tc_strips[scale], state, map, zp);
+        return cudaGetLastError();
+    }
     const int smem = (2 * zp.K * TC_XT + 2 * TC_ZB * TC_XT + 2 * T * 32) * (int)sizeof(float);
     cudaError_t e = ensure_dynamic_smem(k_ztc, smem);
     if (e != cudaSuccess) return e;
