@@ -497,6 +497,25 @@ def test_tensor_core_z_pass(pg, synth, oracle, dims, sigmas, box):
     assert hcount == int(c_tc.item()) and torch.equal(h_mask, m_tc.cpu())
 
 
+def test_tensor_core_z_pass_batch(pg, synth, oracle):
+    """The variant on a batch with halo (several cubes per launch: the TMA map has a cube dimension, out-of-cube
+    channels of one cube must be zeros, not the neighbour cube's planes) and with PGSF_OPT_TUNE bit 5 (the 32-column
+    kernel for every radius)."""
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[4], (96, 40, 140), batch=3, n_sources=6), sigmas=((1, 1, 8), (2, 2, 16)),
+                halo=(8, 8, 20), k=3.0)
+    d = synth.make_workload(w, "cuda")
+    rep, count = _full_compare(pg, oracle, w, d, pg.PGSF_FLAG_TENSOR_ZPASS, check_stats=False)
+    with _plan(pg, w, pg.PGSF_FLAG_TENSOR_ZPASS) as plan:
+        m2, c2, f2 = plan.pgsf_find_multiscale(d, keep_filtered=True)
+        plan.pgsf_plan_set_option(pg.PGSF_OPT_TUNE, 32)
+        m1, c1, f1 = plan.pgsf_find_multiscale(d, keep_filtered=True)
+        torch.cuda.synchronize()
+    assert count > 0 and int(c2.item()) == count
+    assert max(float((a - b).abs().max()) for a, b in zip(f1, f2)) <= 1e-6     # same products, another summation tree
+    assert int((m1 != m2).sum()) <= rep.band_voxels + 2
+
+
 # ------------------------------------------------------------------------------------ streamed host entry point (NEXT-3)
 
 def _host_run(pg, w, d_host, section=None, budget=None, keep=False, flags=0):
