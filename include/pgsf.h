@@ -112,9 +112,10 @@ PGSF_API pgsf_status pgsf_plan_destroy(pgsf_plan *plan);
  *   PGSF_OPT_HOST_DEVICE_BUDGET   pgsf_find_multiscale_host: bytes of device memory its staging may use;
  *                                 0 = 80 % of the memory free at the first call.
  *   PGSF_OPT_TUNE                 measurement aid, a bit set: 1 = statistics kernel without L2 eviction hints,
- *                                 2 = the previous statistics kernel (k_ymarch) instead of k_xyb,
+ *                                 2 = the previous statistics kernel (k_ymarch) instead of k_xyb (where it exists),
  *                                 4 = cp.async staging of every z-pass slab, 8 = TMA bulk tensor copies for every
- *                                 z-pass slab (default: TMA up to a compiled radius of 24, cp.async above).
+ *                                 z-pass slab (default: TMA up to a compiled radius of 24, cp.async above),
+ *                                 32 = the 32-column form of the tensor-core z pass (k_ztc) for every radius.
  * INVALID_ARG for an unknown option or a value outside its range.
  */
 #define PGSF_OPT_GROUP_CUBES 1
@@ -124,6 +125,9 @@ PGSF_API pgsf_status pgsf_plan_destroy(pgsf_plan *plan);
 PGSF_API pgsf_status pgsf_plan_set_option(pgsf_plan *plan, int option, long long value);
 
 /*
+ * The tiled sm_100a kernels take: nx a multiple of 4; x / y radii <= 12 and z radii <= 96 (every scale); statistics
+ * box half-width hx in {4, 8, 12, 16} (any hy, hz); ny, nz <= 65535.  Anything else runs the generic kernels.
+ *
  * pgsf_plan_path -- which kernels this plan runs, as text ("filter: tiled ...; stats: generic (hx = 5 ...)"),
  * so that a caller can see a shape / radius / box that falls off the tiled sm_100a kernels onto the
  * one-thread-per-voxel generic ones (several times slower, same results).  Writes at most cap bytes (NUL
