@@ -2,7 +2,7 @@
 // sums", P:33 / P:282 thresholds; readings C-6..C-10), the successor of k_ymarch (pgsf_stats.cu).
 //
 // Input: the z-direction window sums Z1 = sum f, Z2 = sum f^2 (of k_zm / k_zbox) and the filtered cube f.
-// One CTA = one z plane, 256 staged columns (1, 2 or 4 strips of 32 G columns, G = hx / 2), one chunk of
+// One CTA = 256 staged columns (1, 2 or 4 strips of 32 G columns, G = hx / 2, each of some z plane), one chunk of
 // rows; it marches down y in batches of RB rows.  Every batch has two phases:
 //
 //   y phase   a thread owns ONE PAIR of adjacent columns and keeps the y-direction window sums
@@ -62,6 +62,7 @@ struct XybParams {
     float k2;            // k^2
     int wo;              // output columns per strip (multiple of 8, <= WMAX)
     int nstrips;         // strips across nx
+    long long nplanes;   // planes of the launch (all cubes)
     int ychunk;          // output rows per CTA
 };
 
@@ -147,9 +148,8 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
     __shared__ unsigned wsum[4];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nx = p.d.nx, ny = p.d.ny;
-    const int zz = blockIdx.z;                         // plane of the stack of cubes
-    const int z = zz % p.d.nz + p.z_off;               // channel inside its cube
-    const long long plane_off = (long long)zz * p.d.plane;
+    // A CTA takes NSTRIP consecutive SLOTS; slot = (plane of the stack of cubes) * nstrips + (x strip): with several
+    // strips per CTA (G < 8) the strips of a CTA may belong to different planes, so narrow cubes leave no slot idle.
     const int ya = blockIdx.y * p.ychunk, yb = min(ya + p.ychunk, ny);
     const int hy = p.hy;
     const float piv = __ldg(pivot);                    // Z1, Z2 are sums of f - c0 and (f - c0)^2 (D-2)
@@ -158,9 +158,11 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
     //      r - 2 hy.  Interior batches (every such row inside the cube and inside this chunk's window history) read
     //      through four running pointers with no predicate; threads of columns outside the cube run the same code
     //      on a buffer of zeros with stride 0.
-    const int ystrip = blockIdx.x * NSTRIP + tid / TPS;
+    const long long yslot = (long long)blockIdx.x * NSTRIP + tid / TPS;
+    const int ystrip = (int)(yslot % p.nstrips);
+    const long long yplane = yslot / p.nstrips;
     const int cy = ystrip * p.wo - HX + 2 * (tid % TPS);
-    const bool ycol_ok = tid / TPS < NSTRIP && ystrip < p.nstrips && cy >= 0 && cy + 2 <= nx;
+    const bool ycol_ok = tid / TPS < NSTRIP && yplane < p.nplanes && cy >= 0 && cy + 2 <= nx;
     const int r0 = ya - hy;                            // first row entering the window of output row ya
     const int nrows = (yb - ya) + 2 * hy;              // entering rows r0 .. yb - 1 + hy
     const int nb = (nrows + RB - 1) / RB;
@@ -171,7 +173,7 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
     const unsigned rstride = ycol_ok ? (unsigned)nx * 4u : 0u;     // bytes between rows
     const char *pe1, *pe2, *pl1, *pl2;                             // row 0 of the current batch: entering, leaving
     {
-        const long long o = plane_off + (ycol_ok ? cy : 0);
+        const long long o = (ycol_ok ? yplane : 0) * p.d.plane + (ycol_ok ? cy : 0);
         pe1 = reinterpret_cast<const char *>(ycol_ok ? Z1 + o : zeros);
         pe2 = reinterpret_cast<const char *>(ycol_ok ? Z2 + o : zeros);
         const long long oe = ycol_ok ? (long long)r0 * nx * 4 : 0, ol = ycol_ok ? (long long)(r0 - 2 * hy) * nx * 4 : 0;
@@ -213,13 +215,18 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
     long long voff[UPW];                               // element offset of (xo, row of the current batch's unit)
     int nvq[UPW];                                      // load / store words of the group that lie inside the cube
     {
-        const float nzc = (float)xyb_clipped_len(z, p.hz, p.nz_full);
-        const bool core_z = z >= p.gz && z < p.nz_full - p.gz;
 #pragma unroll
         for (int u = 0; u < UPW; ++u) {
-            const int unit = warp + 4 * u, strip = blockIdx.x * NSTRIP + unit / RB;
+            const int unit = warp + 4 * u;
+            const long long slot = (long long)blockIdx.x * NSTRIP + unit / RB;
+            const int strip = (int)(slot % p.nstrips);
+            const long long zz = slot / p.nstrips;                 // plane of the stack of cubes
+            const int z = (int)(zz % p.d.nz) + p.z_off;            // channel inside its cube
+            const long long plane_off = (zz < p.nplanes ? zz : 0) * p.d.plane;
+            const float nzc = (float)xyb_clipped_len(z, p.hz, p.nz_full);
+            const bool core_z = z >= p.gz && z < p.nz_full - p.gz;
             const int xo = strip * p.wo + G * lane;
-            out_ok[u] = strip < p.nstrips && G * lane < p.wo && xo < nx;
+            out_ok[u] = zz < p.nplanes && G * lane < p.wo && xo < nx;
             nvq[u] = min(NV, max(0, (nx - xo) / VL));          // (the last group of a row may stick out of the cube)
             core_x[u] = 0;
 #pragma unroll
@@ -441,7 +448,8 @@ cudaError_t launch_xyb(const pgsf_plan *pl, const float *f, const float *Z1, con
     if (p.wo > S::WMAX) p.wo = S::WMAX;
     ns = (d.nx + p.wo - 1) / p.wo;
     p.nstrips = ns;
-    const int gx = (ns + S::NSTRIP - 1) / S::NSTRIP;
+    p.nplanes = (long long)d.nz * ncubes;
+    const long long gxl = ((long long)ns * p.nplanes + S::NSTRIP - 1) / S::NSTRIP;
     // y chunks: a function of ny alone -- the running sums of a chunk start afresh, so the rounding of a voxel's
     // statistics must not depend on how many planes a launch happens to hold (a streamed cube is launched section
     // by section and must reproduce the resident call bit for bit).  A chunk start re-reads 2 hy rows.
@@ -449,8 +457,8 @@ cudaError_t launch_xyb(const pgsf_plan *pl, const float *f, const float *Z1, con
     if (nch < 1) nch = 1;
     p.ychunk = (d.ny + nch - 1) / nch;
     nch = (d.ny + p.ychunk - 1) / p.ychunk;
-    if ((long long)d.nz * ncubes > 65535 || nch > 65535) return cudaErrorInvalidConfiguration;
-    dim3 grid(gx, nch, d.nz * ncubes);
+    if (gxl > 0x7fffffffLL || nch > 65535) return cudaErrorInvalidConfiguration;
+    dim3 grid((unsigned)gxl, nch, 1);
     const float *zeros = pl->d_pivot + 16;            // (the plan's constant block: 256 bytes, zero beyond the pivot)
     switch (p.mode) {
     case 0: return launch_xyb_m<G, 0>(f, Z1, Z2, mask, mean, sd, count, p, grid, pl->d_pivot, zeros, st);
