@@ -51,14 +51,23 @@ namespace {
 // Both passes are pure FFMA2 streams with uniform-register taps; no y halo is recomputed and the
 // only shared-memory traffic is the x pass' operand reads.
 
-constexpr int XM_NT = 256;          // threads = columns per CTA
-constexpr int XM_NB = 8;            // row pairs per batch (= warps)
 constexpr int XM_HALO = 16;         // staged columns either side (>= largest x radius, multiple of 4)
-constexpr int XM_SW = XM_NT + 2 * XM_HALO;
-constexpr int XM_GP = 10;           // pitch in pairs of an 8-column group (spreads the banks)
-constexpr int XM_SIN = (XM_SW / 8) * XM_GP;   // pairs of one staged row pair
-constexpr int XM_U = (XM_NT / 8) * XM_GP;     // pairs of one x-filtered row pair
 constexpr int XM_MAXS = 4;
+// GS = columns per lane of the x pass: 8 (256-column strips, 8 warps) or 4 (128-column strips, 4 warps: cubes whose nx
+// would leave most of a second 256-column strip idle, e.g. nx = 320)
+template <int GS>
+struct XmShape {
+    static constexpr int NT = 32 * GS;          // threads = columns per CTA
+    static constexpr int NB = GS;               // row pairs per batch (= warps)
+    static constexpr int SW = NT + 2 * XM_HALO;
+    static constexpr int GP = GS == 8 ? 10 : 6; // pitch in pairs of a GS-column group (even; spreads the banks)
+    static constexpr int SIN = (SW / GS) * GP;  // pairs of one staged row pair
+    static constexpr int U = (NT / GS) * GP;    // pairs of one x-filtered row pair
+    static constexpr int NQ = (SW / 4 + 31) / 32;   // float4 loads per lane and staged row
+};
+
+// 128-column strips where they stage fewer columns than 256-column ones (nx = 320: 3 x 128 against 2 x 256)
+inline int xm_strip_width(int nx) { return (nx + 127) / 128 * 128 < (nx + 255) / 256 * 256 ? 128 : 256; }
 
 struct XymParams {
     Dims d;
@@ -79,26 +88,27 @@ __device__ __forceinline__ float2 fmul2(float2 a, float g)
 }
 
 // x pass of one scale for the warp's staged row pair: lane -> columns 8 lane .. 8 lane + 7
-template <int R>
+template <int R, int GS>
 __device__ __forceinline__ void xm_xpass(const float2 *__restrict__ s_in, float2 *__restrict__ s_u,
                                          const float (&gx)[32], int lane)
 {
+    constexpr int XM_GP = XmShape<GS>::GP;
     constexpr int C0 = XM_HALO - R;     // staged column of tap -R of output column 0
     constexpr int SH = C0 & 1;          // 16-byte loads start at an even staged column
-    constexpr int NL = (8 + 2 * R + SH + 1) / 2;
-    float2 acc[8];
+    constexpr int NL = (GS + 2 * R + SH + 1) / 2;
+    float2 acc[GS];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) acc[i] = make_float2(0.f, 0.f);
+    for (int i = 0; i < GS; ++i) acc[i] = make_float2(0.f, 0.f);
 #pragma unroll
     for (int l = 0; l < NL; ++l) {
         const int sc = C0 - SH + 2 * l;                 // relative to 8 lane; compile time
-        const float4 q = *reinterpret_cast<const float4 *>(s_in + (lane + (sc >> 3)) * XM_GP + (sc & 7));
+        const float4 q = *reinterpret_cast<const float4 *>(s_in + (lane + sc / GS) * XM_GP + sc % GS);
         const float2 v[2] = {make_float2(q.x, q.y), make_float2(q.z, q.w)};
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
             const int j = 2 * l + e - SH;               // input index relative to tap -R of output 0
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
+            for (int i = 0; i < GS; ++i) {
                 const int o = j - i;
                 if (j >= 0 && o >= 0 && o <= 2 * R) acc[i] = ffma2(v[e], gx[o], acc[i]);
             }
@@ -106,7 +116,7 @@ __device__ __forceinline__ void xm_xpass(const float2 *__restrict__ s_in, float2
     }
     float4 *dst = reinterpret_cast<float4 *>(s_u + lane * XM_GP);
 #pragma unroll
-    for (int i = 0; i < 4; ++i) dst[i] = make_float4(acc[2 * i].x, acc[2 * i].y, acc[2 * i + 1].x, acc[2 * i + 1].y);
+    for (int i = 0; i < GS / 2; ++i) dst[i] = make_float4(acc[2 * i].x, acc[2 * i].y, acc[2 * i + 1].x, acc[2 * i + 1].y);
 }
 
 // y pass state of one scale and one column: B[j] = unfinished output pair m = k + dmin + j
@@ -147,9 +157,11 @@ struct XmY {
     }
 };
 
-template <int NS, int RA, int RB, int RC, int RD, bool WGT = false>
-__global__ void __launch_bounds__(XM_NT, 2) k_xym(const float *__restrict__ in, const __grid_constant__ XymParams P)
+template <int NS, int RA, int RB, int RC, int RD, bool WGT = false, int GS = 8>
+__global__ void __launch_bounds__(XmShape<GS>::NT, GS == 8 ? 2 : 4) k_xym(const float *__restrict__ in, const __grid_constant__ XymParams P)
 {
+    using XS = XmShape<GS>;
+    constexpr int XM_NT = XS::NT, XM_NB = XS::NB, XM_SW = XS::SW, XM_GP = XS::GP, XM_SIN = XS::SIN, XM_U = XS::U;
     extern __shared__ __align__(16) float2 xm_smem[];
     float2 *s_in = xm_smem;                        // [8 warps][XM_SIN]
     float2 *s_u = xm_smem + XM_NB * XM_SIN;        // [8 row pairs][NS][XM_U]
@@ -158,7 +170,7 @@ __global__ void __launch_bounds__(XM_NT, 2) k_xym(const float *__restrict__ in, 
     const int x0 = blockIdx.x * XM_NT, z = blockIdx.z;
     const int ya = blockIdx.y * P.ychunk, yb = min(ya + P.ychunk, d.ny);
     const int ys = ya - 16;                        // first input row of the first batch (even)
-    const int nbatch = (yb + 12 - ys + 15) / 16;
+    const int nbatch = (yb + 12 - ys + 2 * XM_NB - 1) / (2 * XM_NB);
     const long long plane_off = (long long)z * d.plane;
     const int gx = x0 + tid;
     const bool col_ok = gx < d.nx;
@@ -175,16 +187,16 @@ __global__ void __launch_bounds__(XM_NT, 2) k_xym(const float *__restrict__ in, 
     XmY<RA> sa; XmY<RB> sb; XmY<RC> sc; XmY<RD> sd;
     sa.init(); sb.init(); sc.init(); sd.init();
 
-    // this warp's row pair of batch b: rows ys + 16 b + 2 w (+1); lane loads float4 columns lane, lane+32, lane+64
-    float4 pf[2][3];
+    // this warp's row pair of batch b: rows ys + 2 NB b + 2 w (+1); lane loads float4 columns lane, lane+32, ...
+    float4 pf[2][XS::NQ];
     auto prefetch = [&](int b) {
-        const int r0 = ys + 16 * b + 2 * w;
+        const int r0 = ys + 2 * XM_NB * b + 2 * w;
 #pragma unroll
         for (int rr = 0; rr < 2; ++rr) {
             const int r = r0 + rr;
             const bool rok = r >= 0 && r < d.ny;
 #pragma unroll
-            for (int q = 0; q < 3; ++q) {
+            for (int q = 0; q < XS::NQ; ++q) {
                 const int idx = lane + 32 * q;
                 const int xx = x0 - XM_HALO + 4 * idx;
                 const bool ok = rok && idx < XM_SW / 4 && xx >= 0 && xx < d.nx;
@@ -203,10 +215,11 @@ __global__ void __launch_bounds__(XM_NT, 2) k_xym(const float *__restrict__ in, 
         {
             float2 *sw = s_in + w * XM_SIN;
 #pragma unroll
-            for (int q = 0; q < 3; ++q) {
+            for (int q = 0; q < XS::NQ; ++q) {
                 const int idx = lane + 32 * q;
                 if (idx < XM_SW / 4) {
-                    float4 *dst = reinterpret_cast<float4 *>(sw + (idx >> 1) * XM_GP + (idx & 1) * 4);
+                    float4 *dst = GS == 8 ? reinterpret_cast<float4 *>(sw + (idx >> 1) * XM_GP + (idx & 1) * 4)
+                                          : reinterpret_cast<float4 *>(sw + idx * XM_GP);
                     const float4 a = pf[0][q], c = pf[1][q];
                     dst[0] = make_float4(a.x, c.x, a.y, c.y);
                     dst[1] = make_float4(a.z, c.z, a.w, c.w);
@@ -214,16 +227,16 @@ __global__ void __launch_bounds__(XM_NT, 2) k_xym(const float *__restrict__ in, 
             }
             __syncwarp();
             float2 *su = s_u + (w * NS) * XM_U;
-            xm_xpass<RA>(sw, su, P.t[0].gx, lane);
-            if constexpr (NS > 1) xm_xpass<RB>(sw, su + XM_U, P.t[NS > 1 ? 1 : 0].gx, lane);
-            if constexpr (NS > 2) xm_xpass<RC>(sw, su + 2 * XM_U, P.t[NS > 2 ? 2 : 0].gx, lane);
-            if constexpr (NS > 3) xm_xpass<RD>(sw, su + 3 * XM_U, P.t[NS > 3 ? 3 : 0].gx, lane);
+            xm_xpass<RA, GS>(sw, su, P.t[0].gx, lane);
+            if constexpr (NS > 1) xm_xpass<RB, GS>(sw, su + XM_U, P.t[NS > 1 ? 1 : 0].gx, lane);
+            if constexpr (NS > 2) xm_xpass<RC, GS>(sw, su + 2 * XM_U, P.t[NS > 2 ? 2 : 0].gx, lane);
+            if constexpr (NS > 3) xm_xpass<RD, GS>(sw, su + 3 * XM_U, P.t[NS > 3 ? 3 : 0].gx, lane);
         }
         if (b + 1 < nbatch) prefetch(b + 1);
         __syncthreads();
         // ---- y phase: 8 steps of the march
         const int kbase = ys / 2 + XM_NB * b;      // ys is even
-        const int pi = (tid >> 3) * XM_GP + (tid & 7);
+        const int pi = (tid / GS) * XM_GP + tid % GS;
 #pragma unroll 2
         for (int kk = 0; kk < XM_NB; ++kk) {
             const float2 *su = s_u + (kk * NS) * XM_U + pi;
@@ -265,16 +278,24 @@ __global__ void __launch_bounds__(XM_NT, 2) k_xym(const float *__restrict__ in, 
     }
 }
 
+template <int NS, int RA, int RB, int RC, int RD, bool WGT, int GS>
+cudaError_t launch_xym_g(const float *in, const XymParams &P, cudaStream_t st)
+{
+    using XS = XmShape<GS>;
+    constexpr int SMEM = (XS::NB * XS::SIN + XS::NB * NS * XS::U) * (int)sizeof(float2);
+    cudaError_t e = ensure_dynamic_smem(k_xym<NS, RA, RB, RC, RD, WGT, GS>, SMEM);
+    if (e != cudaSuccess) return e;
+    dim3 grid((P.d.nx + XS::NT - 1) / XS::NT, (P.d.ny + P.ychunk - 1) / P.ychunk, P.d.nz);
+    k_xym<NS, RA, RB, RC, RD, WGT, GS><<<grid, XS::NT, SMEM, st>>>(in, P);
+    return cudaGetLastError();
+}
+
 template <int NS, int RA, int RB, int RC, int RD, bool WGT = false>
 cudaError_t launch_xym(const float *in, const XymParams &P, int sm_count, cudaStream_t st)
 {
-    constexpr int SMEM = (XM_NB * XM_SIN + XM_NB * NS * XM_U) * (int)sizeof(float2);
-    cudaError_t e = ensure_dynamic_smem(k_xym<NS, RA, RB, RC, RD, WGT>, SMEM);
-    if (e != cudaSuccess) return e;
     (void)sm_count;
-    dim3 grid((P.d.nx + XM_NT - 1) / XM_NT, (P.d.ny + P.ychunk - 1) / P.ychunk, P.d.nz);
-    k_xym<NS, RA, RB, RC, RD, WGT><<<grid, XM_NT, SMEM, st>>>(in, P);
-    return cudaGetLastError();
+    if (xm_strip_width(P.d.nx) == 128) return launch_xym_g<NS, RA, RB, RC, RD, WGT, 4>(in, P, st);
+    return launch_xym_g<NS, RA, RB, RC, RD, WGT, 8>(in, P, st);
 }
 
 }  // namespace
@@ -352,7 +373,7 @@ cudaError_t fast_xy_multi(pgsf_plan *p, const int *scales, int n, const float *i
     // rows per CTA: a few waves of CTAs; a chunk start recomputes 16 + 12 rows
     int nch = 1;
     {
-        const long long base = (long long)((d.nx + XM_NT - 1) / XM_NT) * d.nz;
+        const long long base = (long long)((d.nx + xm_strip_width(d.nx) - 1) / xm_strip_width(d.nx)) * d.nz;
         const long long want = 6LL * p->sm_count * 2;
         nch = (int)((want + base - 1) / base);
         const int maxch = (d.ny + 127) / 128;
