@@ -418,6 +418,89 @@ def test_stats_kernel_variants(pg, synth, dims, box):
     assert float(((out[0][3] - out[2][3]).abs() / out[2][3]).max()) <= 1e-4
 
 
+_GUARD = 1 << 16          # bytes of sentinel on either side of a guarded buffer (multiple of 256: keeps the alignment)
+
+
+class _Guarded:
+    """Device buffers cut out of larger ones whose margins hold a sentinel: a kernel that writes outside an output (or
+    outside the workspace the plan declared) changes a margin."""
+
+    def __init__(self, device="cuda"):
+        self.device, self.bufs = device, []
+
+    def make(self, shape, dtype, fill=None):
+        n = int(np.prod(shape)) * torch.empty((), dtype=dtype).element_size()
+        raw = torch.full((n + 2 * _GUARD,), 0xA5, dtype=torch.uint8, device=self.device)
+        self.bufs.append((raw, n))
+        t = raw[_GUARD:_GUARD + n].view(dtype).view(shape)
+        if fill is not None:
+            t.fill_(fill)
+        return t
+
+    def check(self, what):
+        torch.cuda.synchronize()
+        for i, (raw, n) in enumerate(self.bufs):
+            lo, hi = raw[:_GUARD], raw[_GUARD + n:]
+            assert bool((lo == 0xA5).all()) and bool((hi == 0xA5).all()), f"{what}: buffer {i} written outside its bounds"
+
+
+@pytest.mark.parametrize("dims,sigmas,box,flags", [
+    ((67, 45, 70), ((1, 1, 2), (2, 2, 4)), (4, 4, 8), 0),
+    ((36, 201, 33), ((1, 1, 2), (3, 3, 8)), (8, 8, 4), 0),
+    ((300, 37, 41), ((1, 1, 2), (2, 2, 4), (4, 4, 16)), (12, 12, 6), 0),
+    ((131, 52, 64), ((2, 2, 4),), (16, 16, 32), 0),
+    ((70, 33, 60), ((1, 1, 2),), (10, 7, 5), 0),                  # odd box: the generic statistics kernels
+    ((67, 45, 70), ((1, 1, 2), (2, 2, 4)), (4, 4, 8), 1),        # PGSF_FLAG_FORCE_GENERIC
+    ((96, 40, 150), ((1, 1, 8), (2, 2, 16)), (8, 8, 16), 8),     # PGSF_FLAG_TENSOR_ZPASS
+])
+def test_outputs_stay_inside_their_buffers(pg, synth, dims, sigmas, box, flags):
+    """Every output of every entry point, and the workspace, sits between two 64 KiB margins of sentinel bytes; after
+    the calls the margins are untouched (ragged sizes, so that the last strips, chunks and steps of every tiled kernel
+    are partial)."""
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[2], dims, batch=2, n_sources=8), sigmas=sigmas, box_half=box, k=3.0,
+                halo=(2, 3, 4))
+    d = synth.make_workload(w, "cuda")
+    shape = tuple(d.shape)
+    with _plan(pg, w, flags) as plan:
+        g = _Guarded()
+        nws = plan.pgsf_plan_workspace_bytes()
+        if nws:
+            plan._ws = g.make((nws,), torch.uint8)
+        mask = g.make(shape, torch.uint8)
+        count = g.make((1,), torch.int64, 0)
+        filt = [g.make(shape, torch.float32) for _ in sigmas]
+        plan.pgsf_find_multiscale(d, d_filtered=filt, d_mask=mask, d_count=count)
+        g.check("pgsf_find_multiscale")
+        assert int(count.item()) == int(mask.sum())
+        mask2 = g.make(shape, torch.uint8)
+        plan.pgsf_find_multiscale(d, d_mask=mask2, d_count=count)         # no filtered cubes kept: scratch in the workspace
+        g.check("pgsf_find_multiscale without filtered cubes")
+        assert torch.equal(mask, mask2)
+        f0 = g.make(shape, torch.float32)
+        plan.pgsf_filter3d(len(sigmas) - 1, d, d_out=f0)
+        g.check("pgsf_filter3d")
+        if flags & pg.PGSF_FLAG_TENSOR_ZPASS:       # pgsf_filter3d always takes the CUDA-core z pass
+            assert float((f0 - filt[-1]).abs().max()) <= 1e-5 * float(f0.abs().max())
+        else:
+            assert torch.equal(f0, filt[-1])
+        m1 = g.make(shape, torch.uint8, 0)
+        plan.pgsf_local_threshold(f0, d_mask=m1, want_stats=True)
+        plan.pgsf_local_threshold(filt[0], d_mask=m1, or_into=True)
+        g.check("pgsf_local_threshold")
+        labels = g.make(shape, torch.int32)
+        plan.pgsf_label_objects(mask, d_labels=labels)
+        g.check("pgsf_label_objects")
+        wgt = torch.rand_like(d) + 0.5
+        fw = g.make(shape, torch.float32)
+        plan.pgsf_filter3d_weighted(0, d, wgt, 0, d_out=fw)
+        plan.pgsf_filter3d_weighted(0, d, wgt, 1, d_out=fw)
+        g.check("pgsf_filter3d_weighted")
+        fd = g.make(shape, torch.float32)
+        plan.pgsf_filter3d_direct(torch.rand(5, 3, 7, device="cuda"), d, d_out=fd)
+        g.check("pgsf_filter3d_direct")
+
+
 def test_host_entry_point_and_stream(pg, synth):
     dims = (64, 48, 80)
     d = synth.make_cube((dims[2], dims[1], dims[0]), 8, 6, device="cuda")[None]
