@@ -36,6 +36,19 @@ __device__ __forceinline__ void cp_async_wait_all()
     asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
 }
 
+// Compensated s += v by the branch-free two-sum (Knuth): the rounding error of s + v is recovered exactly and gathered
+// in c; the value of the sum is s + c.  Unlike Kahan's form this is exact also when |v| > |s| -- a bright source
+// entering a window of noise.
+__device__ __forceinline__ void twosum_add(float &s, float &c, float v)
+{
+    const float t = s + v;
+    const float bp = t - s;
+    const float da = s - (t - bp);
+    const float db = v - bp;
+    c += da + db;
+    s = t;
+}
+
 // Kahan-compensated s += v (e holds the running low-order error)
 __device__ __forceinline__ void kahan_add(float &s, float &e, float v)
 {

@@ -54,8 +54,8 @@ __global__ void __launch_bounds__(ZB_NT) k_zbox(const float4 *__restrict__ f, fl
         const float a[4] = {v.x - c0, v.y - c0, v.z - c0, v.w - c0};
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-            kahan_add(s1[u], e1[u], a[u]);
-            kahan_add(s2[u], e2[u], a[u] * a[u]);
+            twosum_add(s1[u], e1[u], a[u]);
+            twosum_add(s2[u], e2[u], a[u] * a[u]);
         }
     }
 #pragma unroll 4
@@ -67,16 +67,16 @@ __global__ void __launch_bounds__(ZB_NT) k_zbox(const float4 *__restrict__ f, fl
         const float a[4] = {l.x - c0, l.y - c0, l.z - c0, l.w - c0}, b[4] = {t.x - c0, t.y - c0, t.z - c0, t.w - c0};
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-            kahan_add(s1[u], e1[u], a[u]);
-            kahan_add(s2[u], e2[u], a[u] * a[u]);
+            twosum_add(s1[u], e1[u], a[u]);
+            twosum_add(s2[u], e2[u], a[u] * a[u]);
         }
         const long long o = (long long)zc * plane4 + c;
-        Z1[o] = make_float4(s1[0] - e1[0], s1[1] - e1[1], s1[2] - e1[2], s1[3] - e1[3]);
-        Z2[o] = make_float4(s2[0] - e2[0], s2[1] - e2[1], s2[2] - e2[2], s2[3] - e2[3]);
+        Z1[o] = make_float4(s1[0] + e1[0], s1[1] + e1[1], s1[2] + e1[2], s1[3] + e1[3]);
+        Z2[o] = make_float4(s2[0] + e2[0], s2[1] + e2[1], s2[2] + e2[2], s2[3] + e2[3]);
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-            kahan_add(s1[u], e1[u], -b[u]);
-            kahan_add(s2[u], e2[u], -(b[u] * b[u]));
+            twosum_add(s1[u], e1[u], -b[u]);
+            twosum_add(s2[u], e2[u], -(b[u] * b[u]));
         }
     }
 }

@@ -1,8 +1,8 @@
 // Micro-benchmark behind the "alu" roofline of DESIGN.md section 6 (not part of libpgsf.so):
 //   nvcc -gencode arch=compute_100a,code=sm_100a -O3 -o pgsf_ubench paper_1507_04941_b200/csrc/pgsf_ubench.cu && ./pgsf_ubench
 // Measures, per SM and clock, what the FMA pipe retires for FFMA (scalar), FFMA2 (fma.rn.f32x2 with a uniform
-// multiplier, the inner instruction of the filter kernels), FADD, FADD2 (add.rn.f32x2, the statistics kernels) and
-// what shared memory delivers for LDS.128, with enough independent chains and resident warps to hide latencies.
+// multiplier, the inner instruction of the filter kernels), FADD, FADD2 (add.rn.f32x2, the statistics kernels), DADD / DFMA and
+// the fp32 <-> fp64 conversions (fp64 window sums were considered for the statistics), and what shared memory delivers for LDS.128, with enough independent chains and resident warps to hide latencies.
 #include <cstdio>
 #include <cuda_runtime.h>
 
@@ -31,6 +31,9 @@ __global__ void __launch_bounds__(1024) k_ubench(float *out, float g, long long 
     for (int i = threadIdx.x; i < 256 * 4; i += 1024) sm[i] = (float)i;
     __syncthreads();
     const float2 gg = make_float2(g, g);
+    double dacc[kChains];
+    for (int i = 0; i < kChains; ++i) dacc[i] = threadIdx.x * 1e-3 + i;
+    const double gd = (double)g;
     const long long t0 = clock64();
     for (int it = 0; it < kIters; ++it) {
 #pragma unroll
@@ -39,6 +42,10 @@ __global__ void __launch_bounds__(1024) k_ubench(float *out, float g, long long 
             else if (OP == 1) { acc[i] = ffma2(acc[i], gg, make_float2(1.f, 1.f)); }  // FFMA2
             else if (OP == 2) { acc[i].x = acc[i].x + g; }                            // FADD
             else if (OP == 3) { acc[i] = fadd2(acc[i], gg); }                         // FADD2
+            else if (OP == 5) { dacc[i] = dacc[i] + gd; }                             // DADD
+            else if (OP == 6) { dacc[i] = fma(dacc[i], gd, 1.0); }                    // DFMA
+            else if (OP == 7) { dacc[i] += (double)acc[i].x; acc[i].x += 1.f; }       // F2F.F64.F32 + DADD (+ FADD)
+            else if (OP == 8) { acc[i].x = (float)dacc[i]; dacc[i] += gd; }           // F2F.F32.F64 + DADD
             else {                                                                    // LDS.128
                 float4 v;
                 asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
@@ -49,7 +56,7 @@ __global__ void __launch_bounds__(1024) k_ubench(float *out, float g, long long 
     }
     const long long t1 = clock64();
     float s = 0.f;
-    for (int i = 0; i < kChains; ++i) s += acc[i].x + acc[i].y;
+    for (int i = 0; i < kChains; ++i) s += acc[i].x + acc[i].y + (float)dacc[i];
     out[blockIdx.x * blockDim.x + threadIdx.x] = s;
     if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
 }
@@ -89,5 +96,9 @@ int main()
     run<2>("FADD", 1, "lane-add", p.multiProcessorCount);
     run<3>("FADD2", 2, "lane-add", p.multiProcessorCount);
     run<4>("LDS.128", 16, "bytes", p.multiProcessorCount);
+    run<5>("DADD", 1, "lane-add", p.multiProcessorCount);
+    run<6>("DFMA", 1, "lane-FMA", p.multiProcessorCount);
+    run<7>("F2F64+DADD", 1, "lane-(cvt+add)", p.multiProcessorCount);
+    run<8>("F2F32+DADD", 1, "lane-(cvt+add)", p.multiProcessorCount);
     return 0;
 }

@@ -248,7 +248,7 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
         for (int v = 0; v < CPL; ++v)
             xr[u][v] = ((warp + 4 * u) % RB) * 128 + swz(((warp + 4 * u) / RB) * TPS + CPL * lane + v);
 
-    float2 Y1 = make_float2(0.f, 0.f), Y2 = make_float2(0.f, 0.f), E2 = make_float2(0.f, 0.f);
+    float2 Y1 = make_float2(0.f, 0.f), Y2 = make_float2(0.f, 0.f), E2 = make_float2(0.f, 0.f), E1 = make_float2(0.f, 0.f);
     unsigned my_count = 0;
     const float guard = kFlatGuard, k2 = p.k2;
     const float nyfull = (float)(2 * hy + 1);
@@ -285,11 +285,14 @@ __global__ void __launch_bounds__(128, XYB_MINB) k_xyb(const float *__restrict__
         // ---- y phase
 #pragma unroll
         for (int i = 0; i < RB; ++i) {
-            Y1 = add2(Y1, e1[i]);
+            float2 y1;
+            if constexpr (STATS) { comp_add2(Y1, E1, e1[i]); y1 = add2(Y1, E1); }    // (the mean is an output: 1e-5 sd)
+            else { Y1 = add2(Y1, e1[i]); y1 = Y1; }
             comp_add2(Y2, E2, e2[i]);
             const float2 y2 = add2(Y2, E2);
-            yw[par * (RB * 128) + i * 128] = make_float4(Y1.x, y2.x, Y1.y, y2.y);
-            Y1 = sub2(Y1, l1[i]);                      // the row leaving the window after this output
+            yw[par * (RB * 128) + i * 128] = make_float4(y1.x, y2.x, y1.y, y2.y);
+            if constexpr (STATS) comp_sub2(Y1, E1, l1[i]);
+            else Y1 = sub2(Y1, l1[i]);                 // the row leaving the window after this output
             comp_sub2(Y2, E2, l2[i]);
         }
         if (b + 1 < nb) load_rows(b + 1);              // in flight during the x phase

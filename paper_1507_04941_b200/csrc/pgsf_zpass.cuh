@@ -173,20 +173,15 @@ __device__ __forceinline__ float *window_run(float &s, float &e, float &pb, cons
                                              const float *__restrict__ trail, float *__restrict__ zp, long long plane, int n,
                                              float c0)
 {
-    // pb = the leaving term of the previous output, not yet subtracted: it is combined with the entering term off the
-    // dependent chain, so the running sum sees ONE (compensated) addition per channel instead of two
+    // (s, e): two-sum compensated running sum, value s + e (exact also when a source far brighter than the window's
+    // content enters or leaves); pb = the leaving term of the previous output, subtracted before the entering one
 #pragma unroll 8
     for (int j = 0; j < n; ++j) {
         const float a = lead[j * XT] - c0, b = trail[j * XT] - c0;     // (pivot c0: D-2)
-        if constexpr (SQ) {
-            kahan_add(s, e, a * a - pb);
-            pb = b * b;
-            *zp = s - e;
-        } else {                // sum of f: enters only through the mean, whose tolerance is ~n times looser
-            s += a - pb;
-            pb = b;
-            *zp = s;
-        }
+        twosum_add(s, e, -pb);
+        twosum_add(s, e, SQ ? a * a : a);
+        pb = SQ ? b * b : b;
+        *zp = s + e;
         zp += plane;
     }
     return zp;
@@ -320,11 +315,11 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
                 if (sq) {
                     zp = window_run<true, XT>(s, e, pb, fs + c, ts + c, zp, d.plane, jsplit, c0);
                     window_run<true, XT>(s, e, pb, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit, c0);
-                    kahan_add(s, e, -pb);
+                    twosum_add(s, e, -pb);
                 } else {
                     zp = window_run<false, XT>(s, e, pb, fs + c, ts + c, zp, d.plane, jsplit, c0);
                     window_run<false, XT>(s, e, pb, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit, c0);
-                    s -= pb;
+                    twosum_add(s, e, -pb);
                 }
             } else {
                 for (int j = 0; j < ZB; ++j) {
@@ -332,16 +327,14 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
                     const int zo = zl - hz;
                     if (zl < nz) {
                         const float v = fs[j * XT + c] - c0;
-                        if (sq) kahan_add(s, e, v * v);
-                        else s += v;
+                        twosum_add(s, e, sq ? v * v : v);
                     }
                     if (zo >= 0 && zo < nz) {
-                        Zq[(long long)zo * d.plane + cb] = s - e;
+                        Zq[(long long)zo * d.plane + cb] = s + e;
                         const int jt = j - 2 * hz;  // the channel leaving after this output, relative to z0
                         if (zo - hz >= 0) {         // (a channel in front of the cube never entered the sum)
                             const float v = (jt >= 0 ? fs[jt * XT + c] : ts[j * XT + c]) - c0;
-                            if (sq) kahan_add(s, e, -(v * v));
-                            else s -= v;
+                            twosum_add(s, e, sq ? -(v * v) : -v);
                         }
                     }
                 }
