@@ -46,16 +46,17 @@ __global__ void __launch_bounds__(ZB_NT) k_zbox(const float4 *__restrict__ f, fl
     const int za = chunk * p.zchunk, zb = min(za + p.zchunk, p.d.nz);
     const long long plane4 = p.d.plane / 4;
     const int hz = p.hz, nz = p.d.nz;
-    float s1[4] = {0.f, 0.f, 0.f, 0.f}, e1[4] = {0.f, 0.f, 0.f, 0.f};
-    float s2[4] = {0.f, 0.f, 0.f, 0.f}, e2[4] = {0.f, 0.f, 0.f, 0.f};
+    // fp64 running sums, the arithmetic of k_zm's window phase (pgsf_zpass.cuh: window_run), so that the per-scale call
+    // and pgsf_find_multiscale see the same Z1 / Z2
+    double s1[4] = {0.0, 0.0, 0.0, 0.0}, s2[4] = {0.0, 0.0, 0.0, 0.0};
     // planes za-hz .. za+hz-1 of the first window (clipped to the cube, C-7)
     for (int z = max(za - hz, 0); z < min(za + hz, nz); ++z) {
         const float4 v = __ldg(f + (long long)z * plane4 + c);
-        const float a[4] = {v.x - c0, v.y - c0, v.z - c0, v.w - c0};
+        const double a[4] = {(double)(v.x - c0), (double)(v.y - c0), (double)(v.z - c0), (double)(v.w - c0)};
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-            twosum_add(s1[u], e1[u], a[u]);
-            twosum_add(s2[u], e2[u], a[u] * a[u]);
+            s1[u] += a[u];
+            s2[u] = fma(a[u], a[u], s2[u]);
         }
     }
 #pragma unroll 4
@@ -64,19 +65,20 @@ __global__ void __launch_bounds__(ZB_NT) k_zbox(const float4 *__restrict__ f, fl
         float4 l = make_float4(c0, c0, c0, c0), t = make_float4(c0, c0, c0, c0);
         if (zl < nz) l = __ldg(f + (long long)zl * plane4 + c);
         if (zt >= 0) t = __ldg(f + (long long)zt * plane4 + c);   // leaves after this output
-        const float a[4] = {l.x - c0, l.y - c0, l.z - c0, l.w - c0}, b[4] = {t.x - c0, t.y - c0, t.z - c0, t.w - c0};
+        const double a[4] = {(double)(l.x - c0), (double)(l.y - c0), (double)(l.z - c0), (double)(l.w - c0)};
+        const double b[4] = {(double)(t.x - c0), (double)(t.y - c0), (double)(t.z - c0), (double)(t.w - c0)};
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-            twosum_add(s1[u], e1[u], a[u]);
-            twosum_add(s2[u], e2[u], a[u] * a[u]);
+            s1[u] += a[u];
+            s2[u] = fma(a[u], a[u], s2[u]);
         }
         const long long o = (long long)zc * plane4 + c;
-        Z1[o] = make_float4(s1[0] + e1[0], s1[1] + e1[1], s1[2] + e1[2], s1[3] + e1[3]);
-        Z2[o] = make_float4(s2[0] + e2[0], s2[1] + e2[1], s2[2] + e2[2], s2[3] + e2[3]);
+        Z1[o] = make_float4((float)s1[0], (float)s1[1], (float)s1[2], (float)s1[3]);
+        Z2[o] = make_float4((float)s2[0], (float)s2[1], (float)s2[2], (float)s2[3]);
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-            twosum_add(s1[u], e1[u], -b[u]);
-            twosum_add(s2[u], e2[u], -(b[u] * b[u]));
+            s1[u] -= b[u];
+            s2[u] = fma(-b[u], b[u], s2[u]);
         }
     }
 }

@@ -159,29 +159,33 @@ __global__ void __launch_bounds__(Z_THREADS) k_z(const float *__restrict__ in, f
 //                 entering the window [z - hz, z + hz] comes from the shared-memory slab, the one
 //                 leaving it is re-read from the f this CTA wrote 2 hz + 1 channels earlier -- the
 //                 strip is narrow, so that plane is still in L2 (fetched with the slab by cp.async).
-//                 The running sum of f^2 is Kahan-compensated as in k_zbox; the sum of f is plain (it
-//                 enters only through the mean: a retained rounding error of one column is divided by
-//                 the window's n and stays below 1 % of the mask band).  Writes Z1 = sum f, Z2 = sum f^2
+//                 The running sums are kept in fp64 (see window_run).  Writes Z1 = sum f, Z2 = sum f^2
 //                 (window clipped to the cube, C-7).
 // Against k_z + k_zbox this saves one HBM read of t2's halo, both HBM reads of f by k_zbox and one
 // launch: 8 + 8 + 16 GB instead of 17 + 35 GB per scale at config 3.
 
-// n steps of the sliding window of one (column, quantity; the sum of f^2 Kahan-compensated): add the entering channel, write
-// the window sum, subtract the leaving channel.  lead / trail advance by one staged channel per step.
+// n steps of the sliding window sums of one column, both quantities (sum of f - c0 and of its square), accumulated in
+// fp64 as the paper accumulates ("sums in double"): the squares and the sums of 2 hz + 1 fp32 values are exact to
+// 2^-53, so nothing of a bright source stays behind once it has left the window.  The FP64 pipe (64 lanes per clock and
+// SM on B200, `pgsf_ubench`) is otherwise idle in this kernel; only the fp32 -> fp64 conversions are slow (16 per clock
+// and SM), two per channel and column.  pb1 / pb2 = the leaving terms of the previous output, not yet subtracted: they
+// are combined with the entering terms off the dependent chain (one DADD per channel and quantity on it).
 template <bool SQ, int XT>
-__device__ __forceinline__ float *window_run(float &s, float &e, float &pb, const float *__restrict__ lead,
+__device__ __forceinline__ float *window_run(double &s, double &pb, const float *__restrict__ lead,
                                              const float *__restrict__ trail, float *__restrict__ zp, long long plane, int n,
                                              float c0)
 {
-    // (s, e): two-sum compensated running sum, value s + e (exact also when a source far brighter than the window's
-    // content enters or leaves); pb = the leaving term of the previous output, subtracted before the entering one
 #pragma unroll 8
     for (int j = 0; j < n; ++j) {
-        const float a = lead[j * XT] - c0, b = trail[j * XT] - c0;     // (pivot c0: D-2)
-        twosum_add(s, e, -pb);
-        twosum_add(s, e, SQ ? a * a : a);
-        pb = SQ ? b * b : b;
-        *zp = s + e;
+        const double a = (double)(lead[j * XT] - c0), b = (double)(trail[j * XT] - c0);     // (pivot c0: D-2)
+        if constexpr (SQ) {
+            s += fma(a, a, -pb);
+            pb = b * b;
+        } else {
+            s += a - pb;
+            pb = b;
+        }
+        *zp = (float)s;
         zp += plane;
     }
     return zp;
@@ -232,16 +236,16 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
     const bool c_ok = x0 + c < d.nx && tid < 2 * XT;
     const long long cb = (long long)y * d.nx + x0 + c;
     float *Zq = sq ? Z2 : Z1;
-    float s = 0.f, e = 0.f;
+    double s = 0.0;
     const int nz = d.nz;
     // march steps kbeg .. kend - 1 of the (nz + hz + ZB - 1) / ZB steps of the whole axis (entering channels
     // 0 .. nz + hz - 1; the tail drains the window).  A march cut into sections (pgsf_find_multiscale_host streams the
     // cube through the device) carries the running window sums from one launch to the next in `state`
-    // ([quantity][s, e][row][column]), so that the sections perform exactly the arithmetic of one whole march.
-    float *st_s = nullptr;
+    // (fp64, [quantity][row][column]), so that the sections perform exactly the arithmetic of one whole march.
+    double *st_s = nullptr;
     if (state != nullptr && c_ok) {
-        st_s = state + ((long long)(sq ? 2 : 0) * d.plane + cb);
-        if (kbeg > 0) { s = st_s[0]; e = st_s[d.plane]; }
+        st_s = reinterpret_cast<double *>(state) + (sq ? d.plane : 0) + cb;
+        if (kbeg > 0) s = st_s[0];
     }
     const long long gstep = (long long)S::GROUPS * d.plane;   // staging: a warp group takes every GROUPS-th channel
 
@@ -311,30 +315,29 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
                 // interior step: all 64 entering and all 64 leaving channels (and all 64 outputs) are inside the cube
                 const int jsplit = min(2 * hz, ZB);   // leaving channel: ts[j] for j < jsplit, else fs[j - 2 hz]
                 float *zp = Zq + (long long)(z0 - hz) * d.plane + cb;
-                float pb = 0.f;
+                double pb = 0.0;
                 if (sq) {
-                    zp = window_run<true, XT>(s, e, pb, fs + c, ts + c, zp, d.plane, jsplit, c0);
-                    window_run<true, XT>(s, e, pb, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit, c0);
-                    twosum_add(s, e, -pb);
+                    zp = window_run<true, XT>(s, pb, fs + c, ts + c, zp, d.plane, jsplit, c0);
+                    window_run<true, XT>(s, pb, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit, c0);
                 } else {
-                    zp = window_run<false, XT>(s, e, pb, fs + c, ts + c, zp, d.plane, jsplit, c0);
-                    window_run<false, XT>(s, e, pb, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit, c0);
-                    twosum_add(s, e, -pb);
+                    zp = window_run<false, XT>(s, pb, fs + c, ts + c, zp, d.plane, jsplit, c0);
+                    window_run<false, XT>(s, pb, fs + jsplit * XT + c, fs + c, zp, d.plane, ZB - jsplit, c0);
                 }
+                s -= pb;
             } else {
                 for (int j = 0; j < ZB; ++j) {
                     const int zl = z0 + j;          // channel entering the window of output zo
                     const int zo = zl - hz;
                     if (zl < nz) {
-                        const float v = fs[j * XT + c] - c0;
-                        twosum_add(s, e, sq ? v * v : v);
+                        const double v = (double)(fs[j * XT + c] - c0);
+                        s = sq ? fma(v, v, s) : s + v;
                     }
                     if (zo >= 0 && zo < nz) {
-                        Zq[(long long)zo * d.plane + cb] = s + e;
+                        Zq[(long long)zo * d.plane + cb] = (float)s;
                         const int jt = j - 2 * hz;  // the channel leaving after this output, relative to z0
                         if (zo - hz >= 0) {         // (a channel in front of the cube never entered the sum)
-                            const float v = (jt >= 0 ? fs[jt * XT + c] : ts[j * XT + c]) - c0;
-                            twosum_add(s, e, sq ? -(v * v) : -v);
+                            const double v = (double)((jt >= 0 ? fs[jt * XT + c] : ts[j * XT + c]) - c0);
+                            s = sq ? fma(-v, v, s) : s - v;
                         }
                     }
                 }
@@ -342,7 +345,7 @@ __global__ void __launch_bounds__(ZmShape<RZ, XT, ZB>::THREADS) k_zm(const float
         }
         __syncthreads();   // slabs are overwritten by the next step
     }
-    if (st_s != nullptr) { st_s[0] = s; st_s[d.plane] = e; }
+    if (st_s != nullptr) st_s[0] = s;
 }
 
 template <int RZ>
