@@ -199,7 +199,7 @@ pgsf_status pgsf_plan_create(pgsf_plan **out, const pgsf_plan_desc *desc, int de
     p->h_stream = nullptr;
     p->hs = nullptr;
     p->tensor_z = false;
-    for (int s = 0; s < PGSF_MAX_SCALES; ++s) p->d_tc_strips[s] = nullptr;
+    for (int s = 0; s < PGSF_MAX_SCALES; ++s) { p->d_tc_strips[s] = nullptr; p->tc_march[s] = 0; }
     for (int s = 0; s < PGSF_MAX_SCALES; ++s) p->h_d_f[s] = nullptr;
 
     const bool force_generic = (desc->flags & PGSF_FLAG_FORCE_GENERIC) != 0;

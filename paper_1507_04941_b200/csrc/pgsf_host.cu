@@ -94,6 +94,7 @@ pgsf_status stage_create(pgsf_plan *p)
     for (int s = 0; s < S; ++s) {
         rmax = std::max(rmax, p->scales[s].rz_c);
         zb = std::max(zb, zm_step_channels_of(p->scales[s].rz_c));
+        zb = std::max(zb, ztc_step_channels(p, s));      // (PGSF_FLAG_TENSOR_ZPASS: 128-channel steps)
     }
     // a section must be a whole number of march steps and at least as long as what is rolled over to the next one
     const int keep = std::max(std::max(2 * rmax, 2 * hz), zb);

@@ -110,6 +110,7 @@ struct pgsf_plan {
     struct pgsf_host_stage *hs;          // streamed sections (pgsf_host.cu)
     bool tensor_z;                       // PGSF_FLAG_TENSOR_ZPASS: k_ztc for compiled z radii >= 24 (pgsf_ztc.cu)
     float *d_tc_strips[PGSF_MAX_SCALES]; // its band-matrix operands
+    int tc_march[PGSF_MAX_SCALES];       // kernel of the march in progress (sections): 0 none yet, 1 k_ztc, 2 k_zm
 };
 
 namespace pgsf {
@@ -162,6 +163,8 @@ constexpr int zm_step_rule(int rz_compiled) { return (rz_compiled >= 96 || rz_co
 int zm_step_channels_of(int rz_compiled);
 // the tensor-core variant of fast_zm (pgsf_ztc.cu): cudaErrorNotSupported = not for this plan / scale, run fast_zm
 bool ztc_radius(int rz_compiled);
+// channels per march step of the tensor-core z pass if `scale` runs on it in this plan, else 0
+int ztc_step_channels(const pgsf_plan *p, int scale);
 cudaError_t ztc_prepare(pgsf_plan *p);
 void ztc_release(pgsf_plan *p);
 cudaError_t fast_ztc(pgsf_plan *p, int scale, const float *in, float *out, float *Z1, float *Z2, int ncubes,

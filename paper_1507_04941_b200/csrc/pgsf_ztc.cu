@@ -510,6 +510,11 @@ static float host_rna_tf32(float x)
 
 bool ztc_radius(int rz_c) { return rz_c >= 24 && rz_c % 4 == 0; }
 
+int ztc_step_channels(const pgsf_plan *p, int scale)
+{
+    return (p->tensor_z && p->d_tc_strips[scale] != nullptr && ztc_radius(p->scales[scale].rz_c)) ? TC_ZB : 0;
+}
+
 // The band-matrix strips of every scale the variant serves: S[t][r][j] = h[4 t + r + j], h[u] = g[u - 127],
 // g[0 .. 2 RZ] the taps centred in the compiled window; hi part, then lo part.
 cudaError_t ztc_prepare(pgsf_plan *p)
@@ -562,10 +567,13 @@ cudaError_t fast_ztc(pgsf_plan *p, int scale, const float *in, float *out, float
     alignas(64) CUtensorMap map;
     bool ok;
     if (sec != nullptr) {
-        if (sec->c0 % TC_ZB != 0 || (sec->c1 % TC_ZB != 0 && sec->c1 < (1 << 29))) return cudaErrorNotSupported;
+        // (pgsf_host.cu sizes its sections in whole steps of every scale's kernel: a section that is not must fail, not
+        // fall back to k_zm -- the sections of one march would then mix the carried states of two kernels)
+        if (sec->c0 % TC_ZB != 0 || (sec->c1 % TC_ZB != 0 && sec->c1 < (1 << 29))) return cudaErrorInvalidValue;
         zp.kbeg = sec->c0 / TC_ZB;
         zp.kend = sec->c1 / TC_ZB < nsteps ? sec->c1 / TC_ZB : nsteps;
         state = sec->state;
+        if (zp.kbeg > 0 && p->tc_march[scale] == 2) return cudaErrorNotSupported;   // the march began on k_zm: stay there
         if (zp.kbeg >= zp.kend) return cudaSuccess;
         const int lo = sec->t2_base > 0 ? sec->t2_base : 0, hi = sec->t2_hi < d.nz ? sec->t2_hi : d.nz;
         zp.zmap_lo = lo;
@@ -575,7 +583,12 @@ cudaError_t fast_ztc(pgsf_plan *p, int scale, const float *in, float *out, float
     } else {
         ok = make_slab_map(&map, in, d.nx, d.ny, d.nz, ncubes, TC_XT, zp.K / zp.nbox, true);
     }
-    if (!ok) return cudaErrorNotSupported;
+    if (!ok) {     // no tensor map (nx % 4 != 0, no driver entry point): k_zm -- but never in the middle of a march
+        if (sec != nullptr && zp.kbeg > 0) return cudaErrorInvalidValue;
+        p->tc_march[scale] = 2;
+        return cudaErrorNotSupported;
+    }
+    p->tc_march[scale] = 1;
     const int T = zp.K / 4 + 30;
     const int smem2 = (2 * zp.K * T2_XT + 2 * TC_ZB * T2_XT + 2 * T * 32) * (int)sizeof(float);
     if (smem2 <= 227 * 1024 && !(p->tune & 32)) {          // 64 columns per CTA, two warp groups (PGSF_OPT_TUNE bit 5: k_ztc)

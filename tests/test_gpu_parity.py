@@ -596,6 +596,30 @@ def test_tensor_core_z_pass(pg, synth, oracle, dims, sigmas, box):
     assert hcount == int(c_tc.item()) and torch.equal(h_mask, m_tc.cpu())
 
 
+@pytest.mark.parametrize("dims,sigmas,box,batch,halo,k,n_sources,seed,section", [
+    ((132, 47, 115), ((1, 1, 8),), (4, 6, 30), 1, (3, 1, 1), 2.5, 3, 14027, 64),
+    ((36, 37, 55), ((3, 1, 4), (1, 3, 8)), (16, 4, 20), 1, (0, 0, 0), 3.0, 7, 21047, 0),
+    ((64, 62, 140), ((3, 3, 1), (1, 1, 8)), (8, 3, 10), 2, (0, 0, 0), 2.5, 7, 21049, 64),
+])
+def test_tensor_core_z_pass_streamed_sections(pg, synth, dims, sigmas, box, batch, halo, k, n_sources, seed, section):
+    """The streamed host entry point with PGSF_FLAG_TENSOR_ZPASS when the requested (or automatic) section is not a
+    whole number of the tensor kernel's 128-channel steps: sections are sized in whole steps of EVERY scale's z kernel,
+    so the march of a scale never changes kernel (and carried state) from one section to the next.  Found by a
+    randomised sweep: with 64-channel sections the last section ran k_ztc on the window state k_zm had left
+    (counts 18453 against 3106), or the streamed call ran k_zm where the resident one ran k_ztc."""
+    from dataclasses import replace
+    w = replace(synth.scaled(synth.WORKLOADS[2], dims, batch=batch, n_sources=n_sources), sigmas=sigmas, box_half=box,
+                k=k, halo=halo, seed=seed)
+    d = synth.make_workload(w, "cuda")
+    with _plan(pg, w, pg.PGSF_FLAG_TENSOR_ZPASS) as plan:
+        mask, cnt, filt = plan.pgsf_find_multiscale(d, keep_filtered=True)
+        torch.cuda.synchronize()
+    h_mask, count, hf = _host_run(pg, w, d.cpu().pin_memory(), section=section, keep=True, flags=pg.PGSF_FLAG_TENSOR_ZPASS)
+    assert count == int(cnt.item()) and torch.equal(h_mask, mask.cpu())
+    for s in range(len(sigmas)):
+        assert torch.equal(hf[s], filt[s].cpu()), f"filtered cube {s} differs"
+
+
 def test_tensor_core_z_pass_batch(pg, synth, oracle):
     """The variant on a batch with halo (several cubes per launch: the TMA map has a cube dimension, out-of-cube
     channels of one cube must be zeros, not the neighbour cube's planes) and with PGSF_OPT_TUNE bit 5 (the 32-column
