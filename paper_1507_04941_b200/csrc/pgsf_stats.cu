@@ -5,9 +5,9 @@
 //   k_zbox    frequency direction first.  Every thread owns four adjacent (x, y) columns and marches
 //             along z with the window sums  Z1 = sum_{|o|<=hz} f(z+o),  Z2 = sum f(z+o)^2  in registers:
 //             the plane entering the window is added, the plane leaving it subtracted (both read from
-//             HBM; nothing is staged).  The running sums are Kahan-compensated: a bright source is
-//             > 10^3 x the filtered noise in f^2, and an uncompensated fp32 running sum would keep the
-//             rounding error made while the source was inside the window long after it has left.
+//             HBM; nothing is staged).  The running sums are fp64 ("sums in double"): a bright source is
+//             > 10^3 x the filtered noise in f^2, and an fp32 running sum would keep the rounding error made
+//             while the source was inside the window long after it has left.
 //             Writes Z1, Z2 (two workspace cubes).
 //   k_ymarch  per z plane: y-direction window sums marched in registers, x-direction window from the
 //             prefix / suffix sums of thread-owned column groups, then m = S1/n, var = S2/n - m^2,
