@@ -249,6 +249,29 @@ PGSF_API pgsf_status pgsf_find_multiscale_host(pgsf_plan *plan, const float *h_i
 PGSF_API pgsf_status pgsf_label_objects(pgsf_plan *plan, const uint8_t *d_mask, uint32_t *d_labels,
                                unsigned long long *d_count, void *cuda_stream);
 
+/*
+ * pgsf_filter3d_noalloc -- pgsf_filter3d (Eq. 2; Eq. 3-5; readings C-1 .. C-5) of ONE cube for callers
+ * that cannot allocate device memory: code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc.  No plan, no workspace: the two intermediate cubes of the three 1-D passes live in a static device
+ * array of 2 x PGSF_NOALLOC_MAX_VOXELS floats (16 MiB, held by every GPU that loads the library until the process
+ * exits).  The call makes no cudaMalloc / cudaFree and calls no allocating library routine; it runs the arithmetic
+ * of the generic kernels on the CURRENT device and enqueues three kernels on `cuda_stream`.
+ * d_in, d_out: DEVICE, nx*ny*nz floats (x fastest), 4-byte aligned, must not overlap; caller owned.
+ * sigma_xyz: HOST, 3 doubles >= 0; radius = ceil(truncate * sigma) <= PGSF_MAX_RADIUS, taps as pgsf_plan_create.
+ * err_text (nullable): HOST buffer of err_cap chars that receives the text of an error ("" on success).
+ * Errors: INVALID_ARG (null / misaligned / overlapping pointer, extent < 1, sigma < 0, truncate <= 0); UNSUPPORTED
+ * when nx*ny*nz > PGSF_NOALLOC_MAX_VOXELS (the text names both numbers), a radius is above PGSF_MAX_RADIUS or the
+ * device is not sm_100; CUDA when a runtime call fails.
+ * The scratch is SHARED by every call on a device and keeps the previous call's contents (nothing in it needs to
+ * start at zero: every pass writes its whole output before the next one reads it).  Calls whose kernels may overlap
+ * on the GPU -- different streams, different host threads -- race on it: serialise them.  The first call on a
+ * device looks the array's device address up (cudaGetSymbolAddress); make one call before starting a graph capture.
+ */
+#define PGSF_NOALLOC_MAX_VOXELS (1 << 21)
+PGSF_API pgsf_status pgsf_filter3d_noalloc(const float *d_in, float *d_out, int nx, int ny, int nz,
+                                  const double *sigma_xyz, double truncate, void *cuda_stream, char *err_text,
+                                  int err_cap);
+
 /* Number of kernels this library has launched on behalf of `plan` since creation (bench.py's
  * gpu_launches evidence). */
 PGSF_API unsigned long long pgsf_plan_launch_count(const pgsf_plan *plan);

@@ -31,7 +31,7 @@ _STATUS = {0: "PGSF_OK", 1: "PGSF_ERR_INVALID_ARG", 2: "PGSF_ERR_UNSUPPORTED", 3
 EXPORTS = ["pgsf_plan_create", "pgsf_plan_destroy", "pgsf_plan_set_option", "pgsf_plan_path",
            "pgsf_plan_workspace_bytes", "pgsf_last_error",
            "pgsf_plan_get_taps", "pgsf_filter3d", "pgsf_filter3d_weighted", "pgsf_filter3d_direct", "pgsf_local_threshold", "pgsf_find_multiscale",
-           "pgsf_find_multiscale_host", "pgsf_label_objects", "pgsf_plan_launch_count", "pgsf_plan_set_profiling",
+           "pgsf_find_multiscale_host", "pgsf_label_objects", "pgsf_filter3d_noalloc", "pgsf_plan_launch_count", "pgsf_plan_set_profiling",
            "pgsf_plan_profile_collect", "pgsf_plan_profile_entry"]
 
 
@@ -83,6 +83,9 @@ def load_library() -> ctypes.CDLL:
         lib.pgsf_filter3d_direct.restype = i
         lib.pgsf_label_objects.argtypes = [vp, vp, vp, vp, vp]
         lib.pgsf_label_objects.restype = i
+        lib.pgsf_filter3d_noalloc.argtypes = [vp, vp, i, i, i, ctypes.POINTER(ctypes.c_double), ctypes.c_double, vp,
+                                              ctypes.c_char_p, i]
+        lib.pgsf_filter3d_noalloc.restype = i
         lib.pgsf_local_threshold.argtypes = [vp, vp, vp, i, vp, vp, vp, vp, vp]
         lib.pgsf_local_threshold.restype = i
         lib.pgsf_find_multiscale.argtypes = [vp, vp, ctypes.POINTER(vp), vp, vp, vp, vp]
@@ -332,3 +335,29 @@ class Plan:
         self._check(self._lib.pgsf_find_multiscale_host(self._h, _ptr(h_in), arr, _ptr(h_mask),
                                                         ctypes.byref(cnt)))
         return h_mask, int(cnt.value)
+
+
+PGSF_NOALLOC_MAX_VOXELS = 1 << 21
+
+
+def pgsf_filter3d_noalloc(d_in: torch.Tensor, sigma_xyz: Sequence[float], truncate: float = 3.0,
+                          d_out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """pgsf_filter3d for one cube [nz, ny, nx] without a plan or workspace: the library's static device scratch holds
+    the intermediates (at most PGSF_NOALLOC_MAX_VOXELS voxels; calls on one device must not overlap on the GPU).
+    The library call itself allocates nothing; pass d_out to keep this wrapper from allocating the output."""
+    lib = load_library()
+    if not d_in.is_cuda or d_in.dtype != torch.float32 or d_in.dim() != 3 or not d_in.is_contiguous():
+        raise ValueError("d_in: need a contiguous cuda float32 tensor [nz, ny, nx]")
+    if d_out is None:
+        d_out = torch.empty_like(d_in)
+    if d_out.shape != d_in.shape or d_out.dtype != torch.float32 or not d_out.is_contiguous() or d_out.device != d_in.device:
+        raise ValueError("d_out: need a contiguous cuda float32 tensor of d_in's shape on its device")
+    nz, ny, nx = d_in.shape
+    sig = (ctypes.c_double * 3)(*[float(s) for s in sigma_xyz])
+    err = ctypes.create_string_buffer(384)
+    with torch.cuda.device(d_in.device):
+        st = lib.pgsf_filter3d_noalloc(_ptr(d_in), _ptr(d_out), nx, ny, nz, sig, float(truncate), _stream_ptr(stream),
+                                       err, len(err))
+    if st != PGSF_OK:
+        raise PgsfError(st, err.value.decode())
+    return d_out

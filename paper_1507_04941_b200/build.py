@@ -12,7 +12,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpgsf.so")
 SOURCES = ["pgsf_z_r96.cu", "pgsf_z_r72.cu", "pgsf_z_r48.cu", "pgsf_z_r24.cu", "pgsf_z_r12.cu", "pgsf_z_r6.cu",
-           "pgsf_api.cu", "pgsf_host.cu", "pgsf_generic.cu", "pgsf_filter.cu", "pgsf_stats.cu", "pgsf_xyb.cu", "pgsf_label.cu", "pgsf_ztc.cu", "pgsf_weighted.cu", "pgsf_direct.cu"]
+           "pgsf_api.cu", "pgsf_host.cu", "pgsf_generic.cu", "pgsf_filter.cu", "pgsf_stats.cu", "pgsf_xyb.cu", "pgsf_label.cu", "pgsf_ztc.cu", "pgsf_weighted.cu", "pgsf_direct.cu", "pgsf_noalloc.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--use_fast_math=false",
